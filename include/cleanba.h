@@ -1,0 +1,148 @@
+/* =============================================================================================
+ * cleanba.h -- C ABI of the B200-native hot path of Cleanba's actor-learner method
+ * (arXiv 2310.00036).  Citations are PAPER.md:<line> or a reading "A<n>" of DESIGN.md section 3.
+ *
+ * The path (Algorithm 1): batched policy/value inference on stacked
+ * 84x84x4 uint8 frames with categorical sampling (l.8), and the learner step (l.11-20): network
+ * forward, V-trace or GAE targets, IMPALA or clipped-PPO loss (Eq. 2-3),
+ * backward, global grad-norm clip and Adam.
+ *
+ * Conventions for EVERY entry point:
+ *   - "dev" pointers are CUDA device pointers, "host" pointers are host pointers.  The caller
+ *     owns every buffer it passes; the library owns only the workspace inside cb_net.
+ *   - All arrays are dense row-major, last index fastest; trajectories are time-major [T,B,...]
+ *     exactly as the paper stores D.
+ *   - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default
+ *     stream).  No call synchronises the device except where stated (workspace growth).
+ *   - Return value: 0 (CB_OK) or a negative code; cb_last_error() gives the text of the last
+ *     failure on the calling thread.  Nothing aborts or throws.
+ *   - Determinism (A16): identical inputs give bitwise identical outputs (fixed-order
+ *     reductions, no floating-point atomics).
+ * ============================================================================================= */
+#ifndef CLEANBA_H_
+#define CLEANBA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { CB_OK = 0, CB_EINVAL = -1, CB_ENOMEM = -2, CB_ECUDA = -3 };
+enum { CB_ARCH_NATURE = 0, CB_ARCH_IMPALA = 1 };
+enum { CB_PREC_FP32_REF = 0, CB_PREC_BF16_TC = 1 };
+enum { CB_ALGO_IMPALA = 0, CB_ALGO_PPO = 1 };
+/* stats record per gradient update: loss, pg_loss, v_loss, entropy, grad_norm (pre-clip),
+ * approx_kl, clip_frac (PPO), mean_rho (IMPALA); unused fields are 0. */
+enum { CB_N_STATS = 8 };
+
+/* Network description.  kind 0 = Nature-CNN (BASELINE.json configs[0]): conv 8x8s4, 4x4s2,
+ * 3x3s1 (VALID), fc, heads.  kind 1 = IMPALA-ResNet: 3 x [conv3x3 pad 1,
+ * max-pool 3x3 s2 SAME (A10), 2 residual blocks], ReLU, fc, ReLU, policy + value heads.
+ * Input is in_c x in_h x in_w uint8 (4 x 84 x 84). */
+typedef struct {
+  int kind;
+  int in_c, in_h, in_w;
+  int channels[3];
+  int fc;
+  int n_actions; /* 18 */
+} cb_arch;
+
+/* Hyper-parameters of one learner call (Tables 2-3; A12 for Adam). */
+typedef struct {
+  int algo;      /* CB_ALGO_* */
+  int precision; /* CB_PREC_* */
+  int T, B;      /* unroll length, envs */
+  float gamma, lambda_;             /* V-trace lambda (1) or GAE lambda (0.95) */
+  float rho_bar, c_bar, rho_pg_bar; /* IMPALA */
+  float clip_eps;                   /* PPO */
+  int epochs, minibatches, norm_adv; /* PPO */
+  uint64_t perm_seed;               /* PPO minibatch permutation (A17) */
+  float vf_coef, ent_coef;          /* c1, c2 */
+  float lr, beta1, beta2, adam_eps, max_grad_norm;
+  int loss_reduction;               /* 0 = mean over samples, 1 = sum (A4) */
+} cb_hparams;
+
+typedef struct cb_net cb_net; /* opaque: layer table, parameter offsets, device workspaces */
+
+/* ---- lifetime -------------------------------------------------------------------------- */
+/* Builds the layer table for `arch`.  max_frames is a hint: the device workspace for
+ * `max_frames` frames is allocated lazily (cudaMalloc) on the first forward/learner call in a
+ * given precision and grown if a later call needs more (growth synchronises the device).
+ * Needs no GPU.  *out is NULL on failure. */
+int cb_net_create(const cb_arch* arch, int max_frames, cb_net** out);
+void cb_net_destroy(cb_net* net);
+
+/* P = number of fp32 parameters.  Canonical flat order: layer order, weight
+ * then bias; conv weights [Cout,Cin,kh,kw]; fc weights [out,in] with `in` flattened (C,H,W);
+ * then pi.w [A,fc], pi.b [A], v.w [fc], v.b [1]. */
+size_t cb_param_count(const cb_net* net);
+/* Tensor i of that order: name (static string), offset in elements, rank and dims (<= 4).
+ * Returns CB_EINVAL past the last tensor. */
+int cb_param_layout(const cb_net* net, int i, const char** name, size_t* offset, int* rank, int dims[4]);
+
+/* He-normal initialisation on the HOST (A14): weights N(0, 2/fan_in), biases 0, Philox4x32-10 +
+ * Box-Muller in fp64; deterministic in `seed`.  params_host: host [P], written. */
+int cb_net_init(const cb_net* net, uint64_t seed, float* params_host);
+
+/* ---- actor side (Alg. 1 l.8) ------------------------------------------------ */
+/* logits, value = net(obs);  actions[b] = argmax_i(logits[b,i] + Gumbel_i), the Gumbel noise
+ * from Philox4x32-10 with key = seed and counter = (env_offset + b, step_lo, step_hi, i/4), word
+ * i%4 (A9).  params: dev [P] fp32.  obs: dev uint8 [B,in_c,in_h,in_w].  precision: CB_PREC_*.
+ * Outputs (dev): logits fp32 [B,A], value fp32 [B], actions int32 [B]; any may be NULL. */
+int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int B, uint64_t seed,
+                      uint64_t step, uint32_t env_offset, int precision, float* logits, float* value,
+                      int32_t* actions, void* stream);
+
+/* ---- learner side (Alg. 1 l.11-20) -------------------------------------- */
+/* One learner call: IMPALA = one V-trace gradient update; PPO = GAE, then epochs x minibatches
+ * updates over a seeded permutation.  Updated in place (dev fp32 [P]): params, adam_m, adam_v.
+ * opt_step: host counter, incremented once per gradient update (Adam's k, from 1).
+ * obs: dev uint8 [T+1,B,in_c,in_h,in_w]; actions: dev int32 [T,B]; rewards: dev fp32 [T,B];
+ * dones: dev uint8 [T,B], 1 <=> the step taken at t ended the episode (A1);
+ * behaviour_logits: dev fp32 [T,B,A].  stats: dev fp32 [n_updates, CB_N_STATS], written.
+ * Returns the number of gradient updates done (> 0) or a negative error. */
+int cb_learner_step(cb_net* net, float* params, float* adam_m, float* adam_v, uint64_t* opt_step,
+                    const uint8_t* obs, const int32_t* actions, const float* rewards,
+                    const uint8_t* dones, const float* behaviour_logits, const cb_hparams* hp,
+                    float* stats, void* stream);
+
+/* Device pointers to the library-owned results of the LAST cb_learner_step (valid until the next
+ * call on this net): which = 0: forward logits fp32 [(T+1)B, A+1] (column A is the value), from the
+ * first forward; 1: vs (IMPALA) or advantages (PPO) fp32 [T,B]; 2: pg advantages (IMPALA) or returns
+ * (PPO) fp32 [T,B]; 3: gradient of the last update before clipping, fp32 [P]. */
+int cb_learner_view(const cb_net* net, int which, const void** dev_ptr, size_t* count);
+
+/* ---- the path's sub-steps, exposed one by one (all dev pointers, fp32 unless noted) -------- */
+/* A9: Gumbel-max sampling from given logits [B,A] -> actions int32 [B]. */
+int cb_sample_actions(const float* logits, int B, int A, uint64_t seed, uint64_t step,
+                      uint32_t env_offset, int32_t* actions, void* stream);
+/* O2: log-softmax of logits [N, ld] (first A columns) -> logp_a [N] = log pi(actions[n]), entropy [N]
+ * (nullable). */
+int cb_logprob_entropy(const float* logits, int ld, int N, int A, const int32_t* actions, float* logp_a,
+                       float* entropy, void* stream);
+/* O4 V-trace (A2): V [T+1,B]; r, logpi, logmu [T,B]; d uint8 [T,B] -> vs, pgadv, rho [T,B]
+ * (rho nullable).  One lane per env, reverse-time scan. */
+int cb_vtrace(int T, int B, const float* V, const float* r, const uint8_t* d, const float* logpi,
+              const float* logmu, float gamma, float lambda_, float rho_bar, float c_bar,
+              float rho_pg_bar, float* vs, float* pgadv, float* rho, void* stream);
+/* O6 GAE (A3): -> adv, ret [T,B]. */
+int cb_gae(int T, int B, const float* V, const float* r, const uint8_t* d, float gamma, float lambda_,
+           float* adv, float* ret, void* stream);
+/* A17: Fisher-Yates permutation of N indices for (seed, epoch) -> perm int32 [N]. */
+int cb_permutation(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* stream);
+/* O9 (A12, A13): global-norm clip + Adam over flat fp32 buffers of P elements (16-byte aligned);
+ * k = update count (from 1).  grad_norm: dev fp32 [1], written (pre-clip norm; nullable).
+ * scratch: dev, at least cb_clip_adam_scratch_bytes(P) bytes. */
+size_t cb_clip_adam_scratch_bytes(size_t P);
+int cb_clip_adam(size_t P, float* params, float* adam_m, float* adam_v, const float* grad, uint64_t k,
+                 float lr, float beta1, float beta2, float eps, float max_norm, float* grad_norm,
+                 void* scratch, void* stream);
+
+const char* cb_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CLEANBA_H_ */

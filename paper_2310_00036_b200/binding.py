@@ -1,0 +1,242 @@
+"""Thin ctypes binding over the C-ABI CUDA library (include/cleanba.h).  Argument marshalling
+only: every step of the path runs in the library's kernels.  torch is used for device memory and
+streams.  There is NO CPU fallback: a missing library or a missing GPU raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from .synth import ArchSpec
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libcleanba.so")
+N_STATS = 8
+STAT_NAMES = ("loss", "pg_loss", "v_loss", "entropy", "grad_norm", "approx_kl", "clip_frac", "mean_rho")
+PREC = {"fp32": 0, "bf16": 1}
+ALGO = {"impala": 0, "ppo": 1}
+
+EXPORTS = ["cb_net_create", "cb_net_destroy", "cb_param_count", "cb_param_layout", "cb_net_init", "cb_policy_forward",
+           "cb_learner_step", "cb_learner_view", "cb_sample_actions", "cb_logprob_entropy", "cb_vtrace", "cb_gae",
+           "cb_permutation", "cb_clip_adam_scratch_bytes", "cb_clip_adam", "cb_last_error"]
+
+
+class CArch(C.Structure):
+    _fields_ = [("kind", C.c_int), ("in_c", C.c_int), ("in_h", C.c_int), ("in_w", C.c_int),
+                ("channels", C.c_int * 3), ("fc", C.c_int), ("n_actions", C.c_int)]
+
+
+class CHParams(C.Structure):
+    _fields_ = [("algo", C.c_int), ("precision", C.c_int), ("T", C.c_int), ("B", C.c_int),
+                ("gamma", C.c_float), ("lambda_", C.c_float),
+                ("rho_bar", C.c_float), ("c_bar", C.c_float), ("rho_pg_bar", C.c_float),
+                ("clip_eps", C.c_float), ("epochs", C.c_int), ("minibatches", C.c_int), ("norm_adv", C.c_int),
+                ("perm_seed", C.c_uint64),
+                ("vf_coef", C.c_float), ("ent_coef", C.c_float),
+                ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("adam_eps", C.c_float),
+                ("max_grad_norm", C.c_float), ("loss_reduction", C.c_int)]
+
+
+class CleanbaError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Loads libcleanba.so (built in-tree by paper_2310_00036_b200/build.py).  Raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise CleanbaError(f"{_SO} is missing: run `python -m paper_2310_00036_b200.build` (no CPU fallback exists)")
+        L = C.CDLL(_SO)
+        L.cb_param_count.restype = C.c_size_t
+        L.cb_clip_adam_scratch_bytes.restype = C.c_size_t
+        L.cb_clip_adam_scratch_bytes.argtypes = [C.c_size_t]
+        L.cb_last_error.restype = C.c_char_p
+        L.cb_net_destroy.restype = None
+        L.cb_net_destroy.argtypes = [C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc < 0:
+        raise CleanbaError(f"cleanba error {rc}: {lib().cb_last_error().decode()}")
+    return rc
+
+
+def make_hparams(algo="impala", precision="bf16", T=20, B=128, **kw):
+    """Defaults: Table 3 (IMPALA) / Table 2 (PPO); Adam for both (A12)."""
+    h = CHParams(); ppo = algo in ("ppo", 1)
+    h.algo = 1 if ppo else 0; h.precision = PREC.get(precision, precision); h.T = T; h.B = B
+    h.gamma = 0.99; h.lambda_ = 0.95 if ppo else 1.0
+    h.rho_bar = h.c_bar = h.rho_pg_bar = 1.0
+    h.clip_eps = 0.1; h.epochs = 4; h.minibatches = 4; h.norm_adv = 1; h.perm_seed = 1
+    h.vf_coef = 0.5; h.ent_coef = 0.01
+    h.lr = 2.5e-4 if ppo else 6e-4; h.beta1 = 0.9; h.beta2 = 0.999; h.adam_eps = 1e-5
+    h.max_grad_norm = 0.5 if ppo else 40.0; h.loss_reduction = 0
+    for k, v in kw.items():
+        if not hasattr(h, k):
+            raise KeyError(k)
+        setattr(h, k, v)
+    return h
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise CleanbaError("no CUDA device: the Cleanba hot path has no CPU fallback")
+    return torch
+
+
+def _ptr(t):
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t, dtype, name):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise CleanbaError(f"{name} must be a contiguous CUDA tensor of dtype {dtype}")
+    return t
+
+
+class Net:
+    """cb_net handle.  Creating it and cb_net_init need no GPU; everything else does."""
+
+    def __init__(self, arch: ArchSpec, max_frames=0):
+        a = CArch(); a.kind = {"nature": 0, "impala": 1}[arch.kind]
+        a.in_c, a.in_h, a.in_w = arch.in_c, arch.in_h, arch.in_w
+        a.channels[:] = list(arch.channels); a.fc = arch.fc; a.n_actions = arch.n_actions
+        self.arch = arch; self._h = C.c_void_p()
+        _check(lib().cb_net_create(C.byref(a), C.c_int(max_frames), C.byref(self._h)))
+        self.P = int(lib().cb_param_count(self._h)); self.A = arch.n_actions
+
+    def close(self):
+        if self._h:
+            lib().cb_net_destroy(self._h); self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def param_layout(self):
+        """[(name, offset, dims)] in canonical order."""
+        out, i = [], 0
+        name = C.c_char_p(); off = C.c_size_t(); rank = C.c_int(); dims = (C.c_int * 4)()
+        while lib().cb_param_layout(self._h, C.c_int(i), C.byref(name), C.byref(off), C.byref(rank), dims) == 0:
+            out.append((name.value.decode(), off.value, tuple(dims[:rank.value]))); i += 1
+        return out
+
+    def init_params(self, seed):
+        """cb_net_init: host He-normal init -> numpy fp32 [P]."""
+        p = np.empty(self.P, np.float32)
+        _check(lib().cb_net_init(self._h, C.c_uint64(seed), p.ctypes.data_as(C.c_void_p)))
+        return p
+
+    def policy_forward(self, params, obs, seed=0, step=0, env_offset=0, precision="bf16", want_actions=True):
+        """cb_policy_forward on the current torch stream.  params: cuda fp32 [P]; obs: cuda uint8 [B,C,H,W].
+        Returns (logits [B,A], value [B], actions int32 [B])."""
+        torch = _torch()
+        _dev(params, torch.float32, "params"); _dev(obs, torch.uint8, "obs")
+        B = obs.shape[0]
+        logits = torch.empty((B, self.A), dtype=torch.float32, device=obs.device)
+        value = torch.empty((B,), dtype=torch.float32, device=obs.device)
+        actions = torch.empty((B,), dtype=torch.int32, device=obs.device) if want_actions else None
+        _check(lib().cb_policy_forward(self._h, _ptr(params), _ptr(obs), C.c_int(B), C.c_uint64(seed), C.c_uint64(step),
+                                       C.c_uint32(env_offset), C.c_int(PREC.get(precision, precision)), _ptr(logits), _ptr(value),
+                                       _ptr(actions), _stream()))
+        return logits, value, actions
+
+    def learner_step(self, params, adam_m, adam_v, opt_step, obs, actions, rewards, dones, behaviour_logits, hp, stats=None):
+        """cb_learner_step on the current torch stream; params/adam_m/adam_v are updated in place.
+        Returns (new opt_step, stats tensor [n_updates, 8])."""
+        torch = _torch()
+        for t, n in ((params, "params"), (adam_m, "adam_m"), (adam_v, "adam_v"), (rewards, "rewards"), (behaviour_logits, "behaviour_logits")):
+            _dev(t, torch.float32, n)
+        _dev(obs, torch.uint8, "obs"); _dev(dones, torch.uint8, "dones"); _dev(actions, torch.int32, "actions")
+        n_upd = hp.epochs * hp.minibatches if hp.algo == 1 else 1
+        if stats is None:
+            stats = torch.zeros((n_upd, N_STATS), dtype=torch.float32, device=obs.device)
+        k = C.c_uint64(opt_step)
+        rc = _check(lib().cb_learner_step(self._h, _ptr(params), _ptr(adam_m), _ptr(adam_v), C.byref(k), _ptr(obs), _ptr(actions),
+                                          _ptr(rewards), _ptr(dones), _ptr(behaviour_logits), C.byref(hp), _ptr(stats), _stream()))
+        assert rc == n_upd
+        return k.value, stats
+
+    def learner_view(self, which):
+        """Copy of a library-owned result of the last learner step (cb_learner_view) as a torch tensor."""
+        torch = _torch()
+        p = C.c_void_p(); n = C.c_size_t()
+        _check(lib().cb_learner_view(self._h, C.c_int(which), C.byref(p), C.byref(n)))
+        torch.cuda.current_stream().synchronize()
+        return torch.as_tensor(_DevView(p.value, n.value), device="cuda").clone()
+
+
+class _DevView:
+    """__cuda_array_interface__ holder for a library-owned fp32 device buffer."""
+
+    def __init__(self, ptr, n):
+        self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f4", "data": (ptr, False), "version": 2}
+
+
+# ---- sub-step entry points --------------------------------------------------------------------------
+def sample_actions(logits, seed, step, env_offset=0):
+    torch = _torch(); _dev(logits, torch.float32, "logits"); B, A = logits.shape
+    act = torch.empty((B,), dtype=torch.int32, device=logits.device)
+    _check(lib().cb_sample_actions(_ptr(logits), C.c_int(B), C.c_int(A), C.c_uint64(seed), C.c_uint64(step), C.c_uint32(env_offset), _ptr(act), _stream()))
+    return act
+
+
+def logprob_entropy(logits, actions):
+    torch = _torch(); _dev(logits, torch.float32, "logits"); _dev(actions, torch.int32, "actions"); N, A = logits.shape
+    lp = torch.empty((N,), dtype=torch.float32, device=logits.device); H = torch.empty_like(lp)
+    _check(lib().cb_logprob_entropy(_ptr(logits), C.c_int(A), C.c_int(N), C.c_int(A), _ptr(actions), _ptr(lp), _ptr(H), _stream()))
+    return lp, H
+
+
+def vtrace(V, r, d, logpi, logmu, gamma=0.99, lam=1.0, rho_bar=1.0, c_bar=1.0, rho_pg_bar=1.0):
+    torch = _torch(); T, B = r.shape
+    for t, n in ((V, "V"), (r, "r"), (logpi, "logpi"), (logmu, "logmu")):
+        _dev(t, torch.float32, n)
+    _dev(d, torch.uint8, "d")
+    vs = torch.empty_like(r); pg = torch.empty_like(r); rho = torch.empty_like(r)
+    _check(lib().cb_vtrace(C.c_int(T), C.c_int(B), _ptr(V), _ptr(r), _ptr(d), _ptr(logpi), _ptr(logmu), C.c_float(gamma), C.c_float(lam),
+                           C.c_float(rho_bar), C.c_float(c_bar), C.c_float(rho_pg_bar), _ptr(vs), _ptr(pg), _ptr(rho), _stream()))
+    return vs, pg, rho
+
+
+def gae(V, r, d, gamma=0.99, lam=0.95):
+    torch = _torch(); T, B = r.shape
+    _dev(V, torch.float32, "V"); _dev(r, torch.float32, "r"); _dev(d, torch.uint8, "d")
+    adv = torch.empty_like(r); ret = torch.empty_like(r)
+    _check(lib().cb_gae(C.c_int(T), C.c_int(B), _ptr(V), _ptr(r), _ptr(d), C.c_float(gamma), C.c_float(lam), _ptr(adv), _ptr(ret), _stream()))
+    return adv, ret
+
+
+def permutation(seed, epoch, N):
+    torch = _torch()
+    perm = torch.empty((N,), dtype=torch.int32, device="cuda")
+    _check(lib().cb_permutation(C.c_uint64(seed), C.c_uint32(epoch), C.c_int(N), _ptr(perm), _stream()))
+    return perm
+
+
+def clip_adam(params, adam_m, adam_v, grad, k, lr, beta1=0.9, beta2=0.999, eps=1e-5, max_norm=40.0, scratch=None):
+    """In place on params/adam_m/adam_v; returns the pre-clip gradient norm as a cuda fp32 [1] tensor."""
+    torch = _torch(); P = params.numel()
+    for t, n in ((params, "params"), (adam_m, "adam_m"), (adam_v, "adam_v"), (grad, "grad")):
+        _dev(t, torch.float32, n)
+    if scratch is None:
+        scratch = torch.empty((int(lib().cb_clip_adam_scratch_bytes(C.c_size_t(P))) + 7) // 8, dtype=torch.float64, device=params.device)
+    gn = torch.empty((1,), dtype=torch.float32, device=params.device)
+    _check(lib().cb_clip_adam(C.c_size_t(P), _ptr(params), _ptr(adam_m), _ptr(adam_v), _ptr(grad), C.c_uint64(k), C.c_float(lr), C.c_float(beta1),
+                              C.c_float(beta2), C.c_float(eps), C.c_float(max_norm), _ptr(gn), _ptr(scratch), _stream()))
+    return gn

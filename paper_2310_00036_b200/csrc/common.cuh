@@ -1,0 +1,141 @@
+// Internal declarations of the Cleanba hot-path library (not part of the C ABI).
+// Layouts inside the library: activations NHWC ([frame, y, x, channel], channel fastest) in the
+// mode's storage type (fp32 in CB_PREC_FP32_REF, bf16 in CB_PREC_BF16_TC); every linear layer
+// (conv, fc, heads) is a convolution: fc = a VALID conv whose kernel covers the whole feature map,
+// heads = a 1x1 conv with A+1 outputs (A logits, then the value).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <algorithm>
+#include <cmath>
+#include <string>
+#include <vector>
+
+#include "../../include/cleanba.h"
+
+namespace cb {
+
+typedef __nv_bfloat16 bf16;
+
+// one convolution-shaped linear layer
+struct Geom {
+  int H, W, Cin;       // input map
+  int Ho, Wo, Cout;    // output map
+  int kh, kw, s, p;    // kernel, stride, zero padding (low side = high side)
+};
+
+// where the layer's parameters live in the canonical flat fp32 buffer.  Output channels
+// n < n_split use (w_off, b_off); the others (w2_off, b2_off) -- only the heads layer splits
+// (pi.w/pi.b then v.w/v.b).
+struct ParamMap {
+  size_t w_off, b_off, w2_off, b2_off;
+  int n_split;
+  __host__ __device__ size_t w(int n, int c, int di, int dj, const Geom& g) const {
+    return n < n_split ? w_off + (((size_t)n * g.Cin + c) * g.kh + di) * g.kw + dj
+                       : w2_off + (((size_t)(n - n_split) * g.Cin + c) * g.kh + di) * g.kw + dj;
+  }
+  __host__ __device__ size_t b(int n) const { return n < n_split ? b_off + n : b2_off + (n - n_split); }
+};
+
+struct Layer {
+  Geom g;
+  ParamMap pm;
+  int in_t, out_t, skip_t;   // activation tensor ids (-1 = observations / none)
+  bool relu_in;              // the layer consumes relu(in)
+  bool u8_in;                // first layer: uint8 NCHW observations, scaled by 1/255 (O1)
+  bool f32_out;              // heads: fp32 output in every mode
+  size_t wf_off, wd_off, bias_off;   // offsets (elements) into the packed weight / bias buffers
+  std::string name;
+};
+
+enum OpKind { OP_CONV, OP_POOL, OP_WGRAD, OP_DGRAD, OP_POOLBWD };
+enum GradBuf { G_NONE = -1, G_HEAD = 0, G_HID, G_A, G_B, G_C, G_COUNT };
+
+struct Op {
+  OpKind kind;
+  int layer;        // CONV / WGRAD / DGRAD
+  int in_t, out_t;  // POOL fwd: tensors;  POOLBWD: in_t = conv-output tensor (pool input)
+  int C, H, W;      // POOL geometry (input map)
+  int dy, dx;       // backward: gradient buffers (GradBuf)
+  int mask_t;       // DGRAD: tensor whose sign gates the result (-1 none)
+  int add;          // DGRAD: gradient buffer added after masking (-1 none)
+};
+
+struct Tensor { size_t per_frame; bool f32; };
+
+struct Workspace {     // one per precision mode
+  int frames = 0;
+  std::vector<void*> act;            // per tensor, [frames * per_frame]
+  void* grad[G_COUNT] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+  void* wf = nullptr; void* wd = nullptr; float* bias = nullptr;   // packed weights (mode type), fp32 bias
+  float* partial = nullptr; size_t partial_elems = 0;             // wgrad split-K partials
+  float* gradbuf = nullptr;          // [P]
+  // learner scratch (fp32 unless noted)
+  float *logpi = nullptr, *logmu = nullptr, *ent = nullptr, *t0 = nullptr, *t1 = nullptr, *rho = nullptr, *values = nullptr;
+  float* terms = nullptr;            // [5, N] per-sample loss terms
+  double* red = nullptr;             // reduction scratch
+  float* advstat = nullptr;          // [2] mean, 1/(std+eps)
+  int32_t* perm = nullptr;           // [epochs, N]
+  uint32_t* permj = nullptr;
+  void* adam_scratch = nullptr;
+  float* gnorm = nullptr;
+  int learn_frames = 0; int learn_N = 0; int learn_epochs = 0;
+};
+
+}  // namespace cb
+
+struct cb_net {
+  cb_arch arch;
+  int max_frames;
+  size_t P;
+  std::vector<cb::Layer> layers;
+  std::vector<cb::Tensor> tensors;
+  std::vector<cb::Op> fwd, bwd;
+  size_t grad_elems[cb::G_COUNT];      // per frame
+  size_t wf_total, wd_total, bias_total, partial_max;
+  int head_t, hid_t;
+  struct PT { std::string name; size_t off; int rank; int dims[4]; int fan_in; };
+  std::vector<PT> ptensors;
+  cb::Workspace ws[2];
+  int last_prec = -1; int last_F = 0, last_N = 0; bool last_ppo = false;
+};
+
+namespace cb {
+
+void set_error(const char* fmt, ...);
+int cuda_fail(cudaError_t e, const char* what);
+#define CB_CUDA(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return cb::cuda_fail(e__, #x); } while (0)
+
+// net.cu
+int ensure_workspace(cb_net* net, int prec, int frames);
+int ensure_learner_scratch(cb_net* net, int prec, int F, int N, int epochs);
+int pack_weights(cb_net* net, int prec, const float* params, cudaStream_t st);
+int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st);
+int backward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, float* grad, cudaStream_t st);
+
+// rl.cu
+int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset,
+                  int32_t* actions, cudaStream_t st);
+int launch_split_head(const float* head, int F, int A, float* logits, float* value, cudaStream_t st);
+int launch_logprob(const float* logits, int ld, int N, int A, const int32_t* actions, const int32_t* idx,
+                   float* logp_a, float* entropy, cudaStream_t st);
+int launch_vtrace(int T, int B, const float* V, int ldV, const float* r, const uint8_t* d, const float* logpi,
+                  const float* logmu, float gamma, float lam, float rho_bar, float c_bar, float rho_pg_bar,
+                  float* vs, float* pgadv, float* rho, cudaStream_t st);
+int launch_gae(int T, int B, const float* V, int ldV, const float* r, const uint8_t* d, float gamma, float lam,
+               float* adv, float* ret, cudaStream_t st);
+int launch_permutation(uint64_t seed, uint32_t epoch0, int n_epochs, int N, int32_t* perm, uint32_t* jbuf, cudaStream_t st);
+// loss kernels write dhead [N, A+1] in the mode's storage type and per-sample terms; reduce writes stats
+int launch_impala_loss(int prec, int N, int A, const float* head, const int32_t* act, const float* vs, const float* pgadv,
+                       const float* rho, float c1, float c2, int reduction, void* dhead, float* terms, double* red,
+                       float* stats, cudaStream_t st);
+int launch_ppo_loss(int prec, int m, int A, const float* head, const int32_t* idx, const int32_t* act, const float* adv,
+                    const float* ret, const float* logp_old, float eps, float c1, float c2, int norm_adv, void* dhead,
+                    float* terms, double* red, float* advstat, float* stats, cudaStream_t st);
+size_t clip_adam_scratch_bytes(size_t P);
+int launch_clip_adam(size_t P, float* params, float* m, float* v, const float* g, uint64_t k, float lr, float b1, float b2,
+                     float eps, float max_norm, float* grad_norm, float* stats_slot, void* scratch, cudaStream_t st);
+
+}  // namespace cb

@@ -1,0 +1,199 @@
+// Network side of the hot path: weight packing, forward and backward
+// (a9-a10) over the layer program built in api.cu.  Plain SIMT path; tcgen05 kernels live in
+// conv_tc.cu and are dispatched from here when the shape qualifies.
+#include "gemm_simt.cuh"
+
+namespace cb {
+
+// ---- weight packing: canonical fp32 [Cout,Cin,kh,kw] -> Wf [(di,dj,c)][n], Wd [(di,dj,n)][c], bias fp32 [n]
+template <typename AT>
+__global__ void pack_kernel(const float* __restrict__ params, Geom g, ParamMap pm, AT* wf, AT* wd, float* bias) {
+  int K = g.kh * g.kw * g.Cin;
+  size_t total = (size_t)K * g.Cout;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    int n = (int)(i % g.Cout); int k = (int)(i / g.Cout);
+    int c = k % g.Cin; int q = k / g.Cin; int dj = q % g.kw, di = q / g.kw;
+    float v = params[pm.w(n, c, di, dj, g)];
+    stv(wf, i, v);
+    stv(wd, ((size_t)(di * g.kw + dj) * g.Cout + n) * g.Cin + c, v);
+    if (k == 0) bias[n] = params[pm.b(n)];
+  }
+}
+
+template <typename AT>
+static int pack_all(cb_net* net, Workspace& ws, const float* params, cudaStream_t st) {
+  for (auto& L : net->layers) {
+    size_t total = (size_t)L.g.kh * L.g.kw * L.g.Cin * L.g.Cout;
+    int blocks = (int)std::min<size_t>((total + 255) / 256, 1184);
+    pack_kernel<AT><<<blocks, 256, 0, st>>>(params, L.g, L.pm, (AT*)ws.wf + L.wf_off, (AT*)ws.wd + L.wd_off, ws.bias + L.bias_off);
+  }
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+int pack_weights(cb_net* net, int prec, const float* params, cudaStream_t st) {
+  Workspace& ws = net->ws[prec];
+  return prec == CB_PREC_FP32_REF ? pack_all<float>(net, ws, params, st) : pack_all<bf16>(net, ws, params, st);
+}
+
+// ---- max-pool 3x3 stride 2, XLA-SAME padding (A10), NHWC ------------------------------------
+__host__ __device__ inline int pool_out(int h) { return (h + 1) / 2; }
+__host__ __device__ inline int pool_pad_lo(int h) { int o = pool_out(h); int tot = (o - 1) * 2 + 3 - h; if (tot < 0) tot = 0; return tot / 2; }
+
+template <typename AT>
+__global__ void pool_fwd_kernel(const AT* __restrict__ x, AT* __restrict__ y, int F, int C, int H, int W) {
+  int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W);
+  size_t total = (size_t)F * Ho * Wo * C;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    int c = (int)(i % C); size_t q = i / C; int ox = (int)(q % Wo); q /= Wo; int oy = (int)(q % Ho); size_t f = q / Ho;
+    float best = -INFINITY;
+    for (int di = 0; di < 3; ++di) {
+      int iy = oy * 2 + di - ph; if ((unsigned)iy >= (unsigned)H) continue;
+      for (int dj = 0; dj < 3; ++dj) {
+        int ix = ox * 2 + dj - pw; if ((unsigned)ix >= (unsigned)W) continue;
+        float v = ldv(x, ((f * H + iy) * W + ix) * C + c);
+        if (v > best) best = v;
+      }
+    }
+    stv(y, i, best);
+  }
+}
+
+// gather form of the adjoint: input pixel (iy,ix) receives dy of every window whose FIRST maximum
+// in row-major window order (A11) is this pixel.  No atomics.
+template <typename AT>
+__global__ void pool_bwd_kernel(const AT* __restrict__ x, const AT* __restrict__ dy, AT* __restrict__ dx, int F, int C, int H, int W) {
+  int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W);
+  size_t total = (size_t)F * H * W * C;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    int c = (int)(i % C); size_t q = i / C; int ix = (int)(q % W); q /= W; int iy = (int)(q % H); size_t f = q / H;
+    float g = 0.f;
+    // windows containing (iy,ix): oy*2 - ph <= iy <= oy*2 - ph + 2
+    int oy_lo = (iy + ph - 2 + 1) / 2; if (iy + ph - 2 < 0) oy_lo = 0;
+    int ox_lo = (ix + pw - 2 + 1) / 2; if (ix + pw - 2 < 0) ox_lo = 0;
+    int oy_hi = min((iy + ph) / 2, Ho - 1), ox_hi = min((ix + pw) / 2, Wo - 1);
+    for (int oy = oy_lo; oy <= oy_hi; ++oy)
+      for (int ox = ox_lo; ox <= ox_hi; ++ox) {
+        float best = -INFINITY; int by = -1, bx = -1;
+        for (int di = 0; di < 3; ++di) {
+          int yy = oy * 2 + di - ph; if ((unsigned)yy >= (unsigned)H) continue;
+          for (int dj = 0; dj < 3; ++dj) {
+            int xx = ox * 2 + dj - pw; if ((unsigned)xx >= (unsigned)W) continue;
+            float v = ldv(x, ((f * H + yy) * W + xx) * C + c);
+            if (v > best) { best = v; by = yy; bx = xx; }
+          }
+        }
+        if (by == iy && bx == ix) g += ldv(dy, ((f * Ho + oy) * Wo + ox) * C + c);
+      }
+    stv(dx, i, g);
+  }
+}
+
+// ---- wgrad second pass: sum split-K partials in split order, scale, scatter to canonical grad ----
+__global__ void wgrad_reduce_kernel(const float* __restrict__ partial, int splits, Geom g, ParamMap pm, float in_scale, float* __restrict__ grad) {
+  int Kw = g.kh * g.kw * g.Cin, M = Kw + 1, N = g.Cout;
+  size_t total = (size_t)M * N;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    float s = 0.f;
+    for (int z = 0; z < splits; ++z) s += partial[(size_t)z * total + i];
+    int n = (int)(i % N), m = (int)(i / N);
+    if (m == Kw) { grad[pm.b(n)] = s; continue; }
+    int c = m % g.Cin; int q = m / g.Cin; int dj = q % g.kw, di = q / g.kw;
+    grad[pm.w(n, c, di, dj, g)] = s * in_scale;
+  }
+}
+
+// split-K policy: a function of the problem shape only (never of the device), so the summation
+// order -- and with it every bit of the gradient -- is fixed (A16).
+static inline void wgrad_split(long long K, int* splits, int* kchunk) {
+  const int target = 4096;
+  long long s = (K + target - 1) / target; if (s < 1) s = 1; if (s > 2048) s = 2048;
+  long long ch = (K + s - 1) / s; ch = (ch + 15) / 16 * 16;
+  *splits = (int)((K + ch - 1) / ch); *kchunk = (int)ch;
+}
+
+size_t wgrad_partial_elems(const Geom& g, long long frames) {
+  int s, ch; wgrad_split(frames * g.Ho * g.Wo, &s, &ch);
+  return (size_t)s * (g.kh * g.kw * g.Cin + 1) * g.Cout;
+}
+
+static inline int grid_for(size_t total) { return (int)std::min<size_t>((total + 255) / 256, (size_t)148 * 16); }
+
+template <typename AT>
+static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st) {
+  for (const Op& op : net->fwd) {
+    if (op.kind == OP_POOL) {
+      size_t total = (size_t)F * pool_out(op.H) * pool_out(op.W) * op.C;
+      pool_fwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (AT*)ws.act[op.out_t], F, op.C, op.H, op.W);
+      CB_CUDA(cudaGetLastError());
+      continue;
+    }
+    const Layer& L = net->layers[op.layer];
+    const Geom& g = L.g;
+    int M = F * g.Ho * g.Wo, N = g.Cout, K = g.kh * g.kw * g.Cin;
+    const AT* wf = (const AT*)ws.wf + L.wf_off; const float* bias = ws.bias + L.bias_off;
+    const AT* skip = L.skip_t >= 0 ? (const AT*)ws.act[L.skip_t] : nullptr;
+    int rc;
+    if (L.u8_in) {
+      FwdProblem<AT, AT, true> p{M, N, K, K, {g, obs, frame_idx, false}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f / 255.0f};
+      rc = launch_gemm(p, 1, st);
+    } else if (L.f32_out) {
+      FwdProblem<AT, float, false> p{M, N, K, K, {g, ws.act[L.in_t], nullptr, L.relu_in}, wf, bias, skip, (float*)ws.act[L.out_t], 1.0f};
+      rc = launch_gemm(p, 1, st);
+    } else {
+      FwdProblem<AT, AT, false> p{M, N, K, K, {g, ws.act[L.in_t], nullptr, L.relu_in}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f};
+      rc = launch_gemm(p, 1, st);
+    }
+    if (rc) return rc;
+  }
+  return CB_OK;
+}
+
+int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st) {
+  Workspace& ws = net->ws[prec];
+  return prec == CB_PREC_FP32_REF ? forward_t<float>(net, ws, obs, frame_idx, F, st) : forward_t<bf16>(net, ws, obs, frame_idx, F, st);
+}
+
+template <typename AT>
+static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, float* grad, cudaStream_t st) {
+  for (const Op& op : net->bwd) {
+    if (op.kind == OP_POOLBWD) {
+      size_t total = (size_t)F * op.H * op.W * op.C;
+      pool_bwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (const AT*)ws.grad[op.dy], (AT*)ws.grad[op.dx], F, op.C, op.H, op.W);
+      CB_CUDA(cudaGetLastError());
+      continue;
+    }
+    const Layer& L = net->layers[op.layer];
+    const Geom& g = L.g;
+    if (op.kind == OP_WGRAD) {
+      int Kpix = F * g.Ho * g.Wo, M = g.kh * g.kw * g.Cin + 1, N = g.Cout, splits, kchunk;
+      wgrad_split(Kpix, &splits, &kchunk);
+      int rc;
+      if (L.u8_in) {
+        WgradProblem<AT, AT, true> p{M, N, Kpix, kchunk, {g, obs, frame_idx, false}, (const AT*)ws.grad[op.dy], ws.partial};
+        rc = launch_gemm(p, splits, st);
+      } else {
+        WgradProblem<AT, AT, false> p{M, N, Kpix, kchunk, {g, ws.act[L.in_t], nullptr, L.relu_in}, (const AT*)ws.grad[op.dy], ws.partial};
+        rc = launch_gemm(p, splits, st);
+      }
+      if (rc) return rc;
+      wgrad_reduce_kernel<<<grid_for((size_t)M * N), 256, 0, st>>>(ws.partial, splits, g, L.pm, L.u8_in ? 1.0f / 255.0f : 1.0f, grad);
+      CB_CUDA(cudaGetLastError());
+    } else {  // OP_DGRAD
+      int M = F * g.H * g.W, N = g.Cin, K = g.kh * g.kw * g.Cout;
+      DgradProblem<AT> p{M, N, K, K, g, (const AT*)ws.grad[op.dy], (const AT*)ws.wd + L.wd_off,
+                         op.mask_t >= 0 ? (const AT*)ws.act[op.mask_t] : nullptr,
+                         op.add >= 0 ? (const AT*)ws.grad[op.add] : nullptr, (AT*)ws.grad[op.dx]};
+      int rc = launch_gemm(p, 1, st);
+      if (rc) return rc;
+    }
+  }
+  return CB_OK;
+}
+
+int backward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, float* grad, cudaStream_t st) {
+  Workspace& ws = net->ws[prec];
+  return prec == CB_PREC_FP32_REF ? backward_t<float>(net, ws, obs, frame_idx, F, grad, st) : backward_t<bf16>(net, ws, obs, frame_idx, F, grad, st);
+}
+
+}  // namespace cb

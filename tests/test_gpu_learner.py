@@ -1,0 +1,197 @@
+"""End-to-end parity of cb_policy_forward / cb_learner_step against the CPU oracle, on BASELINE.json
+config 0 in full and on reduced-size versions of configs 1-4 (ragged shapes included), plus the
+run-to-run bitwise determinism check (A16).  Tolerances: see tests/test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from oracle import oracle
+from paper_2310_00036_b200 import binding, build, synth
+from helpers import close, dev, host, orc_arch, rel_l2
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+RTOL = {"fp32": 1e-5, "bf16": 2e-2}
+PTOL = {"fp32": 1e-4, "bf16": 5e-3}
+SMALL_IMPALA = synth.ArchSpec("impala", (16, 32, 32), 256, 18, 4, 84, 84)
+TINY_IMPALA = synth.ArchSpec("impala", (5, 8, 12), 40, 6, 3, 37, 30)      # ragged everything
+TINY_NATURE = synth.ArchSpec("nature", (6, 10, 12), 24, 5, 2, 44, 52)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build.build()
+
+
+def _hp_pair(algo, prec, T, B, **kw):
+    hp = binding.make_hparams(algo, prec, T, B, **kw)
+    ho = oracle.make_hparams(algo, T, B, **kw)
+    for f in ("gamma", "lambda_", "rho_bar", "c_bar", "rho_pg_bar", "clip_eps", "vf_coef", "ent_coef", "lr", "beta1", "beta2", "adam_eps", "max_grad_norm"):
+        setattr(ho, f, float(getattr(hp, f)))      # the oracle sees exactly the fp32 values the ABI carries
+    return hp, ho
+
+
+def _batch(arch, T, B, seed, blobs):
+    g = synth.rng(seed)
+    rewards, dones = synth.gen_rewards_dones(T, B, seed + 1)
+    if blobs:
+        obs = synth.gen_obs_blobs(T + 1, B, seed, arch, dones)
+    else:
+        obs = synth.gen_obs_uniform((T + 1) * B, seed, arch).reshape(T + 1, B, arch.in_c, arch.in_h, arch.in_w)
+    bl, actions = synth.gen_behaviour(T, B, arch.n_actions, seed + 2)
+    return dict(obs=obs, actions=actions, rewards=rewards, dones=dones, behaviour_logits=bl)
+
+
+@pytest.mark.parametrize("arch,F,prec", [(synth.NATURE, 24, "fp32"), (SMALL_IMPALA, 6, "fp32"), (SMALL_IMPALA, 6, "bf16"),
+                                         (TINY_IMPALA, 133, "fp32"), (TINY_IMPALA, 133, "bf16"), (TINY_NATURE, 131, "fp32"),
+                                         (synth.NATURE, 5, "bf16")])
+def test_policy_forward_parity(arch, F, prec):
+    params = synth.gen_params(arch, 11, bias_scale=0.05)
+    obs = synth.gen_obs_uniform(F, 12, arch)
+    net = binding.Net(arch)
+    logits, value, actions = net.policy_forward(dev(params), dev(obs), seed=5, step=9, env_offset=3, precision=prec)
+    rl, rv = oracle.forward(orc_arch(arch), params, obs)
+    close(host(logits), rl, RTOL[prec], what="logits"); close(host(value), rv, RTOL[prec], what="value")
+    # bit-exact contract (A9): oracle sampling of the logits the GPU returned == the GPU's actions
+    assert np.array_equal(host(actions), oracle.sample(host(logits), 5, 9, 3))
+
+
+def test_policy_forward_config1_shape():
+    """BASELINE.json configs[1]: IMPALA-ResNet, B = 128 blob frames, bf16; oracle on a sample of frames."""
+    arch = synth.IMPALA; B = 128
+    params = synth.gen_params(arch, 1001)
+    obs = synth.gen_obs_blobs(1, B, 1001, arch)[0]
+    net = binding.Net(arch)
+    dp, dobs = dev(params), dev(obs)
+    logits, value, actions = net.policy_forward(dp, dobs, seed=1001, step=0, precision="bf16")
+    sel = np.arange(0, B, 11)
+    rl, rv = oracle.forward(orc_arch(arch), params, obs[sel])
+    close(host(logits)[sel], rl, 2e-2, what="logits"); close(host(value)[sel], rv, 2e-2, what="value")
+    assert np.array_equal(host(actions), oracle.sample(host(logits), 1001, 0, 0))
+    l2, v2, a2 = net.policy_forward(dp, dobs, seed=1001, step=0, precision="bf16")
+    assert torch.equal(l2, logits) and torch.equal(v2, value) and torch.equal(a2, actions)   # A16
+    _, _, a3 = net.policy_forward(dp, dobs, seed=1001, step=1, precision="bf16")
+    assert not torch.equal(a3, actions)
+
+
+def _run_learner(arch, algo, prec, T, B, seed, blobs=False, warm=False, **kw):
+    hp, ho = _hp_pair(algo, prec, T, B, **kw)
+    bt = _batch(arch, T, B, seed, blobs)
+    params = synth.gen_params(arch, seed + 5, bias_scale=0.05); P = params.size
+    g = synth.rng(seed + 6)
+    m = (g.standard_normal(P) * 1e-3).astype(np.float32) if warm else np.zeros(P, np.float32)
+    v = (g.random(P) * 1e-5).astype(np.float32) if warm else np.zeros(P, np.float32)
+    k0 = 100 if warm else 0
+    net = binding.Net(arch)
+    dp, dm, dv = dev(params), dev(m), dev(v)
+    args = [dev(bt[k]) for k in ("obs", "actions", "rewards", "dones", "behaviour_logits")]
+    k1, stats = net.learner_step(dp, dm, dv, k0, *args, hp)
+    torch.cuda.synchronize()
+    got = dict(params=host(dp), m=host(dm), v=host(dv), stats=host(stats), k=k1,
+               head=host(net.learner_view(0)).reshape(-1, arch.n_actions + 1), t0=host(net.learner_view(1)),
+               t1=host(net.learner_view(2)), grad=host(net.learner_view(3)))
+    ref = oracle.learner_step(orc_arch(arch), ho, params, m, v, k0, bt["obs"], bt["actions"], bt["rewards"], bt["dones"],
+                              bt["behaviour_logits"], debug=True)
+    return net, got, ref, params
+
+
+def _check_learner(arch, got, ref, params0, prec, ppo):
+    rt, A = RTOL[prec], arch.n_actions
+    assert got["k"] == ref["opt_step"]
+    close(got["head"][:, :A], ref["logits"], rt, what="logits"); close(got["head"][:, A], ref["values"], rt, what="values")
+    # targets: 1e-5 relative (fp32) / 2e-2 relative + 1e-3 absolute (bf16)
+    for key in ("t0", "t1"):
+        r = ref[key].ravel(); gq = got[key].ravel()
+        tol = rt * np.maximum(np.abs(gq), np.abs(r)) + (1e-3 if prec == "bf16" else rt * np.sqrt(np.mean(r ** 2)))
+        assert (np.abs(gq - r) <= tol).all(), (key, np.abs(gq - r).max())
+    # stats of every update; loss terms can cancel, so the absolute floor is rtol * (|pg| + |v| + |H|) scale
+    for u in range(ref["stats"].shape[0]):
+        gs, rs = got["stats"][u].astype(np.float64), ref["stats"][u].astype(np.float64)
+        scale = np.abs(rs[1]) + np.abs(rs[2]) + 0.01 * np.abs(rs[3]) + 1e-3
+        srt = rt if u == 0 else 10 * rt     # later PPO updates compound the parameter differences
+        for i, name in enumerate(oracle.STAT_NAMES):
+            floor = scale if i < 3 else (1e-3 if prec == "bf16" else 1e-6)
+            assert abs(gs[i] - rs[i]) <= srt * max(abs(gs[i]), abs(rs[i])) + srt * floor, (u, name, gs[i], rs[i])
+    # gradient of the last update: per-tensor relative L2
+    lay = binding.Net(arch).param_layout()
+    if not ppo:
+        for name, off, dims in lay:
+            n = int(np.prod(dims)); e = rel_l2(got["grad"][off:off + n], ref["grad"][off:off + n])
+            assert e < (1e-4 if prec == "fp32" else 3e-2), (name, e)
+    # parameters after the step: per-tensor relative L2 (A15), and the update itself
+    for name, off, dims in lay:
+        n = int(np.prod(dims)); e = rel_l2(got["params"][off:off + n], ref["params"][off:off + n])
+        assert e < PTOL[prec], (name, e)
+    if prec == "fp32" and not ppo:
+        du_g = got["params"].astype(np.float64) - params0; du_r = ref["params"].astype(np.float64) - params0
+        assert rel_l2(du_g, du_r) < 2e-2        # Adam's first step is ~ sign(g) lr: noise-floor elements may flip (A15)
+        assert rel_l2(got["m"], ref["m"]) < 1e-4 and rel_l2(got["v"], ref["v"]) < 2e-4
+
+
+def test_learner_config0_full():
+    """BASELINE.json configs[0]: Nature-CNN, T=5, B=4, fp32, V-trace, Adam lr 6e-4, clip 40 -- in full."""
+    net, got, ref, p0 = _run_learner(synth.NATURE, "impala", "fp32", 5, 4, 1000)
+    _check_learner(synth.NATURE, got, ref, p0, "fp32", False)
+
+
+@pytest.mark.parametrize("prec", ["fp32", "bf16"])
+@pytest.mark.parametrize("warm", [False, True])
+def test_learner_impala_resnet_small(prec, warm):
+    """configs[2] at reduced size (T=3, B=3), cold and warm optimizer state (A15)."""
+    net, got, ref, p0 = _run_learner(SMALL_IMPALA, "impala", prec, 3, 3, 1002, blobs=True, warm=warm)
+    _check_learner(SMALL_IMPALA, got, ref, p0, prec, False)
+
+
+@pytest.mark.parametrize("prec", ["fp32", "bf16"])
+def test_learner_impala_ragged_tiny(prec):
+    net, got, ref, p0 = _run_learner(TINY_IMPALA, "impala", prec, 7, 19, 77, lambda_=0.9, rho_bar=1.3, loss_reduction=1 if prec == "fp32" else 0, max_grad_norm=1.0)
+    _check_learner(TINY_IMPALA, got, ref, p0, prec, False)
+
+
+def test_learner_nature_ragged_tiny():
+    net, got, ref, p0 = _run_learner(TINY_NATURE, "impala", "fp32", 4, 33, 78)
+    _check_learner(TINY_NATURE, got, ref, p0, "fp32", False)
+
+
+@pytest.mark.parametrize("prec", ["fp32", "bf16"])
+def test_learner_ppo_small(prec):
+    """configs[3] at reduced size: GAE, 2 epochs x 2 minibatches over the seeded permutation."""
+    net, got, ref, p0 = _run_learner(TINY_IMPALA, "ppo", prec, 8, 6, 1003, epochs=2, minibatches=2, perm_seed=42)
+    assert ref["stats"].shape[0] == 4
+    _check_learner(TINY_IMPALA, got, ref, p0, prec, True)
+
+
+def test_learner_ppo_resnet_one_update():
+    net, got, ref, p0 = _run_learner(SMALL_IMPALA, "ppo", "fp32", 3, 4, 1004, blobs=True, epochs=1, minibatches=2)
+    _check_learner(SMALL_IMPALA, got, ref, p0, "fp32", True)
+
+
+@pytest.mark.parametrize("algo,prec", [("impala", "bf16"), ("impala", "fp32"), ("ppo", "bf16")])
+def test_learner_bitwise_deterministic(algo, prec):
+    """A16: three runs from identical inputs give identical bytes (params, m, v, stats, targets, grad)."""
+    arch, T, B = SMALL_IMPALA, 4, 6
+    hp = binding.make_hparams(algo, prec, T, B, epochs=2, minibatches=2)
+    bt = _batch(arch, T, B, 5, True); params = synth.gen_params(arch, 6); P = params.size
+    outs = []
+    for rep in range(3):
+        net = binding.Net(arch)
+        dp, dm, dv = dev(params), dev(np.zeros(P, np.float32)), dev(np.zeros(P, np.float32))
+        if rep == 2:    # other work in flight on another stream must not change the result
+            junk = torch.randn(4096, 4096, device="cuda"); s2 = torch.cuda.Stream()
+            with torch.cuda.stream(s2):
+                for _ in range(10):
+                    junk = junk @ junk * 1e-3
+        _, stats = net.learner_step(dp, dm, dv, 0, *[dev(bt[k]) for k in ("obs", "actions", "rewards", "dones", "behaviour_logits")], hp)
+        torch.cuda.synchronize()
+        outs.append(b"".join(host(t).tobytes() for t in (dp, dm, dv, stats, net.learner_view(1), net.learner_view(2), net.learner_view(3))))
+    assert outs[0] == outs[1] == outs[2]
+
+
+def test_errors_on_bad_shapes():
+    net = binding.Net(SMALL_IMPALA)
+    hp = binding.make_hparams("ppo", "fp32", 3, 3, minibatches=4)     # 9 samples do not split in 4
+    z = torch.zeros(16, device="cuda")
+    with pytest.raises(binding.CleanbaError):
+        net.learner_step(torch.zeros(net.P, device="cuda"), torch.zeros(net.P, device="cuda"), torch.zeros(net.P, device="cuda"), 0,
+                         torch.zeros((4, 3, 4, 84, 84), dtype=torch.uint8, device="cuda"), torch.zeros((3, 3), dtype=torch.int32, device="cuda"),
+                         z, torch.zeros(9, dtype=torch.uint8, device="cuda"), torch.zeros((3, 3, 18), device="cuda"), hp)
