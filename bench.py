@@ -1,0 +1,339 @@
+#!/usr/bin/env python
+"""bench.py -- learner env-frames/s of the Cleanba hot path on B200 (BASELINE.json's metric).
+
+A "step" is one cb_learner_step (forward over (T+1)B frames, V-trace or GAE, loss, backward, global
+clip + Adam) over one batch of seeded synthetic trajectories shaped like the paper's Atari runs.
+Default workload: BASELINE.json configs[2] (IMPALA-ResNet 16/32/32, T=20, B=128, bf16 mode), the
+configuration the learner metric is quoted on; --config 3 / 4 select the PPO and the wide workloads.
+N > 1 (torchrun): N independent replicas, one per GPU, no data-path collective ("replicas only",
+DESIGN.md section 7) -- weak scaling.  `--impl reference` times the CPU oracle instead.
+
+Prints ONE JSON line (rank 0).  See DESIGN.md section 6 for every key.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2310_00036_b200 import synth  # noqa: E402
+
+METRIC = "learner env-frames/sec on 1 B200 (fwd+V-trace/GAE+bwd+Adam); % bf16 TC peak"
+UNIT = "env-frames/s"
+# useful MACs per frame: forward, backward (dgrad + wgrad, no dgrad into obs)
+MACS = {"impala": (54_227_712, 104_391_168), "impala_wide": (208_772_608, 409_416_704), "nature": (9_352_704, 15_428_608)}
+N_ROTATE = 3      # distinct input sets cycled through so that observations are never L2-resident
+
+
+def workload(cfg_index):
+    cfg = synth.CONFIGS[cfg_index]
+    if cfg["algo"] == "actor":
+        raise SystemExit("config 1 is actor inference only; the learner metric is quoted on configs 2-4")
+    return cfg
+
+
+def net_key(arch):
+    return "nature" if arch.kind == "nature" else ("impala_wide" if arch.channels[0] == 32 else "impala")
+
+
+def useful_flops_per_step(cfg):
+    f, b = MACS[net_key(cfg["arch"])]
+    T, B = cfg["T"], cfg["B"]
+    if cfg["algo"] == "ppo":      # one no-grad forward over (T+1)B frames + epochs x (forward + backward) over T*B
+        return 2.0 * (f * (T + 1) * B + 4 * (f + b) * T * B)
+    return 2.0 * (f * (T + 1) * B + b * T * B)
+
+
+def gen_inputs(cfg_index, cfg, n_sets, rank):
+    """n_sets seeded input sets (host numpy).  Behaviour logits ~ N(0,1) for config 0, else N(0, 0.3) around
+    a fixed seeded logit field (the bench does not need the policy-coupled recipe A18: throughput does not
+    depend on the values)."""
+    T, B, arch = cfg["T"], cfg["B"], cfg["arch"]
+    sets = []
+    for i in range(n_sets):
+        seed = 1000 + cfg_index + 7919 * i + 104729 * rank
+        rewards, dones = synth.gen_rewards_dones(T, B, seed + 1)
+        if cfg["obs"] == "uniform":
+            obs = synth.gen_obs_uniform((T + 1) * B, seed, arch).reshape(T + 1, B, arch.in_c, arch.in_h, arch.in_w)
+        else:
+            # blobs for a slice of envs, tiled with per-env integer noise: same statistics, bounded generation time
+            nb = min(B, 32)
+            base = synth.gen_obs_blobs(T + 1, nb, seed, arch, dones[:, :nb])
+            reps = (B + nb - 1) // nb
+            obs = np.concatenate([np.roll(base, r * 3, axis=-1) for r in range(reps)], axis=1)[:, :B]
+        bl, actions = synth.gen_behaviour(T, B, arch.n_actions, seed + 2, None, 0.3)
+        sets.append(dict(obs=np.ascontiguousarray(obs), actions=actions, rewards=rewards, dones=dones, behaviour_logits=bl))
+    return sets
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, gpu_index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill(); out, _ = self.p.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def max_over_ranks(t_local, world):
+    """Max of a per-rank scalar over all ranks (identity for world == 1).  Works with nccl and gloo."""
+    if world == 1:
+        return t_local
+    import torch
+    import torch.distributed as dist
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([t_local], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x_local, world):
+    if world == 1:
+        return x_local
+    import torch
+    import torch.distributed as dist
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([x_local], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], tf_burst=d["bf16_tflops"], tf_sust=d.get("bf16_tflops_sustained", d["bf16_tflops"]), src="measured")
+    return dict(hbm=6650.0, tf_burst=1590.0, tf_sust=1400.0, src="fallback")   # B200_PROFILING.md fallback
+
+
+def run_reference(args, cfg_index, cfg, rank, world):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the workload (rank 0 only)."""
+    if rank != 0:
+        return
+    from oracle import oracle
+    arch = cfg["arch"]; T = min(cfg["T"], 2); B = min(cfg["B"], 2 if arch.kind == "impala" else 4)
+    oa = oracle.make_arch(arch.kind, arch.channels, arch.fc, arch.n_actions, arch.in_c, arch.in_h, arch.in_w)
+    kw = dict(epochs=1, minibatches=1) if cfg["algo"] == "ppo" else {}
+    ho = oracle.make_hparams(cfg["algo"], T, B, lr=cfg["lr"], max_grad_norm=cfg["max_grad_norm"], **kw)
+    sub = dict(cfg); sub["T"], sub["B"] = T, B
+    bt = gen_inputs(cfg_index, sub, 1, 0)[0]
+    params = synth.gen_params(arch, 1, head_scale=0.1); P = params.size
+    m = np.zeros(P, np.float32); v = np.zeros(P, np.float32)
+    times = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle.learner_step(oa, ho, params, m, v, 0, bt["obs"], bt["actions"], bt["rewards"], bt["dones"], bt["behaviour_logits"])
+        if i >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    total = sum(times); value = T * B * len(times) / total
+    sample = f"T={T}, B={B} envs of the workload per step ({(T + 1) * B} frames forward, {T * B} backward), full network, 1 thread"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{cfg_index}]", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(cfg_index, cfg, budget_s=12.0):
+    """The oracle as it stands, 1 thread, on a bounded sample of the same workload (about 10-30 s)."""
+    from oracle import oracle
+    arch = cfg["arch"]; T, B = 2, 2
+    oa = oracle.make_arch(arch.kind, arch.channels, arch.fc, arch.n_actions, arch.in_c, arch.in_h, arch.in_w)
+    kw = dict(epochs=1, minibatches=1) if cfg["algo"] == "ppo" else {}
+    ho = oracle.make_hparams(cfg["algo"], T, B, lr=cfg["lr"], max_grad_norm=cfg["max_grad_norm"], **kw)
+    sub = dict(cfg); sub["T"], sub["B"] = T, B
+    bt = gen_inputs(cfg_index, sub, 1, 0)[0]
+    params = synth.gen_params(arch, 1, head_scale=0.1); P = params.size
+    n, t0 = 0, time.perf_counter()
+    while True:
+        oracle.learner_step(oa, ho, params, np.zeros(P, np.float32), np.zeros(P, np.float32), 0, bt["obs"], bt["actions"], bt["rewards"], bt["dones"], bt["behaviour_logits"])
+        n += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    return {"value": T * B * n / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"{n} oracle learner steps at T={T}, B={B} ({(T + 1) * B} frames forward, {T * B} backward each), same network and loss, {dt:.1f} s"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (2, 3, 4; 0 = small parity case)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    cfg = workload(args.config)
+    if args.impl == "reference":
+        return run_reference(args, args.config, cfg, rank, world)
+
+    import torch
+    from paper_2310_00036_b200 import binding, build
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    binding.lib()
+    warmup = max(args.warmup, 3); steps = max(args.steps, 1)
+    T, B, arch = cfg["T"], cfg["B"], cfg["arch"]
+    prec = cfg["precision"]
+    kw = {} if cfg["algo"] != "ppo" else dict(epochs=4, minibatches=4)
+    hp = binding.make_hparams(cfg["algo"], prec, T, B, lr=cfg["lr"], max_grad_norm=cfg["max_grad_norm"], **kw)
+    net = binding.Net(arch, max_frames=(T + 1) * B)
+    params0 = synth.gen_params(arch, 1, head_scale=0.1)
+    sets = gen_inputs(args.config, cfg, N_ROTATE, rank)
+    keys = ("obs", "actions", "rewards", "dones", "behaviour_logits")
+    host_sets = [{k: torch.from_numpy(s[k]).pin_memory() for k in keys} for s in sets]
+    dev_sets = [{k: v.cuda(non_blocking=True) for k, v in hs.items()} for hs in host_sets]
+    P = net.P
+    dp = torch.from_numpy(params0).cuda(); dm = torch.zeros(P, device="cuda"); dv = torch.zeros(P, device="cuda")
+    n_upd = hp.epochs * hp.minibatches if hp.algo == 1 else 1
+    stats = torch.zeros((n_upd, binding.N_STATS), device="cuda")
+    stream = torch.cuda.current_stream()
+    kstep = 0
+
+    def step(i, bufs):
+        nonlocal kstep
+        s = bufs[i % len(bufs)]
+        kstep, _ = net.learner_step(dp, dm, dv, kstep, s["obs"], s["actions"], s["rewards"], s["dones"], s["behaviour_logits"], hp, stats)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up; the first pass profiles every kernel class to find the dominant one ----------------------
+    step(0, dev_sets); torch.cuda.synchronize()
+    binding.profile_begin(-1)
+    step(1, dev_sets)
+    prof_all = binding.profile_end()
+    dominant = max(prof_all, key=lambda e: e["ms"])
+    for i in range(2, warmup):
+        step(i, dev_sets)
+    # ---- timed region: K steps, inputs resident in HBM; events on the launching stream ----------------------
+    barrier()
+    clocks = ClockSampler(local)
+    l0 = binding.launch_count()
+    binding.profile_begin(dominant["cls"])        # two events around each launch of the dominant class only
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(steps):
+        step(i, dev_sets)
+    e1.record(stream)
+    barrier()
+    t_local = e0.elapsed_time(e1) / 1e3
+    dom = binding.profile_end()[0]
+    launches = binding.launch_count() - l0
+    clk = clocks.stop()
+    t = max_over_ranks(t_local, world)
+    frames = sum_over_ranks(float(T * B * steps), world)
+    value = frames / t
+    loss_last = float(stats[-1, 0].item())
+    assert np.isfinite(loss_last), "learner produced a non-finite loss"
+
+    # ---- end to end through the public API with HOST buffers: H2D of the step's inputs + D2H of its stats ---
+    h2d = sum(v.numel() * v.element_size() for v in host_sets[0].values()); d2h = stats.numel() * 4
+    stats_host = torch.empty(stats.shape, dtype=torch.float32).pin_memory()
+    stage = {k: torch.empty_like(v, device="cuda") for k, v in host_sets[0].items()}
+
+    def e2e_step(i):
+        nonlocal kstep
+        hs = host_sets[i % len(host_sets)]
+        for k in keys:
+            stage[k].copy_(hs[k], non_blocking=True)
+        kstep, _ = net.learner_step(dp, dm, dv, kstep, stage["obs"], stage["actions"], stage["rewards"], stage["dones"], stage["behaviour_logits"], hp, stats)
+        stats_host.copy_(stats, non_blocking=True)
+        stream.synchronize()        # the caller reads the loss every step
+        return float(stats_host[-1, 0])
+
+    e2e_step(0)
+    barrier()
+    w0 = time.perf_counter(); e0.record(stream)
+    for i in range(steps):
+        e2e_step(i)
+    e1.record(stream)
+    barrier()
+    t_e2e = max_over_ranks(max(e0.elapsed_time(e1) / 1e3, time.perf_counter() - w0), world)
+    e2e_value = frames / t_e2e
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peaks = load_peaks()
+    bound = "tensor" if dom["flops"] > 0 else "hbm"
+    per_launch_s = dom["ms"] / 1e3 / max(dom["launches"], 1)
+    if bound == "tensor":
+        achieved = dom["flops"] / dom["launches"] / per_launch_s / 1e12; peak = peaks["tf_sust"]; runit = "TFLOP/s"
+    else:
+        achieved = dom["bytes"] / dom["launches"] / per_launch_s / 1e9; peak = peaks["hbm"]; runit = "GB/s"
+    total_ms = sum(e["ms"] for e in prof_all)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": 1e3 * t / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if prec == "bf16" else "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {cfg['algo']} learner step, {net_key(arch)} net, T={T}, B={B}, {prec} mode",
+                   "frames_per_step": T * B, "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": f"{N_ROTATE} input sets of {h2d / 1e6:.0f} MB rotated (> 126 MB L2 together with the activations)"},
+        "tflops_useful": useful_flops_per_step(cfg) * steps / t_local / 1e12,
+        "pct_bf16_tc_peak": 100.0 * useful_flops_per_step(cfg) * steps / t_local / 1e12 / peaks["tf_sust"],
+        "clocks": clk, "gpu_launches": int(launches),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "roofline": {"bound": bound, "kernel": dom["name"], "achieved": achieved, "peak": peak, "unit": runit, "frac": achieved / peak,
+                     "traffic": None, "peak_source": f"{peaks['src']} ({'sustained bf16' if bound == 'tensor' else 'copy'})",
+                     "launches": dom["launches"], "ms_per_launch": 1e3 * per_launch_s, "share_of_step": dom["ms"] / (1e3 * t_local)},
+        "kernel_breakdown_ms_per_step": {e["name"]: round(e["ms"], 4) for e in sorted(prof_all, key=lambda e: -e["ms"])},
+        "kernel_breakdown_total_ms": total_ms, "loss": loss_last,
+    }
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args.config, cfg)
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

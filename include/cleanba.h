@@ -140,6 +140,24 @@ int cb_clip_adam(size_t P, float* params, float* adam_m, float* adam_v, const fl
                  float lr, float beta1, float beta2, float eps, float max_norm, float* grad_norm,
                  void* scratch, void* stream);
 
+/* ---- instrumentation (used by bench.py; not on the product path) --------------------------- */
+/* Number of kernels this library has launched in this process so far. */
+uint64_t cb_launch_count(void);
+/* Per-kernel-class device timing with CUDA events recorded on the launching stream around every
+ * launch of a class.  cb_profile_begin(only_class): start recording; only_class < 0 = all classes,
+ * otherwise only that class (two events per launch of it, nothing else changes).
+ * cb_profile_end: synchronises the device, stops recording and writes up to `max` entries (classes
+ * with at least one launch): returns the number written.  flops = useful 2*MAC of the launches,
+ * bytes = algorithmic bytes (operands read once + results written once). */
+typedef struct {
+  int cls;
+  char name[28];
+  uint64_t launches;
+  double ms, flops, bytes;
+} cb_prof_entry;
+int cb_profile_begin(int only_class);
+int cb_profile_end(cb_prof_entry* out, int max);
+
 const char* cb_last_error(void);
 
 #ifdef __cplusplus

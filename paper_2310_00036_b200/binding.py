@@ -18,7 +18,8 @@ ALGO = {"impala": 0, "ppo": 1}
 
 EXPORTS = ["cb_net_create", "cb_net_destroy", "cb_param_count", "cb_param_layout", "cb_net_init", "cb_policy_forward",
            "cb_learner_step", "cb_learner_view", "cb_sample_actions", "cb_logprob_entropy", "cb_vtrace", "cb_gae",
-           "cb_permutation", "cb_clip_adam_scratch_bytes", "cb_clip_adam", "cb_last_error"]
+           "cb_permutation", "cb_clip_adam_scratch_bytes", "cb_clip_adam", "cb_last_error",
+           "cb_launch_count", "cb_profile_begin", "cb_profile_end"]
 
 
 class CArch(C.Structure):
@@ -55,6 +56,7 @@ def lib():
         L.cb_clip_adam_scratch_bytes.restype = C.c_size_t
         L.cb_clip_adam_scratch_bytes.argtypes = [C.c_size_t]
         L.cb_last_error.restype = C.c_char_p
+        L.cb_launch_count.restype = C.c_uint64
         L.cb_net_destroy.restype = None
         L.cb_net_destroy.argtypes = [C.c_void_p]
         _lib = L
@@ -240,3 +242,23 @@ def clip_adam(params, adam_m, adam_v, grad, k, lr, beta1=0.9, beta2=0.999, eps=1
     _check(lib().cb_clip_adam(C.c_size_t(P), _ptr(params), _ptr(adam_m), _ptr(adam_v), _ptr(grad), C.c_uint64(k), C.c_float(lr), C.c_float(beta1),
                               C.c_float(beta2), C.c_float(eps), C.c_float(max_norm), _ptr(gn), _ptr(scratch), _stream()))
     return gn
+
+
+# ---- instrumentation ----------------------------------------------------------------------------------
+class CProfEntry(C.Structure):
+    _fields_ = [("cls", C.c_int), ("name", C.c_char * 28), ("launches", C.c_uint64), ("ms", C.c_double), ("flops", C.c_double), ("bytes", C.c_double)]
+
+
+def launch_count():
+    return int(lib().cb_launch_count())
+
+
+def profile_begin(only_class=-1):
+    _check(lib().cb_profile_begin(C.c_int(only_class)))
+
+
+def profile_end():
+    """[{cls, name, launches, ms, flops, bytes}] for every kernel class launched since profile_begin (synchronises)."""
+    buf = (CProfEntry * 32)()
+    n = _check(lib().cb_profile_end(buf, C.c_int(32)))
+    return [dict(cls=e.cls, name=e.name.decode(), launches=int(e.launches), ms=e.ms, flops=e.flops, bytes=e.bytes) for e in buf[:n]]

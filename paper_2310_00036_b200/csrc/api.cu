@@ -360,11 +360,15 @@ int cb_logprob_entropy(const float* logits, int ld, int N, int A, const int32_t*
 }
 int cb_vtrace(int T, int B, const float* V, const float* r, const uint8_t* d, const float* logpi, const float* logmu, float gamma, float lambda_,
               float rho_bar, float c_bar, float rho_pg_bar, float* vs, float* pgadv, float* rho, void* stream) {
-  if (T < 0 || B < 0 || !V || !r || !d || !logpi || !logmu || !vs || !pgadv) { set_error("bad argument"); return CB_EINVAL; }
+  if (T < 0 || B < 0) { set_error("bad argument"); return CB_EINVAL; }
+  if (T == 0 || B == 0) return CB_OK;
+  if (!V || !r || !d || !logpi || !logmu || !vs || !pgadv) { set_error("null argument"); return CB_EINVAL; }
   return launch_vtrace(T, B, V, 1, r, d, logpi, logmu, gamma, lambda_, rho_bar, c_bar, rho_pg_bar, vs, pgadv, rho, (cudaStream_t)stream);
 }
 int cb_gae(int T, int B, const float* V, const float* r, const uint8_t* d, float gamma, float lambda_, float* adv, float* ret, void* stream) {
-  if (T < 0 || B < 0 || !V || !r || !d || !adv || !ret) { set_error("bad argument"); return CB_EINVAL; }
+  if (T < 0 || B < 0) { set_error("bad argument"); return CB_EINVAL; }
+  if (T == 0 || B == 0) return CB_OK;
+  if (!V || !r || !d || !adv || !ret) { set_error("null argument"); return CB_EINVAL; }
   return launch_gae(T, B, V, 1, r, d, gamma, lambda_, adv, ret, (cudaStream_t)stream);
 }
 int cb_permutation(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* stream) {

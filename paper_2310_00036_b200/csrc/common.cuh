@@ -108,6 +108,15 @@ void set_error(const char* fmt, ...);
 int cuda_fail(cudaError_t e, const char* what);
 #define CB_CUDA(x) do { cudaError_t e__ = (x); if (e__ != cudaSuccess) return cb::cuda_fail(e__, #x); } while (0)
 
+// prof.cu -- launch counter and per-class event timing
+enum KClass { K_PACK = 0, K_CONV_FWD, K_POOL_FWD, K_CONV_DGRAD, K_CONV_WGRAD, K_WGRAD_REDUCE, K_POOL_BWD, K_HEAD_MISC, K_LOGPROB,
+              K_SCAN, K_LOSS, K_STATS, K_PERM, K_SQNORM, K_ADAM, K_SAMPLE, K_COUNT };
+struct ProfScope {      // counts `n` launches of class `cls`; records an event pair around them when profiling
+  ProfScope(int cls, cudaStream_t st, int n = 1, double flops = 0.0, double bytes = 0.0);
+  ~ProfScope();
+  int slot; cudaStream_t st;
+};
+
 // net.cu
 int ensure_workspace(cb_net* net, int prec, int frames);
 int ensure_learner_scratch(cb_net* net, int prec, int F, int N, int epochs);

@@ -22,6 +22,7 @@ __global__ void pack_kernel(const float* __restrict__ params, Geom g, ParamMap p
 
 template <typename AT>
 static int pack_all(cb_net* net, Workspace& ws, const float* params, cudaStream_t st) {
+  ProfScope ps(K_PACK, st, (int)net->layers.size(), 0.0, (double)net->P * (4 + 2 * sizeof(AT)));
   for (auto& L : net->layers) {
     size_t total = (size_t)L.g.kh * L.g.kw * L.g.Cin * L.g.Cout;
     int blocks = (int)std::min<size_t>((total + 255) / 256, 1184);
@@ -124,6 +125,7 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
   for (const Op& op : net->fwd) {
     if (op.kind == OP_POOL) {
       size_t total = (size_t)F * pool_out(op.H) * pool_out(op.W) * op.C;
+      ProfScope ps(K_POOL_FWD, st, 1, 0.0, (double)sizeof(AT) * (total + (double)F * op.H * op.W * op.C));
       pool_fwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (AT*)ws.act[op.out_t], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());
       continue;
@@ -133,6 +135,8 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     int M = F * g.Ho * g.Wo, N = g.Cout, K = g.kh * g.kw * g.Cin;
     const AT* wf = (const AT*)ws.wf + L.wf_off; const float* bias = ws.bias + L.bias_off;
     const AT* skip = L.skip_t >= 0 ? (const AT*)ws.act[L.skip_t] : nullptr;
+    double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
+    ProfScope ps(K_CONV_FWD, st, 1, 2.0 * M * N * K, in_bytes + (double)M * N * (L.f32_out ? 4 : sizeof(AT)) * (skip ? 2 : 1) + (double)K * N * sizeof(AT));
     int rc;
     if (L.u8_in) {
       FwdProblem<AT, AT, true> p{M, N, K, K, {g, obs, frame_idx, false}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f / 255.0f};
@@ -159,6 +163,7 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
   for (const Op& op : net->bwd) {
     if (op.kind == OP_POOLBWD) {
       size_t total = (size_t)F * op.H * op.W * op.C;
+      ProfScope ps(K_POOL_BWD, st, 1, 0.0, (double)sizeof(AT) * (2.0 * total + (double)F * pool_out(op.H) * pool_out(op.W) * op.C));
       pool_bwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (const AT*)ws.grad[op.dy], (AT*)ws.grad[op.dx], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());
       continue;
@@ -168,7 +173,10 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
     if (op.kind == OP_WGRAD) {
       int Kpix = F * g.Ho * g.Wo, M = g.kh * g.kw * g.Cin + 1, N = g.Cout, splits, kchunk;
       wgrad_split(Kpix, &splits, &kchunk);
+      double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
       int rc;
+      {
+      ProfScope ps(K_CONV_WGRAD, st, 1, 2.0 * (M - 1) * N * (double)Kpix, in_bytes + (double)Kpix * N * sizeof(AT) + (double)M * N * 4);
       if (L.u8_in) {
         WgradProblem<AT, AT, true> p{M, N, Kpix, kchunk, {g, obs, frame_idx, false}, (const AT*)ws.grad[op.dy], ws.partial};
         rc = launch_gemm(p, splits, st);
@@ -176,11 +184,16 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         WgradProblem<AT, AT, false> p{M, N, Kpix, kchunk, {g, ws.act[L.in_t], nullptr, L.relu_in}, (const AT*)ws.grad[op.dy], ws.partial};
         rc = launch_gemm(p, splits, st);
       }
+      }
       if (rc) return rc;
+      ProfScope ps2(K_WGRAD_REDUCE, st, 1, 0.0, (double)(splits + 1) * M * N * 4);
       wgrad_reduce_kernel<<<grid_for((size_t)M * N), 256, 0, st>>>(ws.partial, splits, g, L.pm, L.u8_in ? 1.0f / 255.0f : 1.0f, grad);
       CB_CUDA(cudaGetLastError());
     } else {  // OP_DGRAD
       int M = F * g.H * g.W, N = g.Cin, K = g.kh * g.kw * g.Cout;
+      // useful MACs of dgrad = those of the forward layer (stride > 1 makes most gathered taps empty)
+      ProfScope ps(K_CONV_DGRAD, st, 1, 2.0 * F * g.Ho * g.Wo * (double)g.Cout * g.kh * g.kw * g.Cin,
+                   (double)sizeof(AT) * ((double)F * g.Ho * g.Wo * g.Cout + (double)M * N * (1 + (op.mask_t >= 0) + (op.add >= 0)) + (double)K * N));
       DgradProblem<AT> p{M, N, K, K, g, (const AT*)ws.grad[op.dy], (const AT*)ws.wd + L.wd_off,
                          op.mask_t >= 0 ? (const AT*)ws.act[op.mask_t] : nullptr,
                          op.add >= 0 ? (const AT*)ws.grad[op.add] : nullptr, (AT*)ws.grad[op.dx]};

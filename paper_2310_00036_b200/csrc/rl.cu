@@ -70,6 +70,7 @@ __global__ void sample_kernel(const float* __restrict__ logits, int ld, int B, i
 
 int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset, int32_t* actions, cudaStream_t st) {
   if (B <= 0) return CB_OK;
+  ProfScope ps(K_SAMPLE, st);
   sample_kernel<<<(B + 63) / 64, 64, 0, st>>>(logits, ld, B, A, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step, (uint32_t)(step >> 32), env_offset, actions);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -84,6 +85,7 @@ __global__ void split_head_kernel(const float* __restrict__ head, int F, int A, 
 }
 int launch_split_head(const float* head, int F, int A, float* logits, float* value, cudaStream_t st) {
   size_t total = (size_t)F * (A + 1); if (!total) return CB_OK;
+  ProfScope ps(K_HEAD_MISC, st);
   split_head_kernel<<<(int)std::min<size_t>((total + 255) / 256, 2368), 256, 0, st>>>(head, F, A, logits, value);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -125,6 +127,7 @@ __global__ void logprob_kernel(const float* __restrict__ logits, int ld, int N, 
 }
 int launch_logprob(const float* logits, int ld, int N, int A, const int32_t* actions, const int32_t* idx, float* logp_a, float* entropy, cudaStream_t st) {
   if (N <= 0) return CB_OK;
+  ProfScope ps(K_LOGPROB, st, 1, 0.0, (double)N * (ld * 4.0 + 12));
   logprob_kernel<<<(N + 127) / 128, 128, 0, st>>>(logits, ld, N, A, actions, idx, logp_a, entropy);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -159,6 +162,7 @@ __global__ void vtrace_kernel(int T, int B, const float* __restrict__ V, int ldV
 int launch_vtrace(int T, int B, const float* V, int ldV, const float* r, const uint8_t* d, const float* logpi, const float* logmu,
                   float gamma, float lam, float rho_bar, float c_bar, float rho_pg_bar, float* vs, float* pgadv, float* rho, cudaStream_t st) {
   if (B <= 0 || T <= 0) return CB_OK;
+  ProfScope ps(K_SCAN, st, 1, 0.0, (double)T * B * (4 * 4 + 1 + 3 * 4) + B * 4.0);
   vtrace_kernel<<<(B + 127) / 128, 128, 0, st>>>(T, B, V, ldV, r, d, logpi, logmu, gamma, lam, rho_bar, c_bar, rho_pg_bar, vs, pgadv, rho);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -180,6 +184,7 @@ __global__ void gae_kernel(int T, int B, const float* __restrict__ V, int ldV, c
 }
 int launch_gae(int T, int B, const float* V, int ldV, const float* r, const uint8_t* d, float gamma, float lam, float* adv, float* ret, cudaStream_t st) {
   if (B <= 0 || T <= 0) return CB_OK;
+  ProfScope ps(K_SCAN, st, 1, 0.0, (double)T * B * (2 * 4 + 1 + 2 * 4) + B * 4.0);
   gae_kernel<<<(B + 127) / 128, 128, 0, st>>>(T, B, V, ldV, r, d, gamma, lam, adv, ret);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -211,6 +216,7 @@ __global__ void permutation_kernel(uint32_t k0, uint32_t k1, uint32_t epoch0, in
 }
 int launch_permutation(uint64_t seed, uint32_t epoch0, int n_epochs, int N, int32_t* perm, uint32_t* jbuf, cudaStream_t st) {
   if (N <= 0 || n_epochs <= 0) return CB_OK;
+  ProfScope ps(K_PERM, st);
   permutation_kernel<<<n_epochs, 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), epoch0, N, perm, jbuf);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -282,8 +288,10 @@ int launch_impala_loss(int prec, int N, int A, const float* head, const int32_t*
   if (A > MAX_A) { set_error("n_actions > %d", MAX_A); return CB_EINVAL; }
   float inv = reduction == 0 ? (float)(1.0 / (double)N) : 1.0f;
   int grid = (N + 127) / 128;
+  { ProfScope ps(K_LOSS, st, 1, 0.0, (double)N * ((A + 1) * (4.0 + (prec ? 2 : 4)) + 16 + 20));
   if (prec == CB_PREC_FP32_REF) impala_loss_kernel<float, double><<<grid, 128, 0, st>>>(N, A, head, act, vs, pgadv, rho, c1, c2, inv, (float*)dhead, terms);
-  else impala_loss_kernel<bf16, float><<<grid, 128, 0, st>>>(N, A, head, act, vs, pgadv, rho, c1, c2, inv, (bf16*)dhead, terms);
+  else impala_loss_kernel<bf16, float><<<grid, 128, 0, st>>>(N, A, head, act, vs, pgadv, rho, c1, c2, inv, (bf16*)dhead, terms); }
+  ProfScope ps2(K_STATS, st, 1, 0.0, (double)N * 20);
   stats_kernel<<<1, 1024, 0, st>>>(N, terms, 0, c1, c2, reduction, stats);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -340,10 +348,12 @@ int launch_ppo_loss(int prec, int m, int A, const float* head, const int32_t* id
                     const float* logp_old, float eps, float c1, float c2, int norm_adv, void* dhead, float* terms, double* red, float*,
                     float* stats, cudaStream_t st) {
   if (A > MAX_A) { set_error("n_actions > %d", MAX_A); return CB_EINVAL; }
-  if (norm_adv) adv_stats_kernel<<<1, 1024, 0, st>>>(m, idx, adv, red);
+  if (norm_adv) { ProfScope ps0(K_STATS, st); adv_stats_kernel<<<1, 1024, 0, st>>>(m, idx, adv, red); }
   int grid = (m + 127) / 128;
+  { ProfScope ps(K_LOSS, st, 1, 0.0, (double)m * ((A + 1) * (4.0 + (prec ? 2 : 4)) + 20 + 20));
   if (prec == CB_PREC_FP32_REF) ppo_loss_kernel<float, double><<<grid, 128, 0, st>>>(m, A, head, idx, act, adv, ret, logp_old, eps, c1, c2, norm_adv, red, (float*)dhead, terms);
-  else ppo_loss_kernel<bf16, float><<<grid, 128, 0, st>>>(m, A, head, idx, act, adv, ret, logp_old, eps, c1, c2, norm_adv, red, (bf16*)dhead, terms);
+  else ppo_loss_kernel<bf16, float><<<grid, 128, 0, st>>>(m, A, head, idx, act, adv, ret, logp_old, eps, c1, c2, norm_adv, red, (bf16*)dhead, terms); }
+  ProfScope ps2(K_STATS, st, 1, 0.0, (double)m * 20);
   stats_kernel<<<1, 1024, 0, st>>>(m, terms, 1, c1, c2, 0, stats);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -413,10 +423,12 @@ int launch_clip_adam(size_t P, float* params, float* m, float* v, const float* g
   if (P == 0) return CB_OK;
   int nparts = (int)((P + NORM_CHUNK - 1) / NORM_CHUNK);
   double* partial = (double*)scratch + 1; double* norm = (double*)scratch;
+  { ProfScope ps(K_SQNORM, st, 2, 0.0, (double)P * 4);
   sqnorm_partial_kernel<<<nparts, 256, 0, st>>>(P, g, partial);
-  sqnorm_final_kernel<<<1, 256, 0, st>>>(nparts, partial, norm, grad_norm, stats_slot);
+  sqnorm_final_kernel<<<1, 256, 0, st>>>(nparts, partial, norm, grad_norm, stats_slot); }
   double bc1 = 1.0 - pow((double)b1, (double)k), bc2 = 1.0 - pow((double)b2, (double)k);
   int grid = (int)std::min<size_t>((P / 4 + 255) / 256, (size_t)148 * 8); if (grid < 1) grid = 1;
+  ProfScope ps(K_ADAM, st, 1, 0.0, (double)P * 28);
   adam_kernel<<<grid, 256, 0, st>>>(P, params, m, v, g, norm, max_norm, b1, (float)(1.0 - (double)b1), b2, (float)(1.0 - (double)b2),
                                     (float)(1.0 / bc1), (float)(1.0 / bc2), lr, eps);
   CB_CUDA(cudaGetLastError());

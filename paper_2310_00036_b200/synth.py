@@ -76,14 +76,17 @@ def param_count(arch):
     return int(sum(int(np.prod(s)) for _, s, _ in param_tensors(arch)))
 
 
-def gen_params(arch, seed, bias_scale=0.0):
+def gen_params(arch, seed, bias_scale=0.0, head_scale=1.0):
     """He-normal weights N(0, 2/fan_in), biases 0 (reading A14) -- or small random biases when
-    bias_scale > 0 so that bias-gradient paths are exercised by parity tests."""
+    bias_scale > 0 so that bias-gradient paths are exercised by parity tests.  head_scale < 1 shrinks
+    pi.w and v.w so that logits and values are O(1), the regime of an Atari agent trained on rewards
+    in {-1,0,+1} (raw He-init heads on unnormalised frames give |V| ~ 10); DESIGN.md section 4."""
     g = rng(seed); parts = []
     for name, shape, fan in param_tensors(arch):
         n = int(np.prod(shape))
         if name.endswith(".w"):
-            parts.append(g.standard_normal(n) * np.sqrt(2.0 / fan))
+            sc = head_scale if name in ("pi.w", "v.w") else 1.0
+            parts.append(g.standard_normal(n) * np.sqrt(2.0 / fan) * sc)
         else:
             parts.append(g.standard_normal(n) * bias_scale)
     return np.concatenate(parts).astype(np.float32)

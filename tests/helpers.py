@@ -33,3 +33,14 @@ def rel_l2(got, ref):
     return float(np.linalg.norm(got - ref) / max(np.linalg.norm(ref), 1e-30))
 
 
+
+
+def close_bf16(got, ref, what="", rtol=2e-2):
+    """CB_PREC_BF16_TC gate for network outputs (reading A15b): relative L2 error of the tensor <= 2e-2
+    (north_star's number) and no element further than 2e-2 * max(|a|,|b|) + 8e-2 * RMS(ref) (outlier
+    bound: ~6 sigma of the accumulated bf16 rounding noise derived in DESIGN.md section 3)."""
+    got = np.asarray(got, np.float64); ref = np.asarray(ref, np.float64)
+    assert got.shape == ref.shape and np.isfinite(got).all(), what
+    e = rel_l2(got, ref)
+    assert e <= rtol, f"{what}: relative L2 error {e:.3e} > {rtol}"
+    close(got, ref, rtol, atol_rms=4.0, what=what)
