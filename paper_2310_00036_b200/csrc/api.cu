@@ -156,6 +156,8 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
   size_t es = prec == CB_PREC_FP32_REF ? 4 : 2;
   if (!ws.wf) {
     CB_ALLOC(ws.wf, net->wf_total * es); CB_ALLOC(ws.wd, net->wd_total * es); CB_ALLOC(ws.bias, net->bias_total * 4);
+    if (prec == CB_PREC_BF16_TC) { CB_ALLOC(ws.wtc_f, net->wf_total * 2); CB_ALLOC(ws.wtc_d, net->wf_total * 2); }
+    CB_ALLOC(ws.errflag, 16); CB_CUDA(cudaMemset(ws.errflag, 0, 16));
     CB_ALLOC(ws.gradbuf, net->P * 4); CB_ALLOC(ws.adam_scratch, clip_adam_scratch_bytes(net->P)); CB_ALLOC(ws.gnorm, 16);
   }
   if (ws.frames >= frames) return CB_OK;
@@ -229,6 +231,7 @@ void cb_net_destroy(cb_net* net) {
     Workspace& ws = net->ws[p];
     if (!ws.wf) continue;
     free_workspace(ws); free_scratch(ws);
+    cudaFree(ws.wtc_f); cudaFree(ws.wtc_d); cudaFree(ws.errflag);
     cudaFree(ws.wf); cudaFree(ws.wd); cudaFree(ws.bias); cudaFree(ws.gradbuf); cudaFree(ws.adam_scratch); cudaFree(ws.gnorm);
   }
   delete net;
@@ -340,6 +343,9 @@ int cb_learner_step(cb_net* net, float* params, float* adam_m, float* adam_v, ui
 int cb_learner_view(const cb_net* net, int which, const void** dev_ptr, size_t* count) {
   if (!net || !dev_ptr || !count || net->last_prec < 0) { set_error("no learner step has run on this net"); return CB_EINVAL; }
   const Workspace& ws = net->ws[net->last_prec]; int A = net->arch.n_actions;
+  int flag = 0;
+  CB_CUDA(cudaMemcpy(&flag, ws.errflag, sizeof flag, cudaMemcpyDeviceToHost));
+  if (flag) { set_error("a tcgen05 pipeline wait timed out inside the last learner step"); return CB_ECUDA; }
   switch (which) {
     case 0: *dev_ptr = net->last_ppo ? (const void*)ws.values : (const void*)ws.act[net->head_t]; *count = (size_t)net->last_F * (A + 1); break;
     case 1: *dev_ptr = ws.t0; *count = net->last_N; break;

@@ -70,6 +70,8 @@ struct Workspace {     // one per precision mode
   std::vector<void*> act;            // per tensor, [frames * per_frame]
   void* grad[G_COUNT] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   void* wf = nullptr; void* wd = nullptr; float* bias = nullptr;   // packed weights (mode type), fp32 bias
+  bf16* wtc_f = nullptr; bf16* wtc_d = nullptr;                     // tcgen05 B-operand packs (forward / dgrad), bf16 mode only
+  int* errflag = nullptr;                                          // set by a kernel whose tcgen05 pipeline timed out
   float* partial = nullptr; size_t partial_elems = 0;             // wgrad split-K partials
   float* gradbuf = nullptr;          // [P]
   // learner scratch (fp32 unless noted)
@@ -123,6 +125,11 @@ int ensure_learner_scratch(cb_net* net, int prec, int F, int N, int epochs);
 int pack_weights(cb_net* net, int prec, const float* params, cudaStream_t st);
 int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st);
 int backward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, float* grad, cudaStream_t st);
+
+// conv_tc.cu
+bool conv_tc_supported(const Geom& g);
+int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16* in, const bf16* w, const float* bias, const bf16* aux0,
+                   const bf16* aux1, bf16* out, bool relu_in, int* error_flag, cudaStream_t st);
 
 // rl.cu
 int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset,

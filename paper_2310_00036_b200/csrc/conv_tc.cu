@@ -1,0 +1,275 @@
+// tcgen05 / TMEM implicit-GEMM 3x3 convolution (stride 1, zero pad 1) for CB_PREC_BF16_TC, sm_100a.
+//
+// One kernel serves the forward conv and its dgrad (the same convolution with flipped taps and
+// transposed weights; only the packed weights and the epilogue differ).
+//
+// Data layout in shared memory ("pixel-linear planes"): a group of G frames is staged with its zero
+// halo as  plane[c/8][j*R + (y+1)*Wp + (x+1)][c%8],  R = (H+2)*(W+2), Wp = W+2, 16 bytes per (pixel,
+// channel-chunk).  For an output position q = j*R + y*Wp + x the input under tap (di,dj) is at the
+// linear position q + di*Wp + dj: a tap is a constant shift of the start address.  A 128-row A operand
+// (128 consecutive linear positions, 16 channels) is therefore exactly the canonical K-major
+// no-swizzle UMMA layout (core matrix = 8 pixels x 16 B, SBO = 128 B, LBO = plane stride) for ANY tap,
+// and the whole 3x3 conv is 9*Cin/16 tcgen05.mma instructions per 128-position tile with the fp32
+// accumulator resident in TMEM.  Positions that fall on halo columns/rows are computed and dropped
+// (6-40% of the rows, the price of needing no im2col and no per-tap copies).
+// Weights: B operand [Cout x 16] per (tap, k-step), K-major canonical layout, staged once per CTA.
+#include "common.cuh"
+
+namespace cb {
+
+namespace tc {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// UMMA shared-memory matrix descriptor, no swizzle (layout_type 0), version 1 (Blackwell)
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = (uint64_t)((saddr >> 4) & 0x3FFFu);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
+  d |= (uint64_t)1 << 46;
+  return d;
+}
+// instruction descriptor, kind::f16: D fp32, A/B bf16; a_major/b_major: 0 = K-major, 1 = MN-major
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N, int a_mn, int b_mn) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void mma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
+               :: "r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void mma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" :: "r"(bar), "r"(count) : "memory");
+  asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+}
+// bounded spin: a descriptor mistake must not hang the GPU box; returns false on timeout
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity) {
+  for (uint32_t it = 0; it < (1u << 24); ++it) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return true;
+  }
+  return false;
+}
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t cols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" :: "r"(dst_smem), "r"(cols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t cols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(taddr), "r"(cols) : "memory");
+}
+// 16 consecutive fp32 columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
+  uint32_t r[16];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                 "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+               : "r"(taddr) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+struct ConvTcArgs {
+  const bf16* in;      // [F, H, W, CIN]
+  const bf16* w;       // packed B operand: [tap][CIN/8][COUT][8]
+  const float* bias;   // [COUT] (forward) or nullptr
+  const bf16* aux0;    // forward: skip tensor (added) | dgrad: pre-activation whose sign gates the result; nullable
+  const bf16* aux1;    // dgrad: gradient added after gating; nullable
+  bf16* out;           // [F, H, W, COUT]
+  int F, H, W, G, npix_alloc, relu_in;
+  int* error_flag;
+};
+
+constexpr int TMEM_COLS = 256;
+
+// MODE 0: out = acc + bias (+ aux0).   MODE 1: out = (aux0 ? (aux0 > 0 ? acc : 0) : acc) (+ aux1).
+template <int CIN, int COUT, int MODE>
+__global__ void __launch_bounds__(128) conv3x3_tc_kernel(const ConvTcArgs a) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  constexpr int NCH = CIN / 8, KSTEPS = CIN / 16, TILES_PER_BATCH = TMEM_COLS / COUT;
+  constexpr uint32_t W_BYTES = 9u * CIN * COUT * 2u;
+  __shared__ __align__(8) uint64_t bar_storage;
+  __shared__ uint32_t tmem_base_smem;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int Wp = a.W + 2, R = (a.H + 2) * Wp;
+  uint8_t* w_smem = smem;
+  uint8_t* in_smem = smem + ((W_BYTES + 127u) & ~127u);
+  const uint32_t plane_bytes = (uint32_t)a.npix_alloc * 16u;
+  const uint32_t bar = smem_u32(&bar_storage);
+
+  if (tid == 0) mbar_init(bar, 1);
+  if (warp == 0) tmem_alloc(smem_u32(&tmem_base_smem), TMEM_COLS);
+  // weights (already in operand layout) and a zeroed input area (halo and slack stay zero for the whole kernel)
+  for (uint32_t i = tid; i < W_BYTES / 16; i += 128) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w)[i];
+  for (uint32_t i = tid; i < plane_bytes * NCH / 16; i += 128) reinterpret_cast<uint4*>(in_smem)[i] = make_uint4(0, 0, 0, 0);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_smem;
+  const uint32_t idesc = make_idesc(128, COUT, 0, 0);
+  const uint32_t a_base = smem_u32(in_smem), b_base = smem_u32(w_smem);
+  uint32_t parity = 0;
+  const int ngroups = (a.F + a.G - 1) / a.G;
+
+  for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    const int f0 = grp * a.G, nf = min(a.G, a.F - f0);
+    // ---- stage the group's frames: global NHWC -> planes, ReLU on the way in --------------------------
+    const int per_frame = a.H * a.W * NCH;
+    for (int i = tid; i < a.G * per_frame; i += 128) {
+      int j = i / per_frame, rem = i - j * per_frame;
+      int ch = rem % NCH, pix = rem / NCH;
+      int y = pix / a.W, x = pix - y * a.W;
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (j < nf) {
+        v = *reinterpret_cast<const uint4*>(a.in + ((size_t)(f0 + j) * a.H * a.W + pix) * CIN + ch * 8);
+        if (a.relu_in) {
+          __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+          const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
+        }
+      }
+      *reinterpret_cast<uint4*>(in_smem + (size_t)ch * plane_bytes + (size_t)(j * R + (y + 1) * Wp + (x + 1)) * 16) = v;
+    }
+    fence_async_smem();
+    __syncthreads();
+    const int ntiles = (nf * R + 127) / 128;
+    for (int t0 = 0; t0 < ntiles; t0 += TILES_PER_BATCH) {
+      const int nt = min(TILES_PER_BATCH, ntiles - t0);
+      if (tid == 0) {
+        tc_fence_after();
+        for (int s = 0; s < nt; ++s) {
+          const uint32_t q0 = (uint32_t)(t0 + s) * 128u;
+          uint32_t first = 1;
+#pragma unroll
+          for (int tap = 0; tap < 9; ++tap) {
+            const uint32_t shift = (uint32_t)((tap / 3) * Wp + (tap % 3));
+#pragma unroll
+            for (int ks = 0; ks < KSTEPS; ++ks) {
+              uint64_t ad = make_desc(a_base + (q0 + shift) * 16u + (uint32_t)(2 * ks) * plane_bytes, plane_bytes, 128u);
+              uint64_t bd = make_desc(b_base + (uint32_t)((tap * NCH + 2 * ks) * COUT) * 16u, (uint32_t)COUT * 16u, 128u);
+              mma_f16(tmem_base + (uint32_t)(s * COUT), ad, bd, idesc, first ? 0u : 1u);
+              first = 0;
+            }
+          }
+        }
+        mma_commit(bar);
+      }
+      if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 1; }
+      parity ^= 1;
+      tc_fence_after();
+      // ---- epilogue: TMEM lane = tile row = linear position; one thread per position ----------------------
+      for (int s = 0; s < nt; ++s) {
+        const int q = (t0 + s) * 128 + tid;
+        const int j = q / R, rem = q - j * R;
+        const int y = rem / Wp, x = rem - y * Wp;
+        const bool valid = j < nf && y < a.H && x < a.W;
+        const size_t o = (((size_t)(f0 + j) * a.H + y) * a.W + x) * COUT;
+#pragma unroll
+        for (int c0 = 0; c0 < COUT; c0 += 16) {
+          float v[16];
+          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(s * COUT + c0), v);   // warp-collective: no divergence before it
+          if (!valid) continue;
+          if (MODE == 0) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) v[i] += a.bias[c0 + i];
+            if (a.aux0) {
+              uint4 s0 = *reinterpret_cast<const uint4*>(a.aux0 + o + c0), s1 = *reinterpret_cast<const uint4*>(a.aux0 + o + c0 + 8);
+              const bf16* h0 = reinterpret_cast<const bf16*>(&s0); const bf16* h1 = reinterpret_cast<const bf16*>(&s1);
+#pragma unroll
+              for (int i = 0; i < 8; ++i) { v[i] += __bfloat162float(h0[i]); v[8 + i] += __bfloat162float(h1[i]); }
+            }
+          } else {
+            if (a.aux0) {
+              uint4 s0 = *reinterpret_cast<const uint4*>(a.aux0 + o + c0), s1 = *reinterpret_cast<const uint4*>(a.aux0 + o + c0 + 8);
+              const bf16* h0 = reinterpret_cast<const bf16*>(&s0); const bf16* h1 = reinterpret_cast<const bf16*>(&s1);
+#pragma unroll
+              for (int i = 0; i < 8; ++i) { if (!(__bfloat162float(h0[i]) > 0.f)) v[i] = 0.f; if (!(__bfloat162float(h1[i]) > 0.f)) v[8 + i] = 0.f; }
+            }
+            if (a.aux1) {
+              uint4 s0 = *reinterpret_cast<const uint4*>(a.aux1 + o + c0), s1 = *reinterpret_cast<const uint4*>(a.aux1 + o + c0 + 8);
+              const bf16* h0 = reinterpret_cast<const bf16*>(&s0); const bf16* h1 = reinterpret_cast<const bf16*>(&s1);
+#pragma unroll
+              for (int i = 0; i < 8; ++i) { v[i] += __bfloat162float(h0[i]); v[8 + i] += __bfloat162float(h1[i]); }
+            }
+          }
+          uint4 o0, o1;
+          __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
+          *reinterpret_cast<uint4*>(a.out + o + c0) = o0;
+          *reinterpret_cast<uint4*>(a.out + o + c0 + 8) = o1;
+        }
+      }
+      tc_fence_before();
+      __syncthreads();      // TMEM drained and (after the last batch) the staged frames free for the next group
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+}  // namespace tc
+
+// ---- host side ---------------------------------------------------------------------------------
+bool conv_tc_supported(const Geom& g) {
+  auto okc = [](int c) { return c == 16 || c == 32 || c == 64; };
+  return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && okc(g.Cin) && okc(g.Cout) && g.H == g.Ho && g.W == g.Wo;
+}
+
+struct TcPlan { int G, npix_alloc; size_t smem; };
+static TcPlan tc_plan(int H, int W, int cin, int cout) {
+  const int Wp = W + 2, R = (H + 2) * Wp;
+  const size_t wbytes = ((size_t)9 * cin * cout * 2 + 127) & ~(size_t)127;
+  const size_t budget = 96 * 1024;          // two CTAs per SM where the frame allows it
+  int G = (int)((budget > wbytes ? budget - wbytes : 0) / ((size_t)R * cin * 2));
+  if (G < 1) G = 1;
+  if (G > 8) G = 8;
+  int npix = ((G * R + 127) / 128) * 128 + 2 * Wp + 2;
+  npix = (npix + 7) / 8 * 8;
+  return {G, npix, wbytes + (size_t)npix * cin * 2};
+}
+
+template <int CIN, int COUT, int MODE>
+static int launch_one(const tc::ConvTcArgs& a, size_t smem, int ngroups, cudaStream_t st) {
+  static size_t configured = 0;      // largest dynamic size this instantiation has been opted in for
+  if (smem > configured) {
+    CB_CUDA(cudaFuncSetAttribute(tc::conv3x3_tc_kernel<CIN, COUT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = smem;
+  }
+  int grid = std::min(ngroups, 2 * 148);
+  tc::conv3x3_tc_kernel<CIN, COUT, MODE><<<grid, 128, smem, st>>>(a);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+template <int MODE>
+static int dispatch(int cin, int cout, const tc::ConvTcArgs& a, size_t smem, int ngroups, cudaStream_t st) {
+#define CB_TC_CASE(ci, co) if (cin == ci && cout == co) return launch_one<ci, co, MODE>(a, smem, ngroups, st);
+  CB_TC_CASE(16, 16) CB_TC_CASE(16, 32) CB_TC_CASE(32, 16) CB_TC_CASE(32, 32) CB_TC_CASE(32, 64) CB_TC_CASE(64, 32) CB_TC_CASE(64, 64)
+  CB_TC_CASE(16, 64) CB_TC_CASE(64, 16)
+#undef CB_TC_CASE
+  set_error("conv_tc: unsupported channel counts %d -> %d", cin, cout);
+  return CB_EINVAL;
+}
+
+// mode 0: forward (cin = g.Cin, cout = g.Cout);  mode 1: dgrad (cin = g.Cout, cout = g.Cin, weights packed flipped/transposed)
+int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16* in, const bf16* w, const float* bias, const bf16* aux0,
+                   const bf16* aux1, bf16* out, bool relu_in, int* error_flag, cudaStream_t st) {
+  if (F <= 0) return CB_OK;
+  TcPlan p = tc_plan(H, W, cin, cout);
+  if (p.smem > 220 * 1024) { set_error("conv_tc: frame does not fit shared memory"); return CB_EINVAL; }
+  tc::ConvTcArgs a{in, w, bias, aux0, aux1, out, F, H, W, p.G, p.npix_alloc, relu_in ? 1 : 0, error_flag};
+  int ngroups = (F + p.G - 1) / p.G;
+  return mode == 0 ? dispatch<0>(cin, cout, a, p.smem, ngroups, st) : dispatch<1>(cin, cout, a, p.smem, ngroups, st);
+}
+
+}  // namespace cb

@@ -3,6 +3,8 @@
 // conv_tc.cu and are dispatched from here when the shape qualifies.
 #include "gemm_simt.cuh"
 
+#include <type_traits>
+
 namespace cb {
 
 // ---- weight packing: canonical fp32 [Cout,Cin,kh,kw] -> Wf [(di,dj,c)][n], Wd [(di,dj,n)][c], bias fp32 [n]
@@ -20,6 +22,19 @@ __global__ void pack_kernel(const float* __restrict__ params, Geom g, ParamMap p
   }
 }
 
+// tcgen05 B operands (conv_tc.cu): forward [tap][Cin/8][Cout][8]; dgrad [tap'][Cout/8][Cin][8] with flipped taps
+__global__ void pack_tc_kernel(const float* __restrict__ params, Geom g, ParamMap pm, bf16* wtf, bf16* wtd) {
+  size_t total = (size_t)9 * g.Cin * g.Cout;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    int n = (int)(i % g.Cout); size_t q = i / g.Cout; int c = (int)(q % g.Cin); int tap = (int)(q / g.Cin);
+    int di = tap / 3, dj = tap % 3;
+    bf16 v = __float2bfloat16_rn(params[pm.w(n, c, di, dj, g)]);
+    wtf[(((size_t)tap * (g.Cin / 8) + c / 8) * g.Cout + n) * 8 + c % 8] = v;
+    int tapd = (2 - di) * 3 + (2 - dj);
+    wtd[(((size_t)tapd * (g.Cout / 8) + n / 8) * g.Cin + c) * 8 + n % 8] = v;
+  }
+}
+
 template <typename AT>
 static int pack_all(cb_net* net, Workspace& ws, const float* params, cudaStream_t st) {
   ProfScope ps(K_PACK, st, (int)net->layers.size(), 0.0, (double)net->P * (4 + 2 * sizeof(AT)));
@@ -27,6 +42,8 @@ static int pack_all(cb_net* net, Workspace& ws, const float* params, cudaStream_
     size_t total = (size_t)L.g.kh * L.g.kw * L.g.Cin * L.g.Cout;
     int blocks = (int)std::min<size_t>((total + 255) / 256, 1184);
     pack_kernel<AT><<<blocks, 256, 0, st>>>(params, L.g, L.pm, (AT*)ws.wf + L.wf_off, (AT*)ws.wd + L.wd_off, ws.bias + L.bias_off);
+    if (std::is_same<AT, bf16>::value && conv_tc_supported(L.g))
+      pack_tc_kernel<<<blocks, 256, 0, st>>>(params, L.g, L.pm, ws.wtc_f + L.wf_off, ws.wtc_d + L.wf_off);
   }
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -138,7 +155,10 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
     ProfScope ps(K_CONV_FWD, st, 1, 2.0 * M * N * K, in_bytes + (double)M * N * (L.f32_out ? 4 : sizeof(AT)) * (skip ? 2 : 1) + (double)K * N * sizeof(AT));
     int rc;
-    if (L.u8_in) {
+    if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out) {
+      rc = launch_conv_tc(0, F, g.H, g.W, g.Cin, g.Cout, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (const bf16*)skip, nullptr,
+                          (bf16*)ws.act[L.out_t], L.relu_in, ws.errflag, st);
+    } else if (L.u8_in) {
       FwdProblem<AT, AT, true> p{M, N, K, K, {g, obs, frame_idx, false}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f / 255.0f};
       rc = launch_gemm(p, 1, st);
     } else if (L.f32_out) {
@@ -194,6 +214,13 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
       // useful MACs of dgrad = those of the forward layer (stride > 1 makes most gathered taps empty)
       ProfScope ps(K_CONV_DGRAD, st, 1, 2.0 * F * g.Ho * g.Wo * (double)g.Cout * g.kh * g.kw * g.Cin,
                    (double)sizeof(AT) * ((double)F * g.Ho * g.Wo * g.Cout + (double)M * N * (1 + (op.mask_t >= 0) + (op.add >= 0)) + (double)K * N));
+      if (std::is_same<AT, bf16>::value && conv_tc_supported(g)) {
+        int rc = launch_conv_tc(1, F, g.H, g.W, g.Cout, g.Cin, (const bf16*)ws.grad[op.dy], ws.wtc_d + L.wf_off, nullptr,
+                                op.mask_t >= 0 ? (const bf16*)ws.act[op.mask_t] : nullptr, op.add >= 0 ? (const bf16*)ws.grad[op.add] : nullptr,
+                                (bf16*)ws.grad[op.dx], false, ws.errflag, st);
+        if (rc) return rc;
+        continue;
+      }
       DgradProblem<AT> p{M, N, K, K, g, (const AT*)ws.grad[op.dy], (const AT*)ws.wd + L.wd_off,
                          op.mask_t >= 0 ? (const AT*)ws.act[op.mask_t] : nullptr,
                          op.add >= 0 ? (const AT*)ws.grad[op.add] : nullptr, (AT*)ws.grad[op.dx]};
