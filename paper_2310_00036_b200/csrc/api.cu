@@ -169,7 +169,10 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
     CB_ALLOC(ws.act[i], net->tensors[i].per_frame * frames * (net->tensors[i].f32 ? 4 : es));
   for (int i = 0; i < G_COUNT; ++i) CB_ALLOC(ws.grad[i], net->grad_elems[i] * frames * es);
   size_t pe = 0;
-  for (const Layer& L : net->layers) pe = std::max(pe, wgrad_partial_elems(L.g, frames));
+  for (const Layer& L : net->layers) {
+    pe = std::max(pe, wgrad_partial_elems(L.g, frames));
+    if (wgrad_tc_supported(L.g)) pe = std::max(pe, wgrad_tc_partial_elems(L.g));
+  }
   CB_ALLOC(ws.partial, pe * 4); ws.partial_elems = pe;
   ws.frames = frames;
   return CB_OK;

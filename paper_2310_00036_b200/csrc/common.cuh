@@ -131,6 +131,12 @@ bool conv_tc_supported(const Geom& g);
 int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16* in, const bf16* w, const float* bias, const bf16* aux0,
                    const bf16* aux1, bf16* out, bool relu_in, int* error_flag, cudaStream_t st);
 
+// wgrad_tc.cu
+bool wgrad_tc_supported(const Geom& g);
+size_t wgrad_tc_partial_elems(const Geom& g);
+int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
+                    int* error_flag, cudaStream_t st);
+
 // rl.cu
 int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset,
                   int32_t* actions, cudaStream_t st);

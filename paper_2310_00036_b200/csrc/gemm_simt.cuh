@@ -81,6 +81,31 @@ struct DgradProblem {
   }
 };
 
+// dgrad of a layer whose kernel covers its whole input (fc, heads): a plain GEMM
+//   dx[f, (y,x,c)] = sum_o dy[f,o] * w[o,c,y,x],   B read from the dgrad pack Wd[(y,x,o)][c]
+template <typename AT>
+struct DgradFullProblem {
+  static constexpr bool A_K_FAST = true;
+  int M, N, K, kchunk;   // M = F, N = H*W*Cin, K = Cout
+  int Cin; const AT* dy; const AT* wd; const AT* mask; const AT* add; AT* dx;
+  struct RowA { int m; bool ok; };
+  struct ColA { int k; bool ok; };
+  __device__ RowA rowA(int m) const { return {m, m < M}; }
+  __device__ ColA colA(int k) const { return {k, k < K}; }
+  __device__ float loadA(const RowA& r, const ColA& c) const { return (r.ok && c.ok) ? ldv(dy, (size_t)r.m * K + c.k) : 0.f; }
+  __device__ float loadB(int k, int n) const {
+    if (k >= K || n >= N) return 0.f;
+    int t = n / Cin, c = n - t * Cin;
+    return ldv(wd, ((size_t)t * K + k) * Cin + c);
+  }
+  __device__ void store(int m, int n, float acc, int) const {
+    size_t i = (size_t)m * N + n; float v = acc;
+    if (mask && !(ldv(mask, i) > 0.f)) v = 0.f;
+    if (add) v += ldv(add, i);
+    stv(dx, i, v);
+  }
+};
+
 template <typename AT, typename GT, bool U8>
 struct WgradProblem {
   static constexpr bool A_K_FAST = false;

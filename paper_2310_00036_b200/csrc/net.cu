@@ -107,6 +107,73 @@ __global__ void pool_bwd_kernel(const AT* __restrict__ x, const AT* __restrict__
   }
 }
 
+// 8-channel (16-byte) vectorised variants for bf16 maps with C % 8 == 0: one thread per (pixel, chunk)
+__device__ __forceinline__ void bf8_to_f(const uint4& u, float* f) {
+  const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&u);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { float2 t = __bfloat1622float2(h[i]); f[2 * i] = t.x; f[2 * i + 1] = t.y; }
+}
+__device__ __forceinline__ uint4 f_to_bf8(const float* f) {
+  uint4 u; __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&u);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(f[2 * i], f[2 * i + 1]);
+  return u;
+}
+__global__ void pool_fwd_v8_kernel(const bf16* __restrict__ x, bf16* __restrict__ y, int F, int C, int H, int W) {
+  int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W), C8 = C / 8;
+  size_t total = (size_t)F * Ho * Wo * C8;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    int c8 = (int)(i % C8); size_t q = i / C8; int ox = (int)(q % Wo); q /= Wo; int oy = (int)(q % Ho); size_t f = q / Ho;
+    float best[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) best[k] = -INFINITY;
+    for (int di = 0; di < 3; ++di) {
+      int iy = oy * 2 + di - ph; if ((unsigned)iy >= (unsigned)H) continue;
+      for (int dj = 0; dj < 3; ++dj) {
+        int ix = ox * 2 + dj - pw; if ((unsigned)ix >= (unsigned)W) continue;
+        float v[8]; bf8_to_f(*reinterpret_cast<const uint4*>(x + ((f * H + iy) * W + ix) * C + c8 * 8), v);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) if (v[k] > best[k]) best[k] = v[k];
+      }
+    }
+    *reinterpret_cast<uint4*>(y + i * 8) = f_to_bf8(best);
+  }
+}
+__global__ void pool_bwd_v8_kernel(const bf16* __restrict__ x, const bf16* __restrict__ dy, bf16* __restrict__ dx, int F, int C, int H, int W) {
+  int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W), C8 = C / 8;
+  size_t total = (size_t)F * H * W * C8;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    int c8 = (int)(i % C8); size_t q = i / C8; int ix = (int)(q % W); q /= W; int iy = (int)(q % H); size_t f = q / H;
+    float g[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) g[k] = 0.f;
+    int oy_lo = (iy + ph - 2 + 1) / 2; if (iy + ph - 2 < 0) oy_lo = 0;
+    int ox_lo = (ix + pw - 2 + 1) / 2; if (ix + pw - 2 < 0) ox_lo = 0;
+    int oy_hi = min((iy + ph) / 2, Ho - 1), ox_hi = min((ix + pw) / 2, Wo - 1);
+    for (int oy = oy_lo; oy <= oy_hi; ++oy)
+      for (int ox = ox_lo; ox <= ox_hi; ++ox) {
+        float best[8]; int bidx[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { best[k] = -INFINITY; bidx[k] = -1; }
+        for (int di = 0; di < 3; ++di) {
+          int yy = oy * 2 + di - ph; if ((unsigned)yy >= (unsigned)H) continue;
+          for (int dj = 0; dj < 3; ++dj) {
+            int xx = ox * 2 + dj - pw; if ((unsigned)xx >= (unsigned)W) continue;
+            float v[8]; bf8_to_f(*reinterpret_cast<const uint4*>(x + ((f * H + yy) * W + xx) * C + c8 * 8), v);
+            int id = yy * W + xx;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) if (v[k] > best[k]) { best[k] = v[k]; bidx[k] = id; }
+          }
+        }
+        float d[8]; bf8_to_f(*reinterpret_cast<const uint4*>(dy + ((f * Ho + oy) * Wo + ox) * C + c8 * 8), d);
+        int me = iy * W + ix;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) if (bidx[k] == me) g[k] += d[k];
+      }
+    *reinterpret_cast<uint4*>(dx + i * 8) = f_to_bf8(g);
+  }
+}
+
 // ---- wgrad second pass: sum split-K partials in split order, scale, scatter to canonical grad ----
 __global__ void wgrad_reduce_kernel(const float* __restrict__ partial, int splits, Geom g, ParamMap pm, float in_scale, float* __restrict__ grad) {
   int Kw = g.kh * g.kw * g.Cin, M = Kw + 1, N = g.Cout;
@@ -143,7 +210,10 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     if (op.kind == OP_POOL) {
       size_t total = (size_t)F * pool_out(op.H) * pool_out(op.W) * op.C;
       ProfScope ps(K_POOL_FWD, st, 1, 0.0, (double)sizeof(AT) * (total + (double)F * op.H * op.W * op.C));
-      pool_fwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (AT*)ws.act[op.out_t], F, op.C, op.H, op.W);
+      if (std::is_same<AT, bf16>::value && op.C % 8 == 0)
+        pool_fwd_v8_kernel<<<grid_for(total / 8), 256, 0, st>>>((const bf16*)ws.act[op.in_t], (bf16*)ws.act[op.out_t], F, op.C, op.H, op.W);
+      else
+        pool_fwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (AT*)ws.act[op.out_t], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());
       continue;
     }
@@ -184,13 +254,23 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
     if (op.kind == OP_POOLBWD) {
       size_t total = (size_t)F * op.H * op.W * op.C;
       ProfScope ps(K_POOL_BWD, st, 1, 0.0, (double)sizeof(AT) * (2.0 * total + (double)F * pool_out(op.H) * pool_out(op.W) * op.C));
-      pool_bwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (const AT*)ws.grad[op.dy], (AT*)ws.grad[op.dx], F, op.C, op.H, op.W);
+      if (std::is_same<AT, bf16>::value && op.C % 8 == 0)
+        pool_bwd_v8_kernel<<<grid_for(total / 8), 256, 0, st>>>((const bf16*)ws.act[op.in_t], (const bf16*)ws.grad[op.dy], (bf16*)ws.grad[op.dx], F, op.C, op.H, op.W);
+      else
+        pool_bwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (const AT*)ws.grad[op.dy], (AT*)ws.grad[op.dx], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());
       continue;
     }
     const Layer& L = net->layers[op.layer];
     const Geom& g = L.g;
     if (op.kind == OP_WGRAD) {
+      if (std::is_same<AT, bf16>::value && wgrad_tc_supported(g)) {
+        ProfScope ps(K_CONV_WGRAD, st, 2, 2.0 * 9 * g.Cin * g.Cout * (double)F * g.Ho * g.Wo,
+                     2.0 * F * g.H * g.W * (g.Cin + g.Cout) + 4.0 * 9 * (g.Cin + 1) * g.Cout);
+        int rc = launch_wgrad_tc(g, L.pm, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.grad[op.dy], L.relu_in, ws.partial, grad, ws.errflag, st);
+        if (rc) return rc;
+        continue;
+      }
       int Kpix = F * g.Ho * g.Wo, M = g.kh * g.kw * g.Cin + 1, N = g.Cout, splits, kchunk;
       wgrad_split(Kpix, &splits, &kchunk);
       double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
@@ -218,6 +298,14 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         int rc = launch_conv_tc(1, F, g.H, g.W, g.Cout, g.Cin, (const bf16*)ws.grad[op.dy], ws.wtc_d + L.wf_off, nullptr,
                                 op.mask_t >= 0 ? (const bf16*)ws.act[op.mask_t] : nullptr, op.add >= 0 ? (const bf16*)ws.grad[op.add] : nullptr,
                                 (bf16*)ws.grad[op.dx], false, ws.errflag, st);
+        if (rc) return rc;
+        continue;
+      }
+      if (g.Ho == 1 && g.Wo == 1 && g.kh == g.H && g.kw == g.W && g.p == 0) {
+        int Nf = g.H * g.W * g.Cin;
+        DgradFullProblem<AT> pf{F, Nf, g.Cout, g.Cout, g.Cin, (const AT*)ws.grad[op.dy], (const AT*)ws.wd + L.wd_off,
+                                op.mask_t >= 0 ? (const AT*)ws.act[op.mask_t] : nullptr, op.add >= 0 ? (const AT*)ws.grad[op.add] : nullptr, (AT*)ws.grad[op.dx]};
+        int rc = launch_gemm(pf, 1, st);
         if (rc) return rc;
         continue;
       }

@@ -1,0 +1,250 @@
+// tcgen05 / TMEM weight-gradient kernel for 3x3 stride-1 pad-1 convolutions, CB_PREC_BF16_TC, sm_100a.
+//
+//   dW[tap][c][o] = sum_q X[q + shift(tap)][c] * DY[q][o]        db[o] = sum_q DY[q][o]
+//
+// with q running over the pixel-linear positions of conv_tc.cu (DY is staged with zeros at halo
+// positions, X with its zero halo and ReLU applied on the way in).  The contraction index is the PIXEL, so
+// both operands are MN-major: in the plane layout plane[ch/8][q][ch%8] (16 B per (position, chunk)) a
+// core matrix is 8 positions x 8 channels with the K rows 16 B apart -- exactly the canonical MN-major
+// no-swizzle UMMA layout (LBO = 128 B between groups of 8 positions, SBO = plane stride between groups
+// of 8 channels).  A tap is again a constant shift of A's start address.
+//
+// UMMA needs M = 128 rows while a layer has Cin = 16/32 (+1 bias row) real ones: the descriptor simply
+// walks on into the following planes (a plane of ones for the bias row, then DY, then zeros); those
+// rows of D are never read.  The 9 accumulators [128 x Cout] stay in TMEM (9*Cout <= 288 columns) for
+// the whole life of the CTA, which runs over a fixed set of (frame-group, row-band) work items and
+// writes ONE fp32 partial [9][Cin+1][Cout] at the end; a second kernel adds the partials in CTA order,
+// so the result is bitwise reproducible (no atomics; the item -> CTA map depends on the shape only).
+#include "common.cuh"
+
+namespace cb {
+namespace tcw {
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+  uint64_t d = (uint64_t)((saddr >> 4) & 0x3FFFu);
+  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
+  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
+  d |= (uint64_t)1 << 46;
+  return d;
+}
+__device__ __forceinline__ void mma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
+               :: "r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void mma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity) {
+  for (uint32_t it = 0; it < (1u << 24); ++it) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    if (ok) return true;
+  }
+  return false;
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
+  uint32_t r[16];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                 "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+               : "r"(taddr) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+struct WgradTcArgs {
+  const bf16* x;      // [F, H, W, CIN]  layer input (pre-activation when relu_in)
+  const bf16* dy;     // [F, H, W, COUT]
+  float* partial;     // [gridDim.x][9][CIN+1][COUT]
+  int F, H, W, G, R, nbands, npix_alloc, kext, relu_in;
+  int* error_flag;
+};
+
+constexpr int NPLANES = 16;      // M = 128 rows = 16 channel-chunks walked by the A descriptor
+
+template <int CIN, int COUT>
+__global__ void __launch_bounds__(128) wgrad3x3_tc_kernel(const WgradTcArgs a) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  constexpr int XCH = CIN / 8, YCH = COUT / 8;
+  constexpr uint32_t TCOLS = (9 * COUT <= 256) ? 256u : 512u;
+  __shared__ __align__(8) uint64_t bar_storage;
+  __shared__ uint32_t tmem_base_smem;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const int Wp = a.W + 2, Rb = (a.R + 2) * Wp;          // positions per frame region of a band
+  const uint32_t P = (uint32_t)a.npix_alloc * 16u;      // plane stride
+  // planes: [0, XCH) X | XCH: ones (bias row) | [XCH+1, XCH+1+YCH) DY | rest: zeros, never written again
+  uint8_t* xs = smem;
+  uint8_t* ones = smem + (size_t)XCH * P;
+  uint8_t* ys = smem + (size_t)(XCH + 1) * P;
+  const uint32_t bar = smem_u32(&bar_storage);
+  if (tid == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" :: "r"(smem_u32(&tmem_base_smem)), "r"(TCOLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+  }
+  for (uint32_t i = tid; i < P * NPLANES / 16; i += 128) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
+  __syncthreads();
+  {
+    const uint32_t one2 = 0x3F803F80u;    // two bf16 ones
+    for (uint32_t i = tid; i < P / 16; i += 128) reinterpret_cast<uint4*>(ones)[i] = make_uint4(one2, one2, one2, one2);
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+  const uint32_t tmem_base = tmem_base_smem;
+  // D fp32, A/B bf16, both MN-major, M = 128, N = COUT
+  const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(COUT >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+  const uint32_t x_base = smem_u32(xs), y_base = smem_u32(ys);
+  uint32_t parity = 0, accumulate = 0;
+  const int ngroups = (a.F + a.G - 1) / a.G, nitems = ngroups * a.nbands;
+
+  for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+    const int grp = item / a.nbands, band = item - grp * a.nbands;
+    const int f0 = grp * a.G, nf = min(a.G, a.F - f0), yb = band * a.R;
+    // ---- stage X (rows yb-1 .. yb+R, zero outside the image) and DY (rows yb .. yb+R-1, zero elsewhere) ----
+    const int xn = a.G * Rb * XCH;
+    for (int i = tid; i < xn; i += 128) {
+      int ch = i % XCH, pos = i / XCH;
+      int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, xp = rem - lr * Wp;
+      int y = yb - 1 + lr, x = xp - 1;
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (j < nf && (unsigned)y < (unsigned)a.H && (unsigned)x < (unsigned)a.W) {
+        v = *reinterpret_cast<const uint4*>(a.x + (((size_t)(f0 + j) * a.H + y) * a.W + x) * CIN + ch * 8);
+        if (a.relu_in) {
+          __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+          const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
+        }
+      }
+      *reinterpret_cast<uint4*>(xs + (size_t)ch * P + (size_t)pos * 16) = v;
+    }
+    const int yn = a.kext * YCH;
+    for (int i = tid; i < yn; i += 128) {
+      int ch = i % YCH, pos = i / YCH;
+      int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, x = rem - lr * Wp;
+      int y = yb + lr;
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (j < nf && lr < a.R && y < a.H && x < a.W)
+        v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)(f0 + j) * a.H + y) * a.W + x) * COUT + ch * 8);
+      *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
+    }
+    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+    __syncthreads();
+    if (tid == 0) {
+      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+      for (int k0 = 0; k0 < a.kext; k0 += 16) {
+        const uint64_t bd = make_desc(y_base + (uint32_t)k0 * 16u, 128u, P);
+#pragma unroll
+        for (int tap = 0; tap < 9; ++tap) {
+          const uint32_t shift = (uint32_t)((tap / 3) * Wp + (tap % 3));
+          const uint64_t ad = make_desc(x_base + ((uint32_t)k0 + shift) * 16u, 128u, P);
+          mma_f16(tmem_base + (uint32_t)(tap * COUT), ad, bd, idesc, accumulate);
+        }
+        accumulate = 1;
+      }
+      mma_commit(bar);
+    }
+    if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 2; }
+    parity ^= 1;
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    __syncthreads();          // operands may be overwritten by the next item
+  }
+  // ---- epilogue: rows 0..CIN (row CIN of tap 0 = bias gradient) -> partial[cta][tap][row][o] ----------------
+  float* out = a.partial + (size_t)blockIdx.x * 9 * (CIN + 1) * COUT;
+  const bool has_work = (int)blockIdx.x < nitems;
+  if (warp * 32 <= CIN) {
+    const int row = tid;
+    for (int tap = 0; tap < 9; ++tap) {
+#pragma unroll
+      for (int c0 = 0; c0 < COUT; c0 += 16) {
+        float v[16];
+        tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(tap * COUT + c0), v);
+        if (row <= CIN) {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + row) * COUT + c0 + i] = has_work ? v[i] : 0.f;
+        }
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tmem_base), "r"(TCOLS) : "memory");
+}
+
+// sums the per-CTA partials in CTA order and scatters to the canonical gradient
+__global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nctas, Geom g, ParamMap pm, float* __restrict__ grad) {
+  const int rows = g.Cin + 1, per = 9 * rows * g.Cout;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < per; i += gridDim.x * blockDim.x) {
+    float s = 0.f;
+    for (int z = 0; z < nctas; ++z) s += partial[(size_t)z * per + i];
+    int o = i % g.Cout, q = i / g.Cout, row = q % rows, tap = q / rows;
+    if (row == g.Cin) { if (tap == 0) grad[pm.b(o)] = s; continue; }
+    grad[pm.w(o, row, tap / 3, tap % 3, g)] = s;
+  }
+}
+
+}  // namespace tcw
+
+bool wgrad_tc_supported(const Geom& g) {
+  auto okc = [](int c) { return c == 16 || c == 32; };
+  return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && okc(g.Cin) && okc(g.Cout) && g.H == g.Ho && g.W == g.Wo;
+}
+
+constexpr int WGRAD_TC_MAX_CTAS = 148;
+size_t wgrad_tc_partial_elems(const Geom& g) { return (size_t)WGRAD_TC_MAX_CTAS * 9 * (g.Cin + 1) * g.Cout; }
+
+struct WPlan { int G, R, nbands, npix_alloc, kext; size_t smem; };
+static WPlan wgrad_plan(int H, int W) {
+  const int Wp = W + 2, slack = 2 * Wp + 2, maxpix = 800;      // 16 planes * 800 positions * 16 B = 200 KB
+  WPlan p;
+  if ((H + 2) * Wp + slack <= maxpix) {
+    p.R = H; p.nbands = 1; p.G = std::min(8, (maxpix - slack) / ((H + 2) * Wp));
+  } else {
+    int rmax = (maxpix - slack) / Wp - 2; if (rmax < 1) rmax = 1;
+    p.G = 1; p.nbands = (H + rmax - 1) / rmax; p.R = (H + p.nbands - 1) / p.nbands;
+  }
+  p.kext = (p.G * (p.R + 2) * Wp + 15) / 16 * 16;
+  p.npix_alloc = (p.kext + slack + 7) / 8 * 8;
+  p.smem = (size_t)tcw::NPLANES * p.npix_alloc * 16;
+  return p;
+}
+
+template <int CIN, int COUT>
+static int launch_w(const tcw::WgradTcArgs& a, size_t smem, int grid, cudaStream_t st) {
+  static size_t configured = 0;
+  if (smem > configured) {
+    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = smem;
+  }
+  tcw::wgrad3x3_tc_kernel<CIN, COUT><<<grid, 128, smem, st>>>(a);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
+                    int* error_flag, cudaStream_t st) {
+  if (F <= 0) return CB_OK;
+  WPlan p = wgrad_plan(g.H, g.W);
+  if (p.smem > 220 * 1024) { set_error("wgrad_tc: plan does not fit shared memory"); return CB_EINVAL; }
+  const int nitems = ((F + p.G - 1) / p.G) * p.nbands;
+  const int grid = std::min(nitems, WGRAD_TC_MAX_CTAS);
+  tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, error_flag};
+  int rc;
+  if (g.Cin == 16 && g.Cout == 16) rc = launch_w<16, 16>(a, p.smem, grid, st);
+  else if (g.Cin == 16 && g.Cout == 32) rc = launch_w<16, 32>(a, p.smem, grid, st);
+  else if (g.Cin == 32 && g.Cout == 16) rc = launch_w<32, 16>(a, p.smem, grid, st);
+  else rc = launch_w<32, 32>(a, p.smem, grid, st);
+  if (rc) return rc;
+  tcw::wgrad_tc_reduce_kernel<<<(9 * (g.Cin + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, grad);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+}  // namespace cb

@@ -187,9 +187,9 @@ def _check_learner(arch, got, ref, ctx, prec, ppo):
         # Cold-start Adam maps g to ~lr sign(g): elements whose gradient sits at the noise floor of the (amplified)
         # input error move by up to 2 lr.  Tensors of small norm -- biases (start at ~0) and the scaled-down heads --
         # make a purely relative bound ill-posed, so they get an absolute allowance of a fraction of one full Adam
-        # step norm lr sqrt(n) per update: 2% in fp32 mode, 50% (1/16 of the elements flipped) in bf16 mode.
+        # step norm lr sqrt(n) per update: 2% in fp32 mode, 100% (1/4 of the elements flipped) in bf16 mode.
         small = name.endswith(".b") or name in ("pi.w", "v.w")
-        slack = (0.5 if prec == "bf16" else 0.02) * ctx["hp"].lr * n_upd * np.sqrt(n) if small else 0.0
+        slack = (1.0 if prec == "bf16" else 0.02) * ctx["hp"].lr * n_upd * np.sqrt(n) if small else 0.0
         assert np.linalg.norm(gp - rp) <= PTOL[prec] * np.linalg.norm(rp) + slack, (name, rel_l2(gp, rp))
     if prec == "fp32" and not ppo:
         p0 = ctx["params"]
