@@ -156,7 +156,7 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
   size_t es = prec == CB_PREC_FP32_REF ? 4 : 2;
   if (!ws.wf) {
     CB_ALLOC(ws.wf, net->wf_total * es); CB_ALLOC(ws.wd, net->wd_total * es); CB_ALLOC(ws.bias, net->bias_total * 4);
-    if (prec == CB_PREC_BF16_TC) { CB_ALLOC(ws.wtc_f, net->wf_total * 2); CB_ALLOC(ws.wtc_d, net->wf_total * 2); }
+    if (prec == CB_PREC_BF16_TC) { CB_ALLOC(ws.w0img, conv0_wimg_elems(net->layers[0].g) * 2); CB_ALLOC(ws.wtc_f, net->wf_total * 2); CB_ALLOC(ws.wtc_d, net->wf_total * 2); }
     CB_ALLOC(ws.errflag, 16); CB_CUDA(cudaMemset(ws.errflag, 0, 16));
     CB_ALLOC(ws.gradbuf, net->P * 4); CB_ALLOC(ws.adam_scratch, clip_adam_scratch_bytes(net->P)); CB_ALLOC(ws.gnorm, 16);
   }
@@ -172,6 +172,7 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
   for (const Layer& L : net->layers) {
     pe = std::max(pe, wgrad_partial_elems(L.g, frames));
     if (wgrad_tc_supported(L.g)) pe = std::max(pe, wgrad_tc_partial_elems(L.g));
+    if (L.u8_in && conv0_tc_supported(L.g)) pe = std::max(pe, conv0_partial_elems(L.g));
   }
   CB_ALLOC(ws.partial, pe * 4); ws.partial_elems = pe;
   ws.frames = frames;
@@ -234,7 +235,7 @@ void cb_net_destroy(cb_net* net) {
     Workspace& ws = net->ws[p];
     if (!ws.wf) continue;
     free_workspace(ws); free_scratch(ws);
-    cudaFree(ws.wtc_f); cudaFree(ws.wtc_d); cudaFree(ws.errflag);
+    cudaFree(ws.w0img); cudaFree(ws.wtc_f); cudaFree(ws.wtc_d); cudaFree(ws.errflag);
     cudaFree(ws.wf); cudaFree(ws.wd); cudaFree(ws.bias); cudaFree(ws.gradbuf); cudaFree(ws.adam_scratch); cudaFree(ws.gnorm);
   }
   delete net;

@@ -70,6 +70,7 @@ struct Workspace {     // one per precision mode
   std::vector<void*> act;            // per tensor, [frames * per_frame]
   void* grad[G_COUNT] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   void* wf = nullptr; void* wd = nullptr; float* bias = nullptr;   // packed weights (mode type), fp32 bias
+  bf16* w0img = nullptr;                                           // first-layer forward B image (conv0_tc.cu)
   bf16* wtc_f = nullptr; bf16* wtc_d = nullptr;                     // tcgen05 B-operand packs (forward / dgrad), bf16 mode only
   int* errflag = nullptr;                                          // set by a kernel whose tcgen05 pipeline timed out
   float* partial = nullptr; size_t partial_elems = 0;             // wgrad split-K partials
@@ -136,6 +137,16 @@ bool wgrad_tc_supported(const Geom& g);
 size_t wgrad_tc_partial_elems(const Geom& g);
 int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
                     int* error_flag, cudaStream_t st);
+
+// conv0_tc.cu
+bool conv0_tc_supported(const Geom& g);
+size_t conv0_partial_elems(const Geom& g);
+size_t conv0_wimg_elems(const Geom& g);
+int launch_conv0_pack(const Geom& g, const ParamMap& pm, const float* params, bf16* wimg, cudaStream_t st);
+int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* wimg, const float* bias, bf16* out,
+                     int* error_flag, cudaStream_t st);
+int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, float* partial,
+                       float* grad, int* error_flag, cudaStream_t st);
 
 // rl.cu
 int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset,

@@ -1,0 +1,276 @@
+// tcgen05 kernels for the FIRST layer of the IMPALA-ResNet in CB_PREC_BF16_TC: 3x3 stride-1 pad-1 conv on
+// uint8 NCHW frames with Cin <= 4, forward and weight gradient.  The /255
+// normalisation is fused: the raw integers 0..255 (exact in bf16) are the operand and 1/255 scales the
+// fp32 accumulator.
+//
+// Staging: one plane of 16-byte positions [c0 c1 c2 c3 | 1 | 0 0 0] in the pixel-linear order of
+// conv_tc.cu (row-band of R rows with its halo).  Channel 4 is the constant 1: its forward weights are
+// zero; in the weight gradient it makes row 4 of the accumulator the bias gradient.
+//   forward: a K=16 MMA step = two neighbouring positions (taps (di,0),(di,1); then (di,2) + a zero-weight
+//            slot): K-major A descriptor with LBO = 16 B, six MMAs per 128-position tile.
+//   wgrad:   MN-major A descriptor with SBO = 16 B: the M walk steps over neighbouring positions, so one
+//            M = 128 MMA yields the taps (di, 0..2) at rows 8*dj + c; three accumulators [128 x Cout] (one
+//            per di) live in TMEM for the life of the CTA; per-CTA partials are summed in CTA order.
+#include "common.cuh"
+#include "tc_ptx.cuh"
+
+namespace cb {
+namespace tc0 {
+using namespace ptx;
+
+struct Args {
+  const uint8_t* obs; const int32_t* frame_idx;   // [*, CIN, H, W] uint8, optional frame gather
+  const bf16* w; const float* bias; bf16* out;     // forward: B image [6][2][COUT][8], bias [COUT], out [F,H,W,COUT]
+  const bf16* dy; float* partial;                 // wgrad: dy [F,H,W,COUT], partial [grid][3][24][COUT]
+  int F, H, W, CIN, R, nbands, npix_alloc, kext;
+  int* error_flag;
+};
+
+// stage rows yb-1 .. yb+R of frame `fr` into the plane (all positions rewritten)
+__device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr, int yb, int tid) {
+  const int Wp = a.W + 2, W4 = a.W / 4, rows = a.R + 2;
+  const uint32_t ONE = 0x3F80u;
+  for (int i = tid; i < rows * W4; i += 128) {
+    int lr = i / W4, x0 = (i - lr * W4) * 4, y = yb - 1 + lr;
+    uint32_t px[4] = {0, 0, 0, 0};     // per channel: 4 pixels
+    if ((unsigned)y < (unsigned)a.H)
+      for (int c = 0; c < a.CIN; ++c) px[c] = *reinterpret_cast<const uint32_t*>(a.obs + ((fr * a.CIN + c) * a.H + y) * a.W + x0);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      float v0 = (float)((px[0] >> (8 * k)) & 255u), v1 = (float)((px[1] >> (8 * k)) & 255u);
+      float v2 = (float)((px[2] >> (8 * k)) & 255u), v3 = (float)((px[3] >> (8 * k)) & 255u);
+      __nv_bfloat162 p01 = __floats2bfloat162_rn(v0, v1), p23 = __floats2bfloat162_rn(v2, v3);
+      uint4 o; o.x = *reinterpret_cast<uint32_t*>(&p01); o.y = *reinterpret_cast<uint32_t*>(&p23); o.z = ONE; o.w = 0;
+      *reinterpret_cast<uint4*>(xs + (size_t)(lr * Wp + x0 + 1 + k) * 16) = o;
+    }
+  }
+  for (int i = tid; i < rows * 2; i += 128) {       // halo columns
+    int lr = i >> 1, xp = (i & 1) ? Wp - 1 : 0;
+    *reinterpret_cast<uint4*>(xs + (size_t)(lr * Wp + xp) * 16) = make_uint4(0, 0, ONE, 0);
+  }
+}
+
+constexpr int TMEM_COLS = 256;
+
+template <int COUT>
+__global__ void __launch_bounds__(128) conv0_fwd_kernel(const Args a) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  constexpr uint32_t W_BYTES = 6u * 2u * COUT * 16u;
+  constexpr int TILES_PER_BATCH = TMEM_COLS / COUT;
+  __shared__ __align__(8) uint64_t bar_storage;
+  __shared__ uint32_t tmem_base_smem;
+  const int tid = threadIdx.x, warp = tid >> 5, Wp = a.W + 2;
+  uint8_t* w_smem = smem; uint8_t* xs = smem + W_BYTES;
+  const uint32_t bar = smem_u32(&bar_storage);
+  if (tid == 0) mbar_init(bar, 1);
+  if (warp == 0) tmem_alloc(smem_u32(&tmem_base_smem), TMEM_COLS);
+  for (uint32_t i = tid; i < W_BYTES / 16; i += 128) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w)[i];
+  for (int i = tid; i < a.npix_alloc; i += 128) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
+  tc_fence_before(); __syncthreads(); tc_fence_after();
+  const uint32_t tmem_base = tmem_base_smem, idesc = make_idesc(128, COUT, 0, 0);
+  const uint32_t a_base = smem_u32(xs), b_base = smem_u32(w_smem);
+  uint32_t parity = 0;
+  const int nitems = a.F * a.nbands;
+  for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+    const int f = item / a.nbands, yb = (item - f * a.nbands) * a.R;
+    const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
+    stage_band(a, xs, fr, yb, tid);
+    fence_async_smem();
+    __syncthreads();
+    const int ntiles = (a.R * Wp + 127) / 128;
+    for (int t0 = 0; t0 < ntiles; t0 += TILES_PER_BATCH) {
+      const int nt = min(TILES_PER_BATCH, ntiles - t0);
+      if (tid == 0) {
+        tc_fence_after();
+        for (int s = 0; s < nt; ++s) {
+          const uint32_t q0 = (uint32_t)(t0 + s) * 128u;
+#pragma unroll
+          for (int slot = 0; slot < 6; ++slot) {
+            const uint32_t shift = (uint32_t)((slot >> 1) * Wp + (slot & 1) * 2);
+            uint64_t ad = make_desc(a_base + (q0 + shift) * 16u, 16u, 128u);
+            uint64_t bd = make_desc(b_base + (uint32_t)slot * 2u * COUT * 16u, (uint32_t)COUT * 16u, 128u);
+            mma_f16(tmem_base + (uint32_t)(s * COUT), ad, bd, idesc, slot ? 1u : 0u);
+          }
+        }
+        mma_commit(bar);
+      }
+      if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 3; }
+      parity ^= 1;
+      tc_fence_after();
+      for (int s = 0; s < nt; ++s) {
+        const int q = (t0 + s) * 128 + tid, yl = q / Wp, x = q - yl * Wp, y = yb + yl;
+        const bool valid = yl < a.R && y < a.H && x < a.W;
+        const size_t o = (((size_t)f * a.H + y) * a.W + x) * COUT;
+#pragma unroll
+        for (int c0 = 0; c0 < COUT; c0 += 16) {
+          float v[16];
+          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(s * COUT + c0), v);
+          if (!valid) continue;
+          uint4 o0, o1;
+          __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
+#pragma unroll
+          for (int i = 0; i < 16; ++i) v[i] = fmaf(v[i], 1.0f / 255.0f, a.bias[c0 + i]);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
+          *reinterpret_cast<uint4*>(a.out + o + c0) = o0;
+          *reinterpret_cast<uint4*>(a.out + o + c0 + 8) = o1;
+        }
+      }
+      tc_fence_before();
+      __syncthreads();
+    }
+  }
+  tc_fence_before(); __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem_base, TMEM_COLS);
+}
+
+template <int COUT>
+__global__ void __launch_bounds__(128) conv0_wgrad_kernel(const Args a) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  constexpr int YCH = COUT / 8;
+  constexpr uint32_t TCOLS = 128;
+  __shared__ __align__(8) uint64_t bar_storage;
+  __shared__ uint32_t tmem_base_smem;
+  const int tid = threadIdx.x, warp = tid >> 5, Wp = a.W + 2;
+  const uint32_t P = (uint32_t)a.npix_alloc * 16u;
+  uint8_t* xs = smem; uint8_t* ys = smem + P;
+  const uint32_t bar = smem_u32(&bar_storage);
+  if (tid == 0) mbar_init(bar, 1);
+  if (warp == 0) tmem_alloc(smem_u32(&tmem_base_smem), TCOLS);
+  for (int i = tid; i < a.npix_alloc; i += 128) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
+  for (uint32_t i = tid; i < P * YCH / 16; i += 128) reinterpret_cast<uint4*>(ys)[i] = make_uint4(0, 0, 0, 0);
+  tc_fence_before(); __syncthreads(); tc_fence_after();
+  const uint32_t tmem_base = tmem_base_smem, idesc = make_idesc(128, COUT, 1, 1);
+  const uint32_t x_base = smem_u32(xs), y_base = smem_u32(ys);
+  uint32_t parity = 0, accumulate = 0;
+  const int nitems = a.F * a.nbands;
+  for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
+    const int f = item / a.nbands, yb = (item - f * a.nbands) * a.R;
+    const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
+    stage_band(a, xs, fr, yb, tid);
+    for (int i = tid; i < a.kext * YCH; i += 128) {
+      int ch = i % YCH, pos = i / YCH, yl = pos / Wp, x = pos - yl * Wp, y = yb + yl;
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (yl < a.R && y < a.H && x < a.W) v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)f * a.H + y) * a.W + x) * COUT + ch * 8);
+      *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
+    }
+    fence_async_smem();
+    __syncthreads();
+    if (tid == 0) {
+      tc_fence_after();
+      for (int k0 = 0; k0 < a.kext; k0 += 16) {
+        const uint64_t bd = make_desc(y_base + (uint32_t)k0 * 16u, 128u, P);
+#pragma unroll
+        for (int di = 0; di < 3; ++di) {
+          const uint64_t ad = make_desc(x_base + (uint32_t)(k0 + di * Wp) * 16u, 128u, 16u);
+          mma_f16(tmem_base + (uint32_t)(di * COUT), ad, bd, idesc, accumulate);
+        }
+        accumulate = 1;
+      }
+      mma_commit(bar);
+    }
+    if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 4; }
+    parity ^= 1;
+    tc_fence_after();
+    __syncthreads();
+  }
+  float* out = a.partial + (size_t)blockIdx.x * 3 * 24 * COUT;
+  if (warp == 0) {
+    for (int di = 0; di < 3; ++di) {
+#pragma unroll
+      for (int c0 = 0; c0 < COUT; c0 += 16) {
+        float v[16];
+        tmem_ld16(tmem_base + (uint32_t)(di * COUT + c0), v);
+        if (tid < 24) {
+#pragma unroll
+          for (int i = 0; i < 16; ++i) out[((size_t)di * 24 + tid) * COUT + c0 + i] = v[i];
+        }
+      }
+    }
+  }
+  tc_fence_before(); __syncthreads();
+  if (warp == 0) tmem_dealloc(tmem_base, TCOLS);
+}
+
+// forward B image: slot = 2*di + h; h = 0: chunks (di,0),(di,1); h = 1: chunks (di,2), zero.  [slot][chunk][o][8]
+__global__ void conv0_pack_kernel(const float* __restrict__ params, Geom g, ParamMap pm, bf16* __restrict__ wimg) {
+  int total = 6 * 2 * g.Cout * 8;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+    int c = i & 7, o = (i >> 3) % g.Cout, chunk = ((i >> 3) / g.Cout) & 1, slot = (i >> 3) / g.Cout / 2;
+    int di = slot >> 1, dj = (slot & 1) * 2 + chunk;
+    float v = (c < g.Cin && dj < 3) ? params[pm.w(o, c, di, dj, g)] : 0.f;
+    wimg[i] = __float2bfloat16_rn(v);
+  }
+}
+
+__global__ void conv0_wgrad_reduce_kernel(const float* __restrict__ partial, int nctas, Geom g, ParamMap pm, float* __restrict__ grad) {
+  const int per = 3 * 24 * g.Cout;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < per; i += gridDim.x * blockDim.x) {
+    float s = 0.f;
+    for (int z = 0; z < nctas; ++z) s += partial[(size_t)z * per + i];
+    int o = i % g.Cout, row = (i / g.Cout) % 24, di = i / g.Cout / 24, dj = row >> 3, c = row & 7;
+    if (c < g.Cin) grad[pm.w(o, c, di, dj, g)] = s * (1.0f / 255.0f);
+    else if (c == 4 && dj == 0 && di == 0) grad[pm.b(o)] = s;
+  }
+}
+
+}  // namespace tc0
+
+bool conv0_tc_supported(const Geom& g) {
+  return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && g.Cin <= 4 && (g.Cout == 16 || g.Cout == 32) && g.W % 4 == 0 && g.W >= 8 && g.H == g.Ho && g.W == g.Wo;
+}
+constexpr int CONV0_MAX_CTAS = 296;
+size_t conv0_partial_elems(const Geom& g) { return (size_t)CONV0_MAX_CTAS * 3 * 24 * g.Cout; }
+size_t conv0_wimg_elems(const Geom& g) { return (size_t)6 * 2 * g.Cout * 8; }
+
+int launch_conv0_pack(const Geom& g, const ParamMap& pm, const float* params, bf16* wimg, cudaStream_t st) {
+  tc0::conv0_pack_kernel<<<(6 * 2 * g.Cout * 8 + 255) / 256, 256, 0, st>>>(params, g, pm, wimg);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+template <class K>
+static int set_smem(K kernel, size_t smem, size_t* configured) {
+  if (smem > *configured) { CB_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); *configured = smem; }
+  return CB_OK;
+}
+
+int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* wimg, const float* bias, bf16* out,
+                     int* error_flag, cudaStream_t st) {
+  if (F <= 0) return CB_OK;
+  const int Wp = g.W + 2;
+  int R = std::min(g.H, (90 * 1024 / 16 - 2 * Wp - 130) / Wp - 2); if (R < 1) R = 1;
+  const int nb = (g.H + R - 1) / R; R = (g.H + nb - 1) / nb;
+  const int npix = ((R * Wp + 127) / 128) * 128 + 2 * Wp + 8;
+  const size_t smem = (size_t)6 * 2 * g.Cout * 16 + (size_t)npix * 16;
+  tc0::Args a{obs, frame_idx, wimg, bias, out, nullptr, nullptr, F, g.H, g.W, g.Cin, R, nb, npix, 0, error_flag};
+  const int grid = std::min(F * nb, 296);
+  static size_t c16 = 0, c32 = 0; int rc;
+  if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_fwd_kernel<16>, smem, &c16))) return rc; tc0::conv0_fwd_kernel<16><<<grid, 128, smem, st>>>(a); }
+  else { if ((rc = set_smem(tc0::conv0_fwd_kernel<32>, smem, &c32))) return rc; tc0::conv0_fwd_kernel<32><<<grid, 128, smem, st>>>(a); }
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, float* partial,
+                       float* grad, int* error_flag, cudaStream_t st) {
+  if (F <= 0) return CB_OK;
+  const int Wp = g.W + 2, ych = g.Cout / 8;
+  const int maxpos = (int)(96 * 1024 / 16 / (1 + ych));
+  int R = std::min(g.H, (maxpos - 2 * Wp - 48) / Wp); if (R < 1) R = 1;
+  const int nb = (g.H + R - 1) / R; R = (g.H + nb - 1) / nb;
+  const int kext = (R * Wp + 15) / 16 * 16;
+  const int npix = (kext + 2 * Wp + 40 + 7) / 8 * 8;
+  const size_t smem = (size_t)(1 + ych) * npix * 16;
+  const int grid = std::min(F * nb, CONV0_MAX_CTAS);
+  tc0::Args a{obs, frame_idx, nullptr, nullptr, nullptr, dy, partial, F, g.H, g.W, g.Cin, R, nb, npix, kext, error_flag};
+  static size_t c16 = 0, c32 = 0; int rc;
+  if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_wgrad_kernel<16>, smem, &c16))) return rc; tc0::conv0_wgrad_kernel<16><<<grid, 128, smem, st>>>(a); }
+  else { if ((rc = set_smem(tc0::conv0_wgrad_kernel<32>, smem, &c32))) return rc; tc0::conv0_wgrad_kernel<32><<<grid, 128, smem, st>>>(a); }
+  CB_CUDA(cudaGetLastError());
+  tc0::conv0_wgrad_reduce_kernel<<<(3 * 24 * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, grad);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+}  // namespace cb

@@ -42,6 +42,7 @@ static int pack_all(cb_net* net, Workspace& ws, const float* params, cudaStream_
     size_t total = (size_t)L.g.kh * L.g.kw * L.g.Cin * L.g.Cout;
     int blocks = (int)std::min<size_t>((total + 255) / 256, 1184);
     pack_kernel<AT><<<blocks, 256, 0, st>>>(params, L.g, L.pm, (AT*)ws.wf + L.wf_off, (AT*)ws.wd + L.wd_off, ws.bias + L.bias_off);
+    if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(L.g)) { int rc = launch_conv0_pack(L.g, L.pm, params, ws.w0img, st); if (rc) return rc; }
     if (std::is_same<AT, bf16>::value && conv_tc_supported(L.g))
       pack_tc_kernel<<<blocks, 256, 0, st>>>(params, L.g, L.pm, ws.wtc_f + L.wf_off, ws.wtc_d + L.wf_off);
   }
@@ -228,6 +229,8 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out) {
       rc = launch_conv_tc(0, F, g.H, g.W, g.Cin, g.Cout, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (const bf16*)skip, nullptr,
                           (bf16*)ws.act[L.out_t], L.relu_in, ws.errflag, st);
+    } else if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(g)) {
+      rc = launch_conv0_fwd(g, F, obs, frame_idx, ws.w0img, bias, (bf16*)ws.act[L.out_t], ws.errflag, st);
     } else if (L.u8_in) {
       FwdProblem<AT, AT, true> p{M, N, K, K, {g, obs, frame_idx, false}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f / 255.0f};
       rc = launch_gemm(p, 1, st);
@@ -268,6 +271,12 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         ProfScope ps(K_CONV_WGRAD, st, 2, 2.0 * 9 * g.Cin * g.Cout * (double)F * g.Ho * g.Wo,
                      2.0 * F * g.H * g.W * (g.Cin + g.Cout) + 4.0 * 9 * (g.Cin + 1) * g.Cout);
         int rc = launch_wgrad_tc(g, L.pm, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.grad[op.dy], L.relu_in, ws.partial, grad, ws.errflag, st);
+        if (rc) return rc;
+        continue;
+      }
+      if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(g)) {
+        ProfScope ps(K_CONV_WGRAD, st, 2, 2.0 * 9 * g.Cin * g.Cout * (double)F * g.Ho * g.Wo, (double)F * g.H * g.W * (g.Cin + 2.0 * g.Cout));
+        int rc = launch_conv0_wgrad(g, L.pm, F, obs, frame_idx, (const bf16*)ws.grad[op.dy], ws.partial, grad, ws.errflag, st);
         if (rc) return rc;
         continue;
       }

