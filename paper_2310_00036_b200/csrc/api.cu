@@ -21,7 +21,7 @@ static inline int conv_out_h(int h, int k, int s, int p) { return (h + 2 * p - k
 
 struct Builder {
   cb_net* net; size_t off = 0; int cur = -1; int H, W, C;
-  int tensor(size_t per_frame, bool f32 = false) { net->tensors.push_back({per_frame, f32}); return (int)net->tensors.size() - 1; }
+  int tensor(size_t per_frame, bool f32 = false, int esize = 0) { net->tensors.push_back({per_frame, f32, esize}); return (int)net->tensors.size() - 1; }
   void need(int buf, size_t elems) { if (buf >= 0) net->grad_elems[buf] = std::max(net->grad_elems[buf], elems); }
   void ptensor(const std::string& name, size_t o, std::vector<int> dims, int fan) {
     cb_net::PT t; t.name = name; t.off = o; t.rank = (int)dims.size(); t.fan_in = fan;
@@ -60,7 +60,7 @@ static int build_program(cb_net* net) {
   for (int i = 0; i < G_COUNT; ++i) net->grad_elems[i] = 0;
   net->wf_total = net->bias_total = 0;
   std::vector<int> convs;       // layer ids in forward order
-  struct Stage { int conv, c_t, C, H, W, l[4]; }; std::vector<Stage> stages;
+  struct Stage { int conv, c_t, idx_t, C, H, W, l[4]; }; std::vector<Stage> stages;
   if (a.kind == CB_ARCH_NATURE) {
     convs.push_back(b.conv("conv1", -1, a.channels[0], 8, 8, 4, 0, false, -1));
     convs.push_back(b.conv("conv2", net->layers[convs[0]].out_t, a.channels[1], 4, 4, 2, 0, true, -1));
@@ -72,7 +72,8 @@ static int build_program(cb_net* net) {
       Stage st; st.conv = b.conv(nm, b.cur, a.channels[s], 3, 3, 1, 1, false, -1);
       st.c_t = net->layers[st.conv].out_t; st.C = b.C; st.H = b.H; st.W = b.W;
       int p = b.tensor((size_t)pool_out_h(b.H) * pool_out_h(b.W) * b.C);
-      net->fwd.push_back({OP_POOL, -1, st.c_t, p, b.C, b.H, b.W, -1, -1, -1, -1});
+      st.idx_t = b.tensor((size_t)pool_out_h(b.H) * pool_out_h(b.W) * b.C, false, 1);   // window position of the first maximum (A11)
+      net->fwd.push_back({OP_POOL, -1, st.c_t, p, b.C, b.H, b.W, -1, -1, st.idx_t, -1});
       b.H = pool_out_h(b.H); b.W = pool_out_h(b.W);
       for (int k = 0; k < 2; ++k) {
         snprintf(nm, sizeof nm, "stage%d.block%d.conv1", s, k);
@@ -127,7 +128,7 @@ static int build_program(cb_net* net) {
         b.wgrad(l2, G_A); b.dgrad(l2, G_A, G_B, -1);         // d(relu(h)) masked by h > 0
         b.wgrad(l1, G_B); b.dgrad(l1, G_B, G_A, G_A);        // block path + identity path (in place)
       }
-      net->bwd.push_back({OP_POOLBWD, -1, st.c_t, -1, st.C, st.H, st.W, G_A, G_C, -1, -1});
+      net->bwd.push_back({OP_POOLBWD, -1, st.c_t, -1, st.C, st.H, st.W, G_A, G_C, st.idx_t, -1});
       b.need(G_C, (size_t)st.C * st.H * st.W);
       b.wgrad(st.conv, G_C);
       if (s > 0) b.dgrad(st.conv, G_C, G_A, -1);
@@ -166,7 +167,7 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
   free_workspace(ws);
   ws.act.assign(net->tensors.size(), nullptr);
   for (size_t i = 0; i < net->tensors.size(); ++i)
-    CB_ALLOC(ws.act[i], net->tensors[i].per_frame * frames * (net->tensors[i].f32 ? 4 : es));
+    CB_ALLOC(ws.act[i], net->tensors[i].per_frame * frames * (net->tensors[i].esize ? (size_t)net->tensors[i].esize : (net->tensors[i].f32 ? 4 : es)));
   for (int i = 0; i < G_COUNT; ++i) CB_ALLOC(ws.grad[i], net->grad_elems[i] * frames * es);
   size_t pe = 0;
   for (const Layer& L : net->layers) {

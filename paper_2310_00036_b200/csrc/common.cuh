@@ -59,11 +59,11 @@ struct Op {
   int in_t, out_t;  // POOL fwd: tensors;  POOLBWD: in_t = conv-output tensor (pool input)
   int C, H, W;      // POOL geometry (input map)
   int dy, dx;       // backward: gradient buffers (GradBuf)
-  int mask_t;       // DGRAD: tensor whose sign gates the result (-1 none)
+  int mask_t;       // DGRAD: tensor whose sign gates the result (-1 none); POOL / POOLBWD: uint8 arg-max tensor
   int add;          // DGRAD: gradient buffer added after masking (-1 none)
 };
 
-struct Tensor { size_t per_frame; bool f32; };
+struct Tensor { size_t per_frame; bool f32; int esize; };   // esize: bytes per element, 0 = the mode's storage type
 
 struct Workspace {     // one per precision mode
   int frames = 0;

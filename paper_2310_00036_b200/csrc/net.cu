@@ -120,27 +120,29 @@ __device__ __forceinline__ uint4 f_to_bf8(const float* f) {
   for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(f[2 * i], f[2 * i + 1]);
   return u;
 }
-__global__ void pool_fwd_v8_kernel(const bf16* __restrict__ x, bf16* __restrict__ y, int F, int C, int H, int W) {
+__global__ void pool_fwd_v8_kernel(const bf16* __restrict__ x, bf16* __restrict__ y, uint8_t* __restrict__ arg, int F, int C, int H, int W) {
   int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W), C8 = C / 8;
   size_t total = (size_t)F * Ho * Wo * C8;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
     int c8 = (int)(i % C8); size_t q = i / C8; int ox = (int)(q % Wo); q /= Wo; int oy = (int)(q % Ho); size_t f = q / Ho;
-    float best[8];
+    float best[8]; uint32_t bk[8];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) best[k] = -INFINITY;
+    for (int k = 0; k < 8; ++k) { best[k] = -INFINITY; bk[k] = 15; }
     for (int di = 0; di < 3; ++di) {
       int iy = oy * 2 + di - ph; if ((unsigned)iy >= (unsigned)H) continue;
       for (int dj = 0; dj < 3; ++dj) {
         int ix = ox * 2 + dj - pw; if ((unsigned)ix >= (unsigned)W) continue;
         float v[8]; bf8_to_f(*reinterpret_cast<const uint4*>(x + ((f * H + iy) * W + ix) * C + c8 * 8), v);
 #pragma unroll
-        for (int k = 0; k < 8; ++k) if (v[k] > best[k]) best[k] = v[k];
+        for (int k = 0; k < 8; ++k) if (v[k] > best[k]) { best[k] = v[k]; bk[k] = (uint32_t)(di * 3 + dj); }   // strict >: first maximum
       }
     }
     *reinterpret_cast<uint4*>(y + i * 8) = f_to_bf8(best);
+    uint2 pk; pk.x = bk[0] | (bk[1] << 8) | (bk[2] << 16) | (bk[3] << 24); pk.y = bk[4] | (bk[5] << 8) | (bk[6] << 16) | (bk[7] << 24);
+    *reinterpret_cast<uint2*>(arg + i * 8) = pk;
   }
 }
-__global__ void pool_bwd_v8_kernel(const bf16* __restrict__ x, const bf16* __restrict__ dy, bf16* __restrict__ dx, int F, int C, int H, int W) {
+__global__ void pool_bwd_v8_kernel(const uint8_t* __restrict__ arg, const bf16* __restrict__ dy, bf16* __restrict__ dx, int F, int C, int H, int W) {
   int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W), C8 = C / 8;
   size_t total = (size_t)F * H * W * C8;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
@@ -153,23 +155,12 @@ __global__ void pool_bwd_v8_kernel(const bf16* __restrict__ x, const bf16* __res
     int oy_hi = min((iy + ph) / 2, Ho - 1), ox_hi = min((ix + pw) / 2, Wo - 1);
     for (int oy = oy_lo; oy <= oy_hi; ++oy)
       for (int ox = ox_lo; ox <= ox_hi; ++ox) {
-        float best[8]; int bidx[8];
+        const uint32_t me = (uint32_t)((iy - (oy * 2 - ph)) * 3 + (ix - (ox * 2 - pw)));   // my position inside this window
+        const size_t o = ((f * Ho + oy) * Wo + ox) * C + c8 * 8;
+        const uint2 pk = *reinterpret_cast<const uint2*>(arg + o);
+        float d[8]; bf8_to_f(*reinterpret_cast<const uint4*>(dy + o), d);
 #pragma unroll
-        for (int k = 0; k < 8; ++k) { best[k] = -INFINITY; bidx[k] = -1; }
-        for (int di = 0; di < 3; ++di) {
-          int yy = oy * 2 + di - ph; if ((unsigned)yy >= (unsigned)H) continue;
-          for (int dj = 0; dj < 3; ++dj) {
-            int xx = ox * 2 + dj - pw; if ((unsigned)xx >= (unsigned)W) continue;
-            float v[8]; bf8_to_f(*reinterpret_cast<const uint4*>(x + ((f * H + yy) * W + xx) * C + c8 * 8), v);
-            int id = yy * W + xx;
-#pragma unroll
-            for (int k = 0; k < 8; ++k) if (v[k] > best[k]) { best[k] = v[k]; bidx[k] = id; }
-          }
-        }
-        float d[8]; bf8_to_f(*reinterpret_cast<const uint4*>(dy + ((f * Ho + oy) * Wo + ox) * C + c8 * 8), d);
-        int me = iy * W + ix;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) if (bidx[k] == me) g[k] += d[k];
+        for (int k = 0; k < 4; ++k) { if (((pk.x >> (8 * k)) & 255u) == me) g[k] += d[k]; if (((pk.y >> (8 * k)) & 255u) == me) g[4 + k] += d[4 + k]; }
       }
     *reinterpret_cast<uint4*>(dx + i * 8) = f_to_bf8(g);
   }
@@ -191,15 +182,15 @@ __global__ void wgrad_reduce_kernel(const float* __restrict__ partial, int split
 
 // split-K policy: a function of the problem shape only (never of the device), so the summation
 // order -- and with it every bit of the gradient -- is fixed (A16).
-static inline void wgrad_split(long long K, int* splits, int* kchunk) {
-  const int target = 4096;
+static inline void wgrad_split(long long K, int* splits, int* kchunk, long long tiles_mn = 1 << 20) {
+  const int target = tiles_mn >= 64 ? 4096 : 256;      // few output tiles: split deeper so that the grid fills the GPU
   long long s = (K + target - 1) / target; if (s < 1) s = 1; if (s > 2048) s = 2048;
   long long ch = (K + s - 1) / s; ch = (ch + 15) / 16 * 16;
   *splits = (int)((K + ch - 1) / ch); *kchunk = (int)ch;
 }
 
 size_t wgrad_partial_elems(const Geom& g, long long frames) {
-  int s, ch; wgrad_split(frames * g.Ho * g.Wo, &s, &ch);
+  int s, ch; wgrad_split(frames * g.Ho * g.Wo, &s, &ch, (long long)((g.kh * g.kw * g.Cin + 1 + 127) / 128) * ((g.Cout + 63) / 64));
   return (size_t)s * (g.kh * g.kw * g.Cin + 1) * g.Cout;
 }
 
@@ -212,7 +203,7 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
       size_t total = (size_t)F * pool_out(op.H) * pool_out(op.W) * op.C;
       ProfScope ps(K_POOL_FWD, st, 1, 0.0, (double)sizeof(AT) * (total + (double)F * op.H * op.W * op.C));
       if (std::is_same<AT, bf16>::value && op.C % 8 == 0)
-        pool_fwd_v8_kernel<<<grid_for(total / 8), 256, 0, st>>>((const bf16*)ws.act[op.in_t], (bf16*)ws.act[op.out_t], F, op.C, op.H, op.W);
+        pool_fwd_v8_kernel<<<grid_for(total / 8), 256, 0, st>>>((const bf16*)ws.act[op.in_t], (bf16*)ws.act[op.out_t], (uint8_t*)ws.act[op.mask_t], F, op.C, op.H, op.W);
       else
         pool_fwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (AT*)ws.act[op.out_t], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());
@@ -258,7 +249,7 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
       size_t total = (size_t)F * op.H * op.W * op.C;
       ProfScope ps(K_POOL_BWD, st, 1, 0.0, (double)sizeof(AT) * (2.0 * total + (double)F * pool_out(op.H) * pool_out(op.W) * op.C));
       if (std::is_same<AT, bf16>::value && op.C % 8 == 0)
-        pool_bwd_v8_kernel<<<grid_for(total / 8), 256, 0, st>>>((const bf16*)ws.act[op.in_t], (const bf16*)ws.grad[op.dy], (bf16*)ws.grad[op.dx], F, op.C, op.H, op.W);
+        pool_bwd_v8_kernel<<<grid_for(total / 8), 256, 0, st>>>((const uint8_t*)ws.act[op.mask_t], (const bf16*)ws.grad[op.dy], (bf16*)ws.grad[op.dx], F, op.C, op.H, op.W);
       else
         pool_bwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (const AT*)ws.grad[op.dy], (AT*)ws.grad[op.dx], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());
@@ -281,7 +272,7 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         continue;
       }
       int Kpix = F * g.Ho * g.Wo, M = g.kh * g.kw * g.Cin + 1, N = g.Cout, splits, kchunk;
-      wgrad_split(Kpix, &splits, &kchunk);
+      wgrad_split(Kpix, &splits, &kchunk, (long long)((M + 127) / 128) * ((N + 63) / 64));
       double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
       int rc;
       {

