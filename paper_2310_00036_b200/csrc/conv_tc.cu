@@ -87,17 +87,18 @@ struct ConvTcArgs {
   int* error_flag;
 };
 
-constexpr int TMEM_COLS = 256;
+constexpr int TMEM_COLS = 128;     // 128 columns and <= 72 KB of shared memory per CTA: three CTAs per SM overlap their phases
+constexpr int NT = 256;            // two warpgroups: both stage operands; each drains every second accumulator tile
 
 // MODE 0: out = acc + bias (+ aux0).   MODE 1: out = (aux0 ? (aux0 > 0 ? acc : 0) : acc) (+ aux1).
 template <int CIN, int COUT, int MODE>
-__global__ void __launch_bounds__(128) conv3x3_tc_kernel(const ConvTcArgs a) {
+__global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr int NCH = CIN / 8, KSTEPS = CIN / 16, TILES_PER_BATCH = TMEM_COLS / COUT;
   constexpr uint32_t W_BYTES = 9u * CIN * COUT * 2u;
   __shared__ __align__(8) uint64_t bar_storage;
   __shared__ uint32_t tmem_base_smem;
-  const int tid = threadIdx.x, warp = tid >> 5;
+  const int tid = threadIdx.x, warp = tid >> 5, wg = warp >> 2, lane_row = tid & 127;
   const int Wp = a.W + 2, R = (a.H + 2) * Wp;
   uint8_t* w_smem = smem;
   uint8_t* in_smem = smem + ((W_BYTES + 127u) & ~127u);
@@ -107,8 +108,8 @@ __global__ void __launch_bounds__(128) conv3x3_tc_kernel(const ConvTcArgs a) {
   if (tid == 0) mbar_init(bar, 1);
   if (warp == 0) tmem_alloc(smem_u32(&tmem_base_smem), TMEM_COLS);
   // weights (already in operand layout) and a zeroed input area (halo and slack stay zero for the whole kernel)
-  for (uint32_t i = tid; i < W_BYTES / 16; i += 128) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w)[i];
-  for (uint32_t i = tid; i < plane_bytes * NCH / 16; i += 128) reinterpret_cast<uint4*>(in_smem)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < W_BYTES / 16; i += NT) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w)[i];
+  for (uint32_t i = tid; i < plane_bytes * NCH / 16; i += NT) reinterpret_cast<uint4*>(in_smem)[i] = make_uint4(0, 0, 0, 0);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -121,22 +122,32 @@ __global__ void __launch_bounds__(128) conv3x3_tc_kernel(const ConvTcArgs a) {
   for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
     const int f0 = grp * a.G, nf = min(a.G, a.F - f0);
     // ---- stage the group's frames: global NHWC -> planes, ReLU on the way in --------------------------
-    const int per_frame = a.H * a.W * NCH;
-    for (int i = tid; i < a.G * per_frame; i += 128) {
-      int j = i / per_frame, rem = i - j * per_frame;
-      int ch = rem % NCH, pix = rem / NCH;
-      int y = pix / a.W, x = pix - y * a.W;
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (j < nf) {
-        v = *reinterpret_cast<const uint4*>(a.in + ((size_t)(f0 + j) * a.H * a.W + pix) * CIN + ch * 8);
+    const int per_frame = a.H * a.W * NCH, nwork = a.G * per_frame;
+    for (int i0 = tid; i0 < nwork; i0 += NT * 4) {       // 4 independent 16-byte loads in flight per thread
+      uint4 v[4]; uint32_t dst[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = i0 + u * NT;
+        v[u] = make_uint4(0, 0, 0, 0); dst[u] = 0xFFFFFFFFu;
+        if (i < nwork) {
+          int j = i / per_frame, rem = i - j * per_frame;
+          int ch = rem % NCH, pix = rem / NCH;
+          int y = pix / a.W, x = pix - y * a.W;
+          dst[u] = (uint32_t)ch * plane_bytes + (uint32_t)(j * R + (y + 1) * Wp + (x + 1)) * 16u;
+          if (j < nf) v[u] = *reinterpret_cast<const uint4*>(a.in + ((size_t)(f0 + j) * a.H * a.W + pix) * CIN + ch * 8);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (dst[u] == 0xFFFFFFFFu) continue;
         if (a.relu_in) {
-          __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+          __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v[u]);
           const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
 #pragma unroll
           for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
         }
+        *reinterpret_cast<uint4*>(in_smem + dst[u]) = v[u];
       }
-      *reinterpret_cast<uint4*>(in_smem + (size_t)ch * plane_bytes + (size_t)(j * R + (y + 1) * Wp + (x + 1)) * 16) = v;
     }
     fence_async_smem();
     __syncthreads();
@@ -166,8 +177,8 @@ __global__ void __launch_bounds__(128) conv3x3_tc_kernel(const ConvTcArgs a) {
       parity ^= 1;
       tc_fence_after();
       // ---- epilogue: TMEM lane = tile row = linear position; one thread per position ----------------------
-      for (int s = 0; s < nt; ++s) {
-        const int q = (t0 + s) * 128 + tid;
+      for (int s = wg; s < nt; s += 2) {
+        const int q = (t0 + s) * 128 + lane_row;
         const int j = q / R, rem = q - j * R;
         const int y = rem / Wp, x = rem - y * Wp;
         const bool valid = j < nf && y < a.H && x < a.W;
@@ -175,7 +186,7 @@ __global__ void __launch_bounds__(128) conv3x3_tc_kernel(const ConvTcArgs a) {
 #pragma unroll
         for (int c0 = 0; c0 < COUT; c0 += 16) {
           float v[16];
-          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(s * COUT + c0), v);   // warp-collective: no divergence before it
+          tmem_ld16(tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(s * COUT + c0), v);   // warp-collective: no divergence before it
           if (!valid) continue;
           if (MODE == 0) {
 #pragma unroll
@@ -229,7 +240,7 @@ struct TcPlan { int G, npix_alloc; size_t smem; };
 static TcPlan tc_plan(int H, int W, int cin, int cout) {
   const int Wp = W + 2, R = (H + 2) * Wp;
   const size_t wbytes = ((size_t)9 * cin * cout * 2 + 127) & ~(size_t)127;
-  const size_t budget = 96 * 1024;          // two CTAs per SM where the frame allows it
+  const size_t budget = 72 * 1024;          // three CTAs per SM where the frame allows it
   int G = (int)((budget > wbytes ? budget - wbytes : 0) / ((size_t)R * cin * 2));
   if (G < 1) G = 1;
   if (G > 8) G = 8;
@@ -245,8 +256,8 @@ static int launch_one(const tc::ConvTcArgs& a, size_t smem, int ngroups, cudaStr
     CB_CUDA(cudaFuncSetAttribute(tc::conv3x3_tc_kernel<CIN, COUT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
-  int grid = std::min(ngroups, 2 * 148);
-  tc::conv3x3_tc_kernel<CIN, COUT, MODE><<<grid, 128, smem, st>>>(a);
+  int grid = std::min(ngroups, 3 * 148);
+  tc::conv3x3_tc_kernel<CIN, COUT, MODE><<<grid, tc::NT, smem, st>>>(a);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }

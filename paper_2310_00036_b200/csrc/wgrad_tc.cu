@@ -67,7 +67,7 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
 }
 
-constexpr int NLOAD = 128;       // warps 0-3: stage operands, later read TMEM; warp 4: one thread issues the MMAs
+constexpr int NLOAD = 256;       // warps 0-7: stage operands (warps 0-3 later read TMEM); warp 8: one thread issues the MMAs
 
 // UM = UMMA M (64 or 128): rows 0..CIN(+bias) are real, the rest walks into the following planes and is ignored.
 // Two shared-memory stages: the loader warps fill stage s+1 while the tensor core works on stage s.
@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
     for (int i = 0; i < 5; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
-  if (warp == 4) {
+  if (warp == NLOAD / 32) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" :: "r"(smem_u32(&tmem_base_smem)), "r"(TCOLS) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
   }
@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
   const int ngroups = (a.F + a.G - 1) / a.G, nitems = ngroups * a.nbands;
   const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  if (warp < 4) {
+  if (warp < NLOAD / 32) {
     // ================= loaders =================
     for (int it = 0; it < my_items; ++it) {
       const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
@@ -119,37 +119,58 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
       const int grp = item / a.nbands, band = item - grp * a.nbands;
       const int f0 = grp * a.G, nf = min(a.G, a.F - f0), yb = band * a.R;
       const int xn = a.G * Rb * XCH;
-      for (int i = tid; i < xn; i += NLOAD) {
-        int ch = i % XCH, pos = i / XCH;
-        int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, xp = rem - lr * Wp;
-        int y = yb - 1 + lr, x = xp - 1;
-        uint4 v = make_uint4(0, 0, 0, 0);
-        if (j < nf && (unsigned)y < (unsigned)a.H && (unsigned)x < (unsigned)a.W) {
-          v = *reinterpret_cast<const uint4*>(a.x + (((size_t)(f0 + j) * a.H + y) * a.W + x) * CIN + ch * 8);
+      for (int i0 = tid; i0 < xn; i0 += NLOAD * 4) {
+        uint4 v[4]; uint32_t dst[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int i = i0 + u * NLOAD;
+          v[u] = make_uint4(0, 0, 0, 0); dst[u] = 0xFFFFFFFFu;
+          if (i < xn) {
+            int ch = i % XCH, pos = i / XCH;
+            int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, xp = rem - lr * Wp;
+            int y = yb - 1 + lr, x = xp - 1;
+            dst[u] = (uint32_t)ch * P + (uint32_t)pos * 16u;
+            if (j < nf && (unsigned)y < (unsigned)a.H && (unsigned)x < (unsigned)a.W)
+              v[u] = *reinterpret_cast<const uint4*>(a.x + (((size_t)(f0 + j) * a.H + y) * a.W + x) * CIN + ch * 8);
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (dst[u] == 0xFFFFFFFFu) continue;
           if (a.relu_in) {
-            __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+            __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v[u]);
             const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
 #pragma unroll
             for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
           }
+          *reinterpret_cast<uint4*>(xs + dst[u]) = v[u];
         }
-        *reinterpret_cast<uint4*>(xs + (size_t)ch * P + (size_t)pos * 16) = v;
       }
       const int yn = a.kext * YCH;
-      for (int i = tid; i < yn; i += NLOAD) {
-        int ch = i % YCH, pos = i / YCH;
-        int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, x = rem - lr * Wp;
-        int y = yb + lr;
-        uint4 v = make_uint4(0, 0, 0, 0);
-        if (j < nf && lr < a.R && y < a.H && x < a.W)
-          v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)(f0 + j) * a.H + y) * a.W + x) * COUT + ch * 8);
-        *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
+      for (int i0 = tid; i0 < yn; i0 += NLOAD * 4) {
+        uint4 v[4]; uint32_t dst[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int i = i0 + u * NLOAD;
+          v[u] = make_uint4(0, 0, 0, 0); dst[u] = 0xFFFFFFFFu;
+          if (i < yn) {
+            int ch = i % YCH, pos = i / YCH;
+            int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, x = rem - lr * Wp;
+            int y = yb + lr;
+            dst[u] = (uint32_t)ch * P + (uint32_t)pos * 16u;
+            if (j < nf && lr < a.R && y < a.H && x < a.W)
+              v[u] = *reinterpret_cast<const uint4*>(a.dy + (((size_t)(f0 + j) * a.H + y) * a.W + x) * COUT + ch * 8);
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) if (dst[u] != 0xFFFFFFFFu) *reinterpret_cast<uint4*>(ys + dst[u]) = v[u];
       }
       asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
       asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
       if (tid == 0) mbar_arrive(bar0 + 8u * s);
     }
-    // ================= epilogue =================
+    // ================= epilogue (warps 0-3 own the TMEM lanes) =================
+    if (warp < 4) {
     if (my_items > 0 && !mbar_wait(bar0 + 8u * 4, 0u)) { if (a.error_flag) *a.error_flag = 2; }
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
     float* out = a.partial + (size_t)blockIdx.x * 9 * (CIN + 1) * COUT;
@@ -169,6 +190,7 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
           }
         }
       }
+    }
     }
   } else if (tid == NLOAD) {
     // ================= MMA issuer =================
@@ -195,7 +217,7 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
   }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
-  if (warp == 4) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tmem_base), "r"(TCOLS) : "memory");
+  if (warp == NLOAD / 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tmem_base), "r"(TCOLS) : "memory");
 }
 
 // sums the per-CTA partials in CTA order and scatters to the canonical gradient
