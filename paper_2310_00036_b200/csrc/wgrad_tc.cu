@@ -71,11 +71,16 @@ constexpr int NLOAD = 256;       // warps 0-7: stage operands (warps 0-3 later r
 
 // UM = UMMA M (64 or 128): rows 0..CIN(+bias) are real, the rest walks into the following planes and is ignored.
 // Two shared-memory stages: the loader warps fill stage s+1 while the tensor core works on stage s.
-template <int CIN, int COUT, int UM>
+// ST3 (Cin = 16 only): the loaders store every X element three times, shifted by dj = 0,1,2 positions, into planes
+// (dj, chunk); the M walk of ONE MMA then covers the three taps (di, 0..2) at rows dj*CIN + c -- 3 instead of 9
+// MMAs per 16 positions, and 49 instead of 17 useful rows of 64.
+template <int CIN, int COUT, int UM, bool ST3>
 __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcArgs a) {
   extern __shared__ __align__(128) uint8_t smem[];
-  constexpr int XCH = CIN / 8, YCH = COUT / 8;
-  constexpr uint32_t TCOLS = (9 * COUT <= 256) ? 256u : 512u;
+  constexpr int XCH = CIN / 8, YCH = COUT / 8, XPL = ST3 ? 3 * XCH : XCH;      // X planes per stage
+  constexpr int NACC = ST3 ? 3 : 9;
+  constexpr uint32_t TCOLS = (NACC * COUT <= 128) ? 128u : ((NACC * COUT <= 256) ? 256u : 512u);
+  static_assert(!ST3 || 3 * CIN + 1 <= UM, "3-tap stacking needs 3*CIN+1 rows");
   __shared__ __align__(8) uint64_t bars[5];          // full[2], empty[2], done
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5;
@@ -99,7 +104,7 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
   {
     const uint32_t one2 = 0x3F803F80u;    // two bf16 ones
     for (int st = 0; st < 2; ++st)
-      for (uint32_t i = tid; i < P / 16; i += NLOAD + 32) reinterpret_cast<uint4*>(smem + (size_t)st * stage_bytes + (size_t)XCH * P)[i] = make_uint4(one2, one2, one2, one2);
+      for (uint32_t i = tid; i < P / 16; i += NLOAD + 32) reinterpret_cast<uint4*>(smem + (size_t)st * stage_bytes + (size_t)XPL * P)[i] = make_uint4(one2, one2, one2, one2);
   }
   asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -115,7 +120,7 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
       const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
       if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 2; }
       uint8_t* xs = smem + (size_t)s * stage_bytes;
-      uint8_t* ys = xs + (size_t)(XCH + 1) * P;
+      uint8_t* ys = xs + (size_t)(XPL + 1) * P;
       const int grp = item / a.nbands, band = item - grp * a.nbands;
       const int f0 = grp * a.G, nf = min(a.G, a.F - f0), yb = band * a.R;
       const int xn = a.G * Rb * XCH;
@@ -144,6 +149,11 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
             for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
           }
           *reinterpret_cast<uint4*>(xs + dst[u]) = v[u];
+          if (ST3) {      // dst = ch*P + pos*16: the copies for dj = 1, 2 live XCH / 2*XCH planes further, 1 / 2 positions earlier
+            const uint32_t pos16 = dst[u] % P;
+            if (pos16 >= 16u) *reinterpret_cast<uint4*>(xs + dst[u] + (uint32_t)XCH * P - 16u) = v[u];
+            if (pos16 >= 32u) *reinterpret_cast<uint4*>(xs + dst[u] + 2u * (uint32_t)XCH * P - 32u) = v[u];
+          }
         }
       }
       const int yn = a.kext * YCH;
@@ -177,17 +187,20 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
     // UM = 128: accumulator row r sits in TMEM lane r; UM = 64: in lane 32*(r/16) + r%16
     const int lane = tid & 31;
     const int row = (UM == 128) ? tid : ((lane < 16) ? warp * 16 + lane : 1 << 20);
-    const bool warp_needed = (UM == 128) ? (warp * 32 <= CIN) : (warp * 16 <= CIN);
+    constexpr int LAST_ROW = ST3 ? 3 * CIN : CIN;         // the bias row
+    const bool warp_needed = (UM == 128) ? (warp * 32 <= LAST_ROW) : (warp * 16 <= LAST_ROW);
     if (warp_needed) {
-      for (int tap = 0; tap < 9; ++tap) {
+      for (int acc = 0; acc < NACC; ++acc) {
 #pragma unroll
         for (int c0 = 0; c0 < COUT; c0 += 16) {
           float v[16];
-          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(tap * COUT + c0), v);
-          if (row <= CIN) {
+          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(acc * COUT + c0), v);
+          if (row > LAST_ROW) continue;
+          int tap, r;
+          if (ST3) { if (row == LAST_ROW) { if (acc) continue; tap = 0; r = CIN; } else { tap = acc * 3 + row / CIN; r = row % CIN; } }
+          else { tap = acc; r = row; }
 #pragma unroll
-            for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + row) * COUT + c0 + i] = my_items > 0 ? v[i] : 0.f;
-          }
+          for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + r) * COUT + c0 + i] = v[i];
         }
       }
     }
@@ -200,14 +213,14 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
       const int s = it & 1, use = it >> 1;
       if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
       asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-      const uint32_t x_base = smem_u32(smem + (size_t)s * stage_bytes), y_base = x_base + (uint32_t)(XCH + 1) * P;
+      const uint32_t x_base = smem_u32(smem + (size_t)s * stage_bytes), y_base = x_base + (uint32_t)(XPL + 1) * P;
       for (int k0 = 0; k0 < a.kext; k0 += 16) {
         const uint64_t bd = make_desc(y_base + (uint32_t)k0 * 16u, 128u, P);
 #pragma unroll
-        for (int tap = 0; tap < 9; ++tap) {
-          const uint32_t shift = (uint32_t)((tap / 3) * Wp + (tap % 3));
+        for (int acc = 0; acc < NACC; ++acc) {
+          const uint32_t shift = ST3 ? (uint32_t)(acc * Wp) : (uint32_t)((acc / 3) * Wp + (acc % 3));
           const uint64_t ad = make_desc(x_base + ((uint32_t)k0 + shift) * 16u, 128u, P);
-          mma_f16(tmem_base + (uint32_t)(tap * COUT), ad, bd, idesc, accumulate);
+          mma_f16(tmem_base + (uint32_t)(acc * COUT), ad, bd, idesc, accumulate);
         }
         accumulate = 1;
       }
@@ -246,9 +259,10 @@ constexpr int WGRAD_UM = 64;      // UMMA M of the weight-gradient kernel (128 =
 
 struct WPlan { int G, R, nbands, npix_alloc, kext, stage_planes; size_t smem; };
 static WPlan wgrad_plan(int H, int W, int cin, int cout) {
+  const int xpl = (cin == 16 ? 3 : 1) * (cin / 8);
   const int Wp = W + 2, slack = 2 * Wp + 2;
   WPlan p;
-  p.stage_planes = std::max(WGRAD_UM / 8, cin / 8 + 1 + cout / 8);
+  p.stage_planes = std::max(WGRAD_UM / 8, xpl + 1 + cout / 8);
   const int total_planes = p.stage_planes + std::max(p.stage_planes, WGRAD_UM / 8);
   const int maxpix = (216 * 1024) / (16 * total_planes);
   if ((H + 2) * Wp + slack + 16 <= maxpix) {
@@ -267,10 +281,10 @@ template <int CIN, int COUT>
 static int launch_w(const tcw::WgradTcArgs& a, size_t smem, int grid, cudaStream_t st) {
   static size_t configured = 0;
   if (smem > configured) {
-    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT, WGRAD_UM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT, WGRAD_UM, CIN == 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
-  tcw::wgrad3x3_tc_kernel<CIN, COUT, WGRAD_UM><<<grid, tcw::NLOAD + 32, smem, st>>>(a);
+  tcw::wgrad3x3_tc_kernel<CIN, COUT, WGRAD_UM, CIN == 16><<<grid, tcw::NLOAD + 32, smem, st>>>(a);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
