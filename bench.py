@@ -299,6 +299,23 @@ def main():
     t_e2e = max_over_ranks(max(e0.elapsed_time(e1) / 1e3, time.perf_counter() - w0), world)
     e2e_value = frames / t_e2e
 
+    # ---- actor side (BASELINE.json configs[1]): policy/value inference + Gumbel-max sampling, B = 128, bf16 mode ----
+    inference = None
+    if rank == 0 and arch.kind == "impala":
+        Bi = 128
+        obs_i = [dev_sets[i % len(dev_sets)]["obs"].reshape(-1, arch.in_c, arch.in_h, arch.in_w)[j * Bi:(j + 1) * Bi].contiguous()
+                 for i in range(N_ROTATE) for j in range(4)]
+        for i in range(5):
+            net.policy_forward(dp, obs_i[i % len(obs_i)], seed=1, step=i, precision=prec)
+        torch.cuda.synchronize()
+        li = binding.launch_count(); ncall = 100
+        e0.record(stream)
+        for i in range(ncall):
+            net.policy_forward(dp, obs_i[i % len(obs_i)], seed=1, step=i, precision=prec)
+        e1.record(stream); torch.cuda.synchronize()
+        us = 1e3 * e0.elapsed_time(e1) / ncall
+        inference = {"workload": "BASELINE.json configs[1]: IMPALA-ResNet policy/value forward + Gumbel-max sampling, B=128, bf16 mode",
+                     "us_per_call": us, "env_frames_per_s": Bi / (us * 1e-6), "launches_per_call": (binding.launch_count() - li) / ncall}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -326,7 +343,7 @@ def main():
                      "traffic": None, "peak_source": f"{peaks['src']} ({'sustained bf16' if bound == 'tensor' else 'copy'})",
                      "launches": dom["launches"], "ms_per_launch": 1e3 * per_launch_s, "share_of_step": dom["ms"] / (1e3 * t_local)},
         "kernel_breakdown_ms_per_step": {e["name"]: round(e["ms"], 4) for e in sorted(prof_all, key=lambda e: -e["ms"])},
-        "kernel_breakdown_total_ms": total_ms, "loss": loss_last,
+        "kernel_breakdown_total_ms": total_ms, "loss": loss_last, "inference": inference,
     }
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(args.config, cfg)

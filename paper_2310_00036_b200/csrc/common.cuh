@@ -148,6 +148,11 @@ int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* fr
 int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, float* partial,
                        float* grad, int* error_flag, cudaStream_t st);
 
+// dense_tc.cu
+bool dense_tc_supported(const Geom& g);
+int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wf, const float* bias, bf16* out, bool relu_in, int* error_flag, cudaStream_t st);
+int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* A, const bf16* dy, bool relu_in, float* grad, int* error_flag, cudaStream_t st);
+
 // rl.cu
 int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset,
                   int32_t* actions, cudaStream_t st);

@@ -220,6 +220,8 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out) {
       rc = launch_conv_tc(0, F, g.H, g.W, g.Cin, g.Cout, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (const bf16*)skip, nullptr,
                           (bf16*)ws.act[L.out_t], L.relu_in, ws.errflag, st);
+    } else if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
+      rc = launch_dense_fwd_tc(g, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.wf + L.wf_off, bias, (bf16*)ws.act[L.out_t], L.relu_in, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(g)) {
       rc = launch_conv0_fwd(g, F, obs, frame_idx, ws.w0img, bias, (bf16*)ws.act[L.out_t], ws.errflag, st);
     } else if (L.u8_in) {
@@ -262,6 +264,12 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         ProfScope ps(K_CONV_WGRAD, st, 2, 2.0 * 9 * g.Cin * g.Cout * (double)F * g.Ho * g.Wo,
                      2.0 * F * g.H * g.W * (g.Cin + g.Cout) + 4.0 * 9 * (g.Cin + 1) * g.Cout);
         int rc = launch_wgrad_tc(g, L.pm, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.grad[op.dy], L.relu_in, ws.partial, grad, ws.errflag, st);
+        if (rc) return rc;
+        continue;
+      }
+      if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
+        ProfScope ps(K_CONV_WGRAD, st, 2, 2.0 * g.H * g.W * g.Cin * g.Cout * (double)F, 2.0 * F * (g.H * g.W * g.Cin + g.Cout) + 4.0 * g.H * g.W * g.Cin * g.Cout);
+        int rc = launch_dense_wgrad_tc(g, L.pm, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.grad[op.dy], L.relu_in, grad, ws.errflag, st);
         if (rc) return rc;
         continue;
       }
