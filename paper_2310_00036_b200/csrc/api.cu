@@ -159,6 +159,14 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
     CB_ALLOC(ws.wf, net->wf_total * es); CB_ALLOC(ws.wd, net->wd_total * es); CB_ALLOC(ws.bias, net->bias_total * 4);
     if (prec == CB_PREC_BF16_TC) { CB_ALLOC(ws.w0img, conv0_wimg_elems(net->layers[0].g) * 2); CB_ALLOC(ws.wtc_f, net->wf_total * 2); CB_ALLOC(ws.wtc_d, net->wf_total * 2); }
     CB_ALLOC(ws.errflag, 16); CB_CUDA(cudaMemset(ws.errflag, 0, 16));
+    {
+      std::vector<PackDesc> tab;
+      for (const Layer& L : net->layers)
+        tab.push_back({L.g, L.pm, L.wf_off, L.bias_off, (prec == CB_PREC_BF16_TC && conv_tc_supported(L.g)) ? 1 : 0,
+                       (prec == CB_PREC_BF16_TC && L.u8_in && conv0_tc_supported(L.g)) ? 1 : 0});
+      CB_ALLOC(ws.packtab, tab.size() * sizeof(PackDesc));
+      CB_CUDA(cudaMemcpy(ws.packtab, tab.data(), tab.size() * sizeof(PackDesc), cudaMemcpyHostToDevice));
+    }
     CB_ALLOC(ws.gradbuf, net->P * 4); CB_ALLOC(ws.adam_scratch, clip_adam_scratch_bytes(net->P)); CB_ALLOC(ws.gnorm, 16);
   }
   if (ws.frames >= frames) return CB_OK;
@@ -174,6 +182,7 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
     pe = std::max(pe, wgrad_partial_elems(L.g, frames));
     if (wgrad_tc_supported(L.g)) pe = std::max(pe, wgrad_tc_partial_elems(L.g));
     if (L.u8_in && conv0_tc_supported(L.g)) pe = std::max(pe, conv0_partial_elems(L.g));
+    if (dense_tc_supported(L.g)) pe = std::max(pe, (size_t)8 * std::min(frames, 1024) * L.g.Cout);
   }
   CB_ALLOC(ws.partial, pe * 4); ws.partial_elems = pe;
   ws.frames = frames;
@@ -236,7 +245,7 @@ void cb_net_destroy(cb_net* net) {
     Workspace& ws = net->ws[p];
     if (!ws.wf) continue;
     free_workspace(ws); free_scratch(ws);
-    cudaFree(ws.w0img); cudaFree(ws.wtc_f); cudaFree(ws.wtc_d); cudaFree(ws.errflag);
+    cudaFree(ws.packtab); cudaFree(ws.w0img); cudaFree(ws.wtc_f); cudaFree(ws.wtc_d); cudaFree(ws.errflag);
     cudaFree(ws.wf); cudaFree(ws.wd); cudaFree(ws.bias); cudaFree(ws.gradbuf); cudaFree(ws.adam_scratch); cudaFree(ws.gnorm);
   }
   delete net;
@@ -288,11 +297,13 @@ int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int 
   cudaStream_t st = (cudaStream_t)stream; int rc;
   if ((rc = ensure_workspace(net, precision, B))) return rc;
   if ((rc = pack_weights(net, precision, params, st))) return rc;
-  if ((rc = forward(net, precision, obs, nullptr, B, st))) return rc;
-  const float* head = (const float*)net->ws[precision].act[net->head_t];
-  int A = net->arch.n_actions;
-  if (logits || value) if ((rc = launch_split_head(head, B, A, logits, value, st))) return rc;
-  if (actions) if ((rc = launch_sample(head, A + 1, B, A, seed, step, env_offset, actions, st))) return rc;
+  if ((rc = forward(net, precision, obs, nullptr, B, st, true))) return rc;      // everything up to the hidden layer
+  Workspace& ws = net->ws[precision];
+  const Layer& HL = net->layers.back();
+  const int A = net->arch.n_actions;
+  const size_t es = precision == CB_PREC_FP32_REF ? 4 : 2;
+  if ((rc = launch_heads_sample(precision, ws.act[net->hid_t], (const char*)ws.wf + HL.wf_off * es, ws.bias + HL.bias_off, B, net->arch.fc, A, seed, step,
+                                env_offset, (float*)ws.act[net->head_t], logits, value, actions, st))) return rc;
   return CB_OK;
 }
 

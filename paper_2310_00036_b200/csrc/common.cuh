@@ -63,6 +63,9 @@ struct Op {
   int add;          // DGRAD: gradient buffer added after masking (-1 none)
 };
 
+// one entry per layer of the single-launch weight-packing kernel
+struct PackDesc { Geom g; ParamMap pm; size_t wf_off, bias_off; int tc, conv0; };
+
 struct Tensor { size_t per_frame; bool f32; int esize; };   // esize: bytes per element, 0 = the mode's storage type
 
 struct Workspace {     // one per precision mode
@@ -72,6 +75,7 @@ struct Workspace {     // one per precision mode
   void* wf = nullptr; void* wd = nullptr; float* bias = nullptr;   // packed weights (mode type), fp32 bias
   bf16* w0img = nullptr;                                           // first-layer forward B image (conv0_tc.cu)
   bf16* wtc_f = nullptr; bf16* wtc_d = nullptr;                     // tcgen05 B-operand packs (forward / dgrad), bf16 mode only
+  PackDesc* packtab = nullptr;                                     // device copy of the layer table for packing
   int* errflag = nullptr;                                          // set by a kernel whose tcgen05 pipeline timed out
   float* partial = nullptr; size_t partial_elems = 0;             // wgrad split-K partials
   float* gradbuf = nullptr;          // [P]
@@ -124,7 +128,7 @@ struct ProfScope {      // counts `n` launches of class `cls`; records an event 
 int ensure_workspace(cb_net* net, int prec, int frames);
 int ensure_learner_scratch(cb_net* net, int prec, int F, int N, int epochs);
 int pack_weights(cb_net* net, int prec, const float* params, cudaStream_t st);
-int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st);
+int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads = false);
 int backward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, float* grad, cudaStream_t st);
 
 // conv_tc.cu
@@ -150,12 +154,14 @@ int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* 
 
 // dense_tc.cu
 bool dense_tc_supported(const Geom& g);
-int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wf, const float* bias, bf16* out, bool relu_in, int* error_flag, cudaStream_t st);
+int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wf, const float* bias, bf16* out, bool relu_in, float* partial, int* error_flag, cudaStream_t st);
 int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* A, const bf16* dy, bool relu_in, float* grad, int* error_flag, cudaStream_t st);
 
 // rl.cu
 int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset,
                   int32_t* actions, cudaStream_t st);
+int launch_heads_sample(int prec, const void* hid, const void* wf, const float* bias, int B, int fc, int A, uint64_t seed, uint64_t step,
+                        uint32_t env_offset, float* head, float* logits, float* value, int32_t* actions, cudaStream_t st);
 int launch_split_head(const float* head, int F, int A, float* logits, float* value, cudaStream_t st);
 int launch_logprob(const float* logits, int ld, int N, int A, const int32_t* actions, const int32_t* idx,
                    float* logp_a, float* entropy, cudaStream_t st);

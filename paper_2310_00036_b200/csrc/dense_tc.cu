@@ -20,6 +20,7 @@ struct Args {
   bf16* out;          // MODE 0: [F][N]
   float* grad;        // MODE 1: canonical fp32 gradient buffer
   int F, K, N, relu_in;
+  float* part; int ksplit;      // MODE 0 with ksplit > 1: fp32 partial sums [ksplit][F][N] instead of out
   int H, W, C; size_t w_off;   // MODE 1: feature k = (y*W + x)*C + c  ->  canonical fc.w index n*K + (c*H + y)*W + x
   int* error_flag;
 };
@@ -58,11 +59,13 @@ __global__ void __launch_bounds__(NLOAD + 32) dense_tc_kernel(const Args a) {
   const uint32_t tmem_base = tmem_base_smem;
   const int m0 = blockIdx.x * 128, n0 = blockIdx.y * BN;
   const int L = MODE == 0 ? a.K : a.F;                  // contraction length
-  const int ntiles = (L + BK - 1) / BK;
+  const int all_tiles = (L + BK - 1) / BK;
+  const int per_z = (all_tiles + (int)gridDim.z - 1) / (int)gridDim.z;
+  const int tbeg = (int)blockIdx.z * per_z, ntiles = max(0, min(all_tiles, tbeg + per_z) - tbeg);      // this CTA's k-tiles
 
   if (warp < NLOAD / 32) {
     for (int t = 0; t < ntiles; ++t) {
-      const int s = t % NSTAGE, use = t / NSTAGE, l0 = t * BK;
+      const int s = t % NSTAGE, use = t / NSTAGE, l0 = (tbeg + t) * BK;
       if (use > 0 && !mbar_wait(bar0 + 8u * (NSTAGE + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 5; }
       uint8_t* as = smem + (size_t)s * STAGE; uint8_t* bs = as + APL * PA;
       // ---- A tile ----
@@ -96,7 +99,7 @@ __global__ void __launch_bounds__(NLOAD + 32) dense_tc_kernel(const Args a) {
       if (tid == 0) mbar_arrive(bar0 + 8u * s);
     }
     if (warp < 4) {
-      if (!mbar_wait(bar0 + 8u * (2 * NSTAGE), 0u)) { if (a.error_flag) *a.error_flag = 5; }
+      if (ntiles > 0 && !mbar_wait(bar0 + 8u * (2 * NSTAGE), 0u)) { if (a.error_flag) *a.error_flag = 5; }
       tc_fence_after();
       const int row = m0 + tid;
 #pragma unroll
@@ -107,6 +110,11 @@ __global__ void __launch_bounds__(NLOAD + 32) dense_tc_kernel(const Args a) {
         if (n >= a.N) continue;
         if (MODE == 0) {
           if (row >= a.F) continue;
+          if (a.ksplit > 1) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) a.part[((size_t)blockIdx.z * a.F + row) * a.N + n + i] = ntiles > 0 ? v[i] : 0.f;
+            continue;
+          }
 #pragma unroll
           for (int i = 0; i < 16; ++i) v[i] += a.bias[n + i];
           uint4 o0, o1;
@@ -139,10 +147,20 @@ __global__ void __launch_bounds__(NLOAD + 32) dense_tc_kernel(const Args a) {
       }
       mma_commit(bar0 + 8u * (NSTAGE + s));
     }
-    mma_commit(bar0 + 8u * (2 * NSTAGE));
+    if (ntiles > 0) mma_commit(bar0 + 8u * (2 * NSTAGE));
   }
   tc_fence_before(); __syncthreads();
   if (warp == NLOAD / 32) tmem_dealloc(tmem_base, TCOLS);
+}
+
+// out[f][n] = bf16(sum_z part[z][f][n] + bias[n]), z in order
+__global__ void dense_reduce_kernel(const float* __restrict__ part, int S, int F, int N, const float* __restrict__ bias, bf16* __restrict__ out) {
+  size_t total = (size_t)F * N;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    float s = 0.f;
+    for (int z = 0; z < S; ++z) s += part[(size_t)z * total + i];
+    out[i] = __float2bfloat16_rn(s + bias[i % N]);
+  }
 }
 
 // db[n] = sum_f dY[f][n], serial in f (fixed order), one thread per n
@@ -162,6 +180,7 @@ bool dense_tc_supported(const Geom& g) {
 
 template <int MODE, int BN>
 static int launch_d(const dn::Args& a, dim3 grid, cudaStream_t st) {
+  if (a.ksplit > 1) grid.z = a.ksplit;
   constexpr size_t PA = (MODE == 0 ? 128 : dn::BK) * 16 + 16;
   constexpr size_t smem = dn::NSTAGE * ((MODE == 0 ? dn::BK / 8 : 16) * PA + (BN / 8) * dn::PB);
   static bool configured = false;
@@ -171,17 +190,22 @@ static int launch_d(const dn::Args& a, dim3 grid, cudaStream_t st) {
   return CB_OK;
 }
 
-int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wf, const float* bias, bf16* out, bool relu_in, int* error_flag, cudaStream_t st) {
+int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wf, const float* bias, bf16* out, bool relu_in, float* partial, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
   const int K = g.H * g.W * g.Cin, N = g.Cout;
-  dn::Args a{A, wf, bias, out, nullptr, F, K, N, relu_in ? 1 : 0, g.H, g.W, g.Cin, 0, error_flag};
-  return launch_d<0, 32>(a, dim3((F + 127) / 128, (N + 31) / 32), st);
+  const int ksplit = (F <= 1024 && partial) ? 8 : 1;      // few frames (actor side): split the contraction so that the grid fills the GPU
+  dn::Args a{A, wf, bias, out, nullptr, F, K, N, relu_in ? 1 : 0, partial, ksplit, g.H, g.W, g.Cin, 0, error_flag};
+  int rc = launch_d<0, 32>(a, dim3((F + 127) / 128, (N + 31) / 32), st);
+  if (rc || ksplit == 1) return rc;
+  dn::dense_reduce_kernel<<<std::min((F * N + 255) / 256, 1184), 256, 0, st>>>(partial, ksplit, F, N, bias, out);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
 }
 
 int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* A, const bf16* dy, bool relu_in, float* grad, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
   const int K = g.H * g.W * g.Cin, N = g.Cout;
-  dn::Args a{A, dy, nullptr, nullptr, grad, F, K, N, relu_in ? 1 : 0, g.H, g.W, g.Cin, pm.w_off, error_flag};
+  dn::Args a{A, dy, nullptr, nullptr, grad, F, K, N, relu_in ? 1 : 0, nullptr, 1, g.H, g.W, g.Cin, pm.w_off, error_flag};
   int rc = launch_d<1, 64>(a, dim3((K + 127) / 128, (N + 63) / 64), st);
   if (rc) return rc;
   dn::colsum_kernel<<<(N + 127) / 128, 128, 0, st>>>(dy, F, N, grad + pm.b_off);

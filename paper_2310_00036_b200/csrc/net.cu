@@ -35,17 +35,46 @@ __global__ void pack_tc_kernel(const float* __restrict__ params, Geom g, ParamMa
   }
 }
 
+// all layers in ONE launch: blockIdx.y = layer, blocks of a layer stride over its weights.  Per weight element:
+// Wf, Wd (SIMT operands), bias, and for the tensor-core layers the B-operand images of conv_tc.cu / conv0_tc.cu.
+template <typename AT>
+__global__ void pack_all_kernel(const float* __restrict__ params, const PackDesc* __restrict__ tab, AT* wf_all, AT* wd_all, float* bias_all,
+                                bf16* wtf_all, bf16* wtd_all, bf16* w0img) {
+  const PackDesc d = tab[blockIdx.y];
+  const Geom g = d.g;
+  const int K = g.kh * g.kw * g.Cin;
+  const size_t total = (size_t)K * g.Cout;
+  AT* wf = wf_all + d.wf_off; AT* wd = wd_all + d.wf_off; float* bias = bias_all + d.bias_off;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    int n = (int)(i % g.Cout); int k = (int)(i / g.Cout);
+    int c = k % g.Cin; int q = k / g.Cin; int dj = q % g.kw, di = q / g.kw;
+    float v = params[d.pm.w(n, c, di, dj, g)];
+    stv(wf, i, v);
+    stv(wd, ((size_t)(di * g.kw + dj) * g.Cout + n) * g.Cin + c, v);
+    if (k == 0) bias[n] = params[d.pm.b(n)];
+    if (d.tc) {
+      const int tap = di * 3 + dj, tapd = (2 - di) * 3 + (2 - dj);
+      const bf16 h = __float2bfloat16_rn(v);
+      (wtf_all + d.wf_off)[(((size_t)tap * (g.Cin / 8) + c / 8) * g.Cout + n) * 8 + c % 8] = h;
+      (wtd_all + d.wf_off)[(((size_t)tapd * (g.Cout / 8) + n / 8) * g.Cin + c) * 8 + n % 8] = h;
+    }
+  }
+  if (d.conv0) {      // forward B image [slot = 2*di + h][chunk][o][8]: chunks (di, 2h), (di, 2h+1); channels >= Cin and dj = 3 are zero
+    const int tot0 = 6 * 2 * g.Cout * 8;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < tot0; i += gridDim.x * blockDim.x) {
+      int c = i & 7, o = (i >> 3) % g.Cout, chunk = ((i >> 3) / g.Cout) & 1, slot = (i >> 3) / g.Cout / 2;
+      int di = slot >> 1, dj = (slot & 1) * 2 + chunk;
+      float v = (c < g.Cin && dj < 3) ? params[d.pm.w(o, c, di, dj, g)] : 0.f;
+      w0img[i] = __float2bfloat16_rn(v);
+    }
+  }
+}
+
 template <typename AT>
 static int pack_all(cb_net* net, Workspace& ws, const float* params, cudaStream_t st) {
-  ProfScope ps(K_PACK, st, (int)net->layers.size(), 0.0, (double)net->P * (4 + 2 * sizeof(AT)));
-  for (auto& L : net->layers) {
-    size_t total = (size_t)L.g.kh * L.g.kw * L.g.Cin * L.g.Cout;
-    int blocks = (int)std::min<size_t>((total + 255) / 256, 1184);
-    pack_kernel<AT><<<blocks, 256, 0, st>>>(params, L.g, L.pm, (AT*)ws.wf + L.wf_off, (AT*)ws.wd + L.wd_off, ws.bias + L.bias_off);
-    if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(L.g)) { int rc = launch_conv0_pack(L.g, L.pm, params, ws.w0img, st); if (rc) return rc; }
-    if (std::is_same<AT, bf16>::value && conv_tc_supported(L.g))
-      pack_tc_kernel<<<blocks, 256, 0, st>>>(params, L.g, L.pm, ws.wtc_f + L.wf_off, ws.wtc_d + L.wf_off);
-  }
+  ProfScope ps(K_PACK, st, 1, 0.0, (double)net->P * (4 + 2 * sizeof(AT)));
+  dim3 grid(64, (unsigned)net->layers.size());
+  pack_all_kernel<AT><<<grid, 256, 0, st>>>(params, ws.packtab, (AT*)ws.wf, (AT*)ws.wd, ws.bias, ws.wtc_f, ws.wtc_d, ws.w0img);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
@@ -197,8 +226,9 @@ size_t wgrad_partial_elems(const Geom& g, long long frames) {
 static inline int grid_for(size_t total) { return (int)std::min<size_t>((total + 255) / 256, (size_t)148 * 16); }
 
 template <typename AT>
-static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st) {
+static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads) {
   for (const Op& op : net->fwd) {
+    if (skip_heads && op.kind == OP_CONV && net->layers[op.layer].f32_out) continue;
     if (op.kind == OP_POOL) {
       size_t total = (size_t)F * pool_out(op.H) * pool_out(op.W) * op.C;
       ProfScope ps(K_POOL_FWD, st, 1, 0.0, (double)sizeof(AT) * (total + (double)F * op.H * op.W * op.C));
@@ -221,7 +251,7 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
       rc = launch_conv_tc(0, F, g.H, g.W, g.Cin, g.Cout, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (const bf16*)skip, nullptr,
                           (bf16*)ws.act[L.out_t], L.relu_in, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
-      rc = launch_dense_fwd_tc(g, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.wf + L.wf_off, bias, (bf16*)ws.act[L.out_t], L.relu_in, ws.errflag, st);
+      rc = launch_dense_fwd_tc(g, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.wf + L.wf_off, bias, (bf16*)ws.act[L.out_t], L.relu_in, ws.partial, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(g)) {
       rc = launch_conv0_fwd(g, F, obs, frame_idx, ws.w0img, bias, (bf16*)ws.act[L.out_t], ws.errflag, st);
     } else if (L.u8_in) {
@@ -239,9 +269,9 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
   return CB_OK;
 }
 
-int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st) {
+int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads) {
   Workspace& ws = net->ws[prec];
-  return prec == CB_PREC_FP32_REF ? forward_t<float>(net, ws, obs, frame_idx, F, st) : forward_t<bf16>(net, ws, obs, frame_idx, F, st);
+  return prec == CB_PREC_FP32_REF ? forward_t<float>(net, ws, obs, frame_idx, F, st, skip_heads) : forward_t<bf16>(net, ws, obs, frame_idx, F, st, skip_heads);
 }
 
 template <typename AT>

@@ -5,6 +5,8 @@
 
 namespace cb {
 
+constexpr int MAX_A = 32;      // n_actions + 1 must not exceed this
+
 // ------------------------------------------------------------------------------------------------
 // A9: Philox4x32-10 counter-based generator (Salmon et al. 2011), 10 rounds.
 // ------------------------------------------------------------------------------------------------
@@ -76,6 +78,75 @@ int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint
   return CB_OK;
 }
 
+// Actor-side head epilogue in ONE kernel: one warp per env computes the A logits and the value
+// from relu(hidden) (lanes stride over the hidden units, fixed shuffle tree), writes them, and draws the action:
+// lane i < A forms logit_i + Gumbel_i, the warp takes the arg-max with the lowest index on ties (O3 / A9).
+template <typename AT>
+__global__ void heads_sample_kernel(const AT* __restrict__ hid, const AT* __restrict__ wf, const float* __restrict__ bias, int B, int fc, int A,
+                                    uint32_t k0, uint32_t k1, uint32_t step_lo, uint32_t step_hi, uint32_t env_offset,
+                                    float* __restrict__ head, float* __restrict__ logits, float* __restrict__ value, int32_t* __restrict__ actions) {
+  const int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (b >= B) return;
+  const int N = A + 1;
+  float acc[MAX_A];
+#pragma unroll
+  for (int n = 0; n < MAX_A; ++n) acc[n] = 0.f;
+  for (int k = lane; k < fc; k += 32) {
+    float h;
+    if (sizeof(AT) == 2) h = __bfloat162float(reinterpret_cast<const bf16*>(hid)[(size_t)b * fc + k]); else h = reinterpret_cast<const float*>(hid)[(size_t)b * fc + k];
+    h = fmaxf(h, 0.f);
+#pragma unroll
+    for (int n = 0; n < MAX_A; ++n) if (n < N) {
+      float w;
+      if (sizeof(AT) == 2) w = __bfloat162float(reinterpret_cast<const bf16*>(wf)[(size_t)k * N + n]); else w = reinterpret_cast<const float*>(wf)[(size_t)k * N + n];
+      acc[n] = fmaf(h, w, acc[n]);
+    }
+  }
+  float mine = 0.f;      // lane n ends up holding output n
+#pragma unroll
+  for (int n = 0; n < MAX_A; ++n) if (n < N) {
+    float v = acc[n];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == n) mine = v + bias[n];
+  }
+  if (lane < N) {
+    if (head) head[(size_t)b * N + lane] = mine;
+    if (lane < A) { if (logits) logits[(size_t)b * A + lane] = mine; } else if (value) value[b] = mine;
+  }
+  if (actions) {
+    float sc = -INFINITY;
+    if (lane < A) {
+      uint32_t r[4];
+      philox4x32_10(env_offset + (uint32_t)b, step_lo, step_hi, (uint32_t)(lane >> 2), k0, k1, r);
+      sc = __fadd_rn(mine, gumbel_from_u32(r[lane & 3]));
+    }
+    int best = lane;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      float os = __shfl_xor_sync(0xffffffffu, sc, o); int ob = __shfl_xor_sync(0xffffffffu, best, o);
+      if (os > sc || (os == sc && ob < best)) { sc = os; best = ob; }
+    }
+    if (lane == 0) actions[b] = best;
+  }
+}
+
+int launch_heads_sample(int prec, const void* hid, const void* wf, const float* bias, int B, int fc, int A, uint64_t seed, uint64_t step,
+                        uint32_t env_offset, float* head, float* logits, float* value, int32_t* actions, cudaStream_t st) {
+  if (B <= 0) return CB_OK;
+  if (A + 1 > MAX_A) { set_error("n_actions too large"); return CB_EINVAL; }
+  ProfScope ps(K_SAMPLE, st);
+  const int grid = (B * 32 + 127) / 128;
+  if (prec == CB_PREC_FP32_REF)
+    heads_sample_kernel<float><<<grid, 128, 0, st>>>((const float*)hid, (const float*)wf, bias, B, fc, A, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step,
+                                                      (uint32_t)(step >> 32), env_offset, head, logits, value, actions);
+  else
+    heads_sample_kernel<bf16><<<grid, 128, 0, st>>>((const bf16*)hid, (const bf16*)wf, bias, B, fc, A, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step,
+                                                     (uint32_t)(step >> 32), env_offset, head, logits, value, actions);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
 __global__ void split_head_kernel(const float* __restrict__ head, int F, int A, float* __restrict__ logits, float* __restrict__ value) {
   size_t total = (size_t)F * (A + 1);
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
@@ -101,7 +172,6 @@ template <typename R> __device__ __forceinline__ R rlog(R x);
 template <> __device__ __forceinline__ float rlog<float>(float x) { return logf(x); }
 template <> __device__ __forceinline__ double rlog<double>(double x) { return log(x); }
 
-constexpr int MAX_A = 32;
 
 template <typename R>
 __device__ __forceinline__ void log_softmax(const float* l, int A, R* lp, R* H) {
