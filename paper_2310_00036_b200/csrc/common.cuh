@@ -133,6 +133,7 @@ int backward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx
 
 // conv_tc.cu
 bool conv_tc_supported(const Geom& g);
+bool conv_tc_fits(int H, int W, int cin, int cout);
 int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16* in, const bf16* w, const float* bias, const bf16* aux0,
                    const bf16* aux1, bf16* out, bool relu_in, int* error_flag, cudaStream_t st);
 
@@ -149,8 +150,8 @@ size_t conv0_wimg_elems(const Geom& g);
 int launch_conv0_pack(const Geom& g, const ParamMap& pm, const float* params, bf16* wimg, cudaStream_t st);
 int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* wimg, const float* bias, bf16* out,
                      int* error_flag, cudaStream_t st);
-int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, float* partial,
-                       float* grad, int* error_flag, cudaStream_t st);
+int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, const uint8_t* pool_arg,
+                       const bf16* dpool, float* partial, float* grad, int* error_flag, cudaStream_t st);
 
 // dense_tc.cu
 bool dense_tc_supported(const Geom& g);

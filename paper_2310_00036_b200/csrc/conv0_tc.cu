@@ -22,15 +22,16 @@ struct Args {
   const uint8_t* obs; const int32_t* frame_idx;   // [*, CIN, H, W] uint8, optional frame gather
   const bf16* w; const float* bias; bf16* out;     // forward: B image [6][2][COUT][8], bias [COUT], out [F,H,W,COUT]
   const bf16* dy; float* partial;                 // wgrad: dy [F,H,W,COUT], partial [grid][3][24][COUT]
+  const uint8_t* pool_arg; const bf16* dpool;     // wgrad, fused max-pool adjoint: dy is gathered from dpool [F,Ho,Wo,COUT] through pool_arg
   int F, H, W, CIN, R, nbands, npix_alloc, kext;
   int* error_flag;
 };
 
 // stage rows yb-1 .. yb+R of frame `fr` into the plane (all positions rewritten)
-__device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr, int yb, int tid) {
+__device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr, int yb, int tid, int nthr = 128) {
   const int Wp = a.W + 2, W4 = a.W / 4, rows = a.R + 2;
   const uint32_t ONE = 0x3F80u;
-  for (int i = tid; i < rows * W4; i += 128) {
+  for (int i = tid; i < rows * W4; i += nthr) {
     int lr = i / W4, x0 = (i - lr * W4) * 4, y = yb - 1 + lr;
     uint32_t px[4] = {0, 0, 0, 0};     // per channel: 4 pixels
     if ((unsigned)y < (unsigned)a.H)
@@ -44,10 +45,44 @@ __device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr
       *reinterpret_cast<uint4*>(xs + (size_t)(lr * Wp + x0 + 1 + k) * 16) = o;
     }
   }
-  for (int i = tid; i < rows * 2; i += 128) {       // halo columns
+  for (int i = tid; i < rows * 2; i += nthr) {       // halo columns
     int lr = i >> 1, xp = (i & 1) ? Wp - 1 : 0;
     *reinterpret_cast<uint4*>(xs + (size_t)(lr * Wp + xp) * 16) = make_uint4(0, 0, ONE, 0);
   }
+}
+
+// adjoint of the 3x3 stride-2 SAME max-pool, gather form, evaluated while staging dy: conv-output pixel (y,x)
+// receives dpool of every window (<= 4) whose stored arg-max position is this pixel (A11); sums in fp32, in
+// window order, then rounds to bf16 exactly like the stand-alone pool_bwd_v8_kernel.
+__device__ __forceinline__ uint4 pool_gather(const Args& a, int f, int y, int x, int ch, int cout) {
+  const int Ho = (a.H + 1) / 2, Wo = (a.W + 1) / 2;
+  int th = (Ho - 1) * 2 + 3 - a.H; if (th < 0) th = 0; const int ph = th / 2;
+  int tw = (Wo - 1) * 2 + 3 - a.W; if (tw < 0) tw = 0; const int pw = tw / 2;
+  float g[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) g[k] = 0.f;
+  int oy_lo = (y + ph - 2 + 1) / 2; if (y + ph - 2 < 0) oy_lo = 0;
+  int ox_lo = (x + pw - 2 + 1) / 2; if (x + pw - 2 < 0) ox_lo = 0;
+  const int oy_hi = min((y + ph) / 2, Ho - 1), ox_hi = min((x + pw) / 2, Wo - 1);
+  for (int oy = oy_lo; oy <= oy_hi; ++oy)
+    for (int ox = ox_lo; ox <= ox_hi; ++ox) {
+      const uint32_t me = (uint32_t)((y - (oy * 2 - ph)) * 3 + (x - (ox * 2 - pw)));
+      const size_t o = (((size_t)f * Ho + oy) * Wo + ox) * cout + ch * 8;
+      const uint2 pk = *reinterpret_cast<const uint2*>(a.pool_arg + o);
+      const uint4 dv = *reinterpret_cast<const uint4*>(a.dpool + o);
+      const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&dv);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const float2 t = __bfloat1622float2(h[k]);
+        const uint32_t w = k < 2 ? pk.x : pk.y; const int sh = (k & 1) * 16;
+        if (((w >> sh) & 255u) == me) g[2 * k] += t.x;
+        if (((w >> (sh + 8)) & 255u) == me) g[2 * k + 1] += t.y;
+      }
+    }
+  uint4 r; __nv_bfloat162* o2 = reinterpret_cast<__nv_bfloat162*>(&r);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) o2[k] = __floats2bfloat162_rn(g[2 * k], g[2 * k + 1]);
+  return r;
 }
 
 constexpr int TMEM_COLS = 256;
@@ -124,40 +159,85 @@ __global__ void __launch_bounds__(128) conv0_fwd_kernel(const Args a) {
   if (warp == 0) tmem_dealloc(tmem_base, TMEM_COLS);
 }
 
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
+}
+
+constexpr int WNLOAD = 256;     // warps 0-7 stage (warps 0-1 later drain TMEM); warp 8: one thread issues the MMAs
+
+// Two stages of (X plane, DY planes): the loaders fill one while the tensor core reads the other.  UMMA M = 64:
+// accumulator row r = 8*dj + c sits in TMEM lane 32*(r/16) + r%16.
 template <int COUT>
-__global__ void __launch_bounds__(128) conv0_wgrad_kernel(const Args a) {
+__global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr int YCH = COUT / 8;
   constexpr uint32_t TCOLS = 128;
-  __shared__ __align__(8) uint64_t bar_storage;
+  __shared__ __align__(8) uint64_t bars[5];       // full[2], empty[2], done
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5, Wp = a.W + 2;
-  const uint32_t P = (uint32_t)a.npix_alloc * 16u;
-  uint8_t* xs = smem; uint8_t* ys = smem + P;
-  const uint32_t bar = smem_u32(&bar_storage);
-  if (tid == 0) mbar_init(bar, 1);
-  if (warp == 0) tmem_alloc(smem_u32(&tmem_base_smem), TCOLS);
-  for (int i = tid; i < a.npix_alloc; i += 128) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
-  for (uint32_t i = tid; i < P * YCH / 16; i += 128) reinterpret_cast<uint4*>(ys)[i] = make_uint4(0, 0, 0, 0);
+  const uint32_t P = (uint32_t)a.npix_alloc * 16u, STAGE = (1u + YCH) * P;
+  const uint32_t bar0 = smem_u32(&bars[0]);
+  if (tid == 0) {
+    for (int i = 0; i < 5; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  if (warp == WNLOAD / 32) tmem_alloc(smem_u32(&tmem_base_smem), TCOLS);
+  for (int st = 0; st < 2; ++st) {
+    uint8_t* xs = smem + (size_t)st * STAGE;
+    for (int i = tid; i < a.npix_alloc; i += WNLOAD + 32) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
+    for (uint32_t i = tid; i < P * YCH / 16; i += WNLOAD + 32) reinterpret_cast<uint4*>(xs + P)[i] = make_uint4(0, 0, 0, 0);
+  }
+  fence_async_smem();
   tc_fence_before(); __syncthreads(); tc_fence_after();
-  const uint32_t tmem_base = tmem_base_smem, idesc = make_idesc(128, COUT, 1, 1);
-  const uint32_t x_base = smem_u32(xs), y_base = smem_u32(ys);
-  uint32_t parity = 0, accumulate = 0;
+  const uint32_t tmem_base = tmem_base_smem;
   const int nitems = a.F * a.nbands;
-  for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-    const int f = item / a.nbands, yb = (item - f * a.nbands) * a.R;
-    const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
-    stage_band(a, xs, fr, yb, tid);
-    for (int i = tid; i < a.kext * YCH; i += 128) {
-      int ch = i % YCH, pos = i / YCH, yl = pos / Wp, x = pos - yl * Wp, y = yb + yl;
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (yl < a.R && y < a.H && x < a.W) v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)f * a.H + y) * a.W + x) * COUT + ch * 8);
-      *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
+  const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+  if (warp < WNLOAD / 32) {
+    for (int it = 0; it < my_items; ++it) {
+      const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
+      if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 4; }
+      uint8_t* xs = smem + (size_t)s * STAGE; uint8_t* ys = xs + P;
+      const int f = item / a.nbands, yb = (item - f * a.nbands) * a.R;
+      const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
+      stage_band(a, xs, fr, yb, tid, WNLOAD);
+      for (int i = tid; i < a.kext * YCH; i += WNLOAD) {
+        int ch = i % YCH, pos = i / YCH, yl = pos / Wp, x = pos - yl * Wp, y = yb + yl;
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (yl < a.R && y < a.H && x < a.W) {
+          if (a.pool_arg == nullptr) v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)f * a.H + y) * a.W + x) * COUT + ch * 8);
+          else v = pool_gather(a, f, y, x, ch, COUT);
+        }
+        *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
+      }
+      fence_async_smem();
+      asm volatile("bar.sync 1, %0;\n" :: "n"(WNLOAD) : "memory");
+      if (tid == 0) mbar_arrive(bar0 + 8u * s);
     }
-    fence_async_smem();
-    __syncthreads();
-    if (tid == 0) {
+    if (warp < 2) {
+      if (my_items > 0 && !mbar_wait(bar0 + 8u * 4, 0u)) { if (a.error_flag) *a.error_flag = 4; }
       tc_fence_after();
+      float* out = a.partial + (size_t)blockIdx.x * 3 * 24 * COUT;
+      const int lane = tid & 31, row = lane < 16 ? warp * 16 + lane : 1 << 20;
+      for (int di = 0; di < 3; ++di) {
+#pragma unroll
+        for (int c0 = 0; c0 < COUT; c0 += 16) {
+          float v[16];
+          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(di * COUT + c0), v);
+          if (row < 24) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i) out[((size_t)di * 24 + row) * COUT + c0 + i] = v[i];
+          }
+        }
+      }
+    }
+  } else if (tid == WNLOAD) {
+    const uint32_t idesc = make_idesc(64, COUT, 1, 1);
+    uint32_t accumulate = 0;
+    for (int it = 0; it < my_items; ++it) {
+      const int s = it & 1, use = it >> 1;
+      if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 4; }
+      tc_fence_after();
+      const uint32_t x_base = smem_u32(smem + (size_t)s * STAGE), y_base = x_base + P;
       for (int k0 = 0; k0 < a.kext; k0 += 16) {
         const uint64_t bd = make_desc(y_base + (uint32_t)k0 * 16u, 128u, P);
 #pragma unroll
@@ -167,29 +247,12 @@ __global__ void __launch_bounds__(128) conv0_wgrad_kernel(const Args a) {
         }
         accumulate = 1;
       }
-      mma_commit(bar);
+      mma_commit(bar0 + 8u * (2 + s));
     }
-    if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 4; }
-    parity ^= 1;
-    tc_fence_after();
-    __syncthreads();
-  }
-  float* out = a.partial + (size_t)blockIdx.x * 3 * 24 * COUT;
-  if (warp == 0) {
-    for (int di = 0; di < 3; ++di) {
-#pragma unroll
-      for (int c0 = 0; c0 < COUT; c0 += 16) {
-        float v[16];
-        tmem_ld16(tmem_base + (uint32_t)(di * COUT + c0), v);
-        if (tid < 24) {
-#pragma unroll
-          for (int i = 0; i < 16; ++i) out[((size_t)di * 24 + tid) * COUT + c0 + i] = v[i];
-        }
-      }
-    }
+    mma_commit(bar0 + 8u * 4);
   }
   tc_fence_before(); __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem_base, TCOLS);
+  if (warp == WNLOAD / 32) tmem_dealloc(tmem_base, TCOLS);
 }
 
 // forward B image: slot = 2*di + h; h = 0: chunks (di,0),(di,1); h = 1: chunks (di,2), zero.  [slot][chunk][o][8]
@@ -219,7 +282,7 @@ __global__ void conv0_wgrad_reduce_kernel(const float* __restrict__ partial, int
 bool conv0_tc_supported(const Geom& g) {
   return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && g.Cin <= 4 && (g.Cout == 16 || g.Cout == 32) && g.W % 4 == 0 && g.W >= 8 && g.H == g.Ho && g.W == g.Wo;
 }
-constexpr int CONV0_MAX_CTAS = 296;
+constexpr int CONV0_MAX_CTAS = 148;
 size_t conv0_partial_elems(const Geom& g) { return (size_t)CONV0_MAX_CTAS * 3 * 24 * g.Cout; }
 size_t conv0_wimg_elems(const Geom& g) { return (size_t)6 * 2 * g.Cout * 8; }
 
@@ -243,7 +306,7 @@ int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* fr
   const int nb = (g.H + R - 1) / R; R = (g.H + nb - 1) / nb;
   const int npix = ((R * Wp + 127) / 128) * 128 + 2 * Wp + 8;
   const size_t smem = (size_t)6 * 2 * g.Cout * 16 + (size_t)npix * 16;
-  tc0::Args a{obs, frame_idx, wimg, bias, out, nullptr, nullptr, F, g.H, g.W, g.Cin, R, nb, npix, 0, error_flag};
+  tc0::Args a{obs, frame_idx, wimg, bias, out, nullptr, nullptr, nullptr, nullptr, F, g.H, g.W, g.Cin, R, nb, npix, 0, error_flag};
   const int grid = std::min(F * nb, 296);
   static size_t c16 = 0, c32 = 0; int rc;
   if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_fwd_kernel<16>, smem, &c16))) return rc; tc0::conv0_fwd_kernel<16><<<grid, 128, smem, st>>>(a); }
@@ -252,21 +315,21 @@ int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* fr
   return CB_OK;
 }
 
-int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, float* partial,
-                       float* grad, int* error_flag, cudaStream_t st) {
+int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, const uint8_t* pool_arg,
+                       const bf16* dpool, float* partial, float* grad, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
   const int Wp = g.W + 2, ych = g.Cout / 8;
-  const int maxpos = (int)(96 * 1024 / 16 / (1 + ych));
+  const int maxpos = (int)(100 * 1024 / 16 / (1 + ych));      // two stages of (1 + ych) planes in <= 200 KB
   int R = std::min(g.H, (maxpos - 2 * Wp - 48) / Wp); if (R < 1) R = 1;
   const int nb = (g.H + R - 1) / R; R = (g.H + nb - 1) / nb;
   const int kext = (R * Wp + 15) / 16 * 16;
   const int npix = (kext + 2 * Wp + 40 + 7) / 8 * 8;
-  const size_t smem = (size_t)(1 + ych) * npix * 16;
+  const size_t smem = (size_t)2 * (1 + ych) * npix * 16;
   const int grid = std::min(F * nb, CONV0_MAX_CTAS);
-  tc0::Args a{obs, frame_idx, nullptr, nullptr, nullptr, dy, partial, F, g.H, g.W, g.Cin, R, nb, npix, kext, error_flag};
+  tc0::Args a{obs, frame_idx, nullptr, nullptr, nullptr, dy, partial, pool_arg, dpool, F, g.H, g.W, g.Cin, R, nb, npix, kext, error_flag};
   static size_t c16 = 0, c32 = 0; int rc;
-  if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_wgrad_kernel<16>, smem, &c16))) return rc; tc0::conv0_wgrad_kernel<16><<<grid, 128, smem, st>>>(a); }
-  else { if ((rc = set_smem(tc0::conv0_wgrad_kernel<32>, smem, &c32))) return rc; tc0::conv0_wgrad_kernel<32><<<grid, 128, smem, st>>>(a); }
+  if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_wgrad_kernel<16>, smem, &c16))) return rc; tc0::conv0_wgrad_kernel<16><<<grid, tc0::WNLOAD + 32, smem, st>>>(a); }
+  else { if ((rc = set_smem(tc0::conv0_wgrad_kernel<32>, smem, &c32))) return rc; tc0::conv0_wgrad_kernel<32><<<grid, tc0::WNLOAD + 32, smem, st>>>(a); }
   CB_CUDA(cudaGetLastError());
   tc0::conv0_wgrad_reduce_kernel<<<(3 * 24 * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, grad);
   CB_CUDA(cudaGetLastError());

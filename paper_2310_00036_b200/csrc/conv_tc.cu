@@ -249,6 +249,9 @@ static TcPlan tc_plan(int H, int W, int cin, int cout) {
   return {G, npix, wbytes + (size_t)npix * cin * 2};
 }
 
+// the staged frame group (with halo) plus the weight image must fit one CTA's shared memory
+bool conv_tc_fits(int H, int W, int cin, int cout) { return tc_plan(H, W, cin, cout).smem <= 220 * 1024; }
+
 template <int CIN, int COUT, int MODE>
 static int launch_one(const tc::ConvTcArgs& a, size_t smem, int ngroups, cudaStream_t st) {
   static size_t configured = 0;      // largest dynamic size this instantiation has been opted in for

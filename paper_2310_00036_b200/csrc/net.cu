@@ -247,7 +247,7 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
     ProfScope ps(K_CONV_FWD, st, 1, 2.0 * M * N * K, in_bytes + (double)M * N * (L.f32_out ? 4 : sizeof(AT)) * (skip ? 2 : 1) + (double)K * N * sizeof(AT));
     int rc;
-    if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out) {
+    if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out && conv_tc_fits(g.H, g.W, g.Cin, g.Cout)) {
       rc = launch_conv_tc(0, F, g.H, g.W, g.Cin, g.Cout, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (const bf16*)skip, nullptr,
                           (bf16*)ws.act[L.out_t], L.relu_in, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
@@ -276,8 +276,14 @@ int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx,
 
 template <typename AT>
 static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, float* grad, cudaStream_t st) {
-  for (const Op& op : net->bwd) {
+  const Op* fused_pool = nullptr;      // a max-pool adjoint folded into the next (first-layer) weight gradient
+  for (size_t oi = 0; oi < net->bwd.size(); ++oi) {
+    const Op& op = net->bwd[oi];
     if (op.kind == OP_POOLBWD) {
+      if (std::is_same<AT, bf16>::value && op.C % 8 == 0 && oi + 1 < net->bwd.size() && net->bwd[oi + 1].kind == OP_WGRAD) {
+        const Layer& NL = net->layers[net->bwd[oi + 1].layer];
+        if (NL.u8_in && conv0_tc_supported(NL.g)) { fused_pool = &op; continue; }      // its only consumer gathers through the arg-max itself
+      }
       size_t total = (size_t)F * op.H * op.W * op.C;
       ProfScope ps(K_POOL_BWD, st, 1, 0.0, (double)sizeof(AT) * (2.0 * total + (double)F * pool_out(op.H) * pool_out(op.W) * op.C));
       if (std::is_same<AT, bf16>::value && op.C % 8 == 0)
@@ -305,7 +311,10 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
       }
       if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(g)) {
         ProfScope ps(K_CONV_WGRAD, st, 2, 2.0 * 9 * g.Cin * g.Cout * (double)F * g.Ho * g.Wo, (double)F * g.H * g.W * (g.Cin + 2.0 * g.Cout));
-        int rc = launch_conv0_wgrad(g, L.pm, F, obs, frame_idx, (const bf16*)ws.grad[op.dy], ws.partial, grad, ws.errflag, st);
+        int rc = launch_conv0_wgrad(g, L.pm, F, obs, frame_idx, (const bf16*)ws.grad[op.dy],
+                                    fused_pool ? (const uint8_t*)ws.act[fused_pool->mask_t] : nullptr, fused_pool ? (const bf16*)ws.grad[fused_pool->dy] : nullptr,
+                                    ws.partial, grad, ws.errflag, st);
+        fused_pool = nullptr;
         if (rc) return rc;
         continue;
       }
@@ -332,7 +341,7 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
       // useful MACs of dgrad = those of the forward layer (stride > 1 makes most gathered taps empty)
       ProfScope ps(K_CONV_DGRAD, st, 1, 2.0 * F * g.Ho * g.Wo * (double)g.Cout * g.kh * g.kw * g.Cin,
                    (double)sizeof(AT) * ((double)F * g.Ho * g.Wo * g.Cout + (double)M * N * (1 + (op.mask_t >= 0) + (op.add >= 0)) + (double)K * N));
-      if (std::is_same<AT, bf16>::value && conv_tc_supported(g)) {
+      if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && conv_tc_fits(g.H, g.W, g.Cout, g.Cin)) {
         int rc = launch_conv_tc(1, F, g.H, g.W, g.Cout, g.Cin, (const bf16*)ws.grad[op.dy], ws.wtc_d + L.wf_off, nullptr,
                                 op.mask_t >= 0 ? (const bf16*)ws.act[op.mask_t] : nullptr, op.add >= 0 ? (const bf16*)ws.grad[op.add] : nullptr,
                                 (bf16*)ws.grad[op.dx], false, ws.errflag, st);

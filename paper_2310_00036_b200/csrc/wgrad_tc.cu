@@ -255,11 +255,12 @@ bool wgrad_tc_supported(const Geom& g) {
 constexpr int WGRAD_TC_MAX_CTAS = 148;
 size_t wgrad_tc_partial_elems(const Geom& g) { return (size_t)WGRAD_TC_MAX_CTAS * 9 * (g.Cin + 1) * g.Cout; }
 
-constexpr int WGRAD_UM = 64;      // UMMA M of the weight-gradient kernel (128 = known-good fallback)
+// 3-tap stacking needs 3*Cin+1 accumulator rows: UMMA M = 64 for Cin = 16, M = 128 for Cin = 32
+constexpr int wgrad_um(int cin) { return cin == 16 ? 64 : 128; }
 
 struct WPlan { int G, R, nbands, npix_alloc, kext, stage_planes; size_t smem; };
 static WPlan wgrad_plan(int H, int W, int cin, int cout) {
-  const int xpl = (cin == 16 ? 3 : 1) * (cin / 8);
+  const int xpl = 3 * (cin / 8), WGRAD_UM = wgrad_um(cin);
   const int Wp = W + 2, slack = 2 * Wp + 2;
   WPlan p;
   p.stage_planes = std::max(WGRAD_UM / 8, xpl + 1 + cout / 8);
@@ -281,10 +282,10 @@ template <int CIN, int COUT>
 static int launch_w(const tcw::WgradTcArgs& a, size_t smem, int grid, cudaStream_t st) {
   static size_t configured = 0;
   if (smem > configured) {
-    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT, WGRAD_UM, CIN == 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
-  tcw::wgrad3x3_tc_kernel<CIN, COUT, WGRAD_UM, CIN == 16><<<grid, tcw::NLOAD + 32, smem, st>>>(a);
+  tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true><<<grid, tcw::NLOAD + 32, smem, st>>>(a);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
