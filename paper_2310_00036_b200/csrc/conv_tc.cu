@@ -14,6 +14,9 @@
 // (6-40% of the rows, the price of needing no im2col and no per-tap copies).
 // Weights: B operand [Cout x 16] per (tap, k-step), K-major canonical layout, staged once per CTA.
 #include "common.cuh"
+#include "tma.cuh"
+
+#include <cstring>
 
 namespace cb {
 
@@ -83,7 +86,7 @@ struct ConvTcArgs {
   const bf16* aux0;    // forward: skip tensor (added) | dgrad: pre-activation whose sign gates the result; nullable
   const bf16* aux1;    // dgrad: gradient added after gating; nullable
   bf16* out;           // [F, H, W, COUT]
-  int F, H, W, G, npix_alloc, relu_in;
+  int F, H, W, G, npix_alloc, relu_in, use_tma;
   int* error_flag;
 };
 
@@ -92,11 +95,12 @@ constexpr int NT = 256;            // two warpgroups: both stage operands; each 
 
 // MODE 0: out = acc + bias (+ aux0).   MODE 1: out = (aux0 ? (aux0 > 0 ? acc : 0) : acc) (+ aux1).
 template <int CIN, int COUT, int MODE>
-__global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a) {
+__global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, const __grid_constant__ CUtensorMap tmap) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr int NCH = CIN / 8, KSTEPS = CIN / 16, TILES_PER_BATCH = TMEM_COLS / COUT;
   constexpr uint32_t W_BYTES = 9u * CIN * COUT * 2u;
   __shared__ __align__(8) uint64_t bar_storage;
+  __shared__ __align__(8) uint64_t ldbar_storage;
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5, wg = warp >> 2, lane_row = tid & 127;
   const int Wp = a.W + 2, R = (a.H + 2) * Wp;
@@ -105,7 +109,8 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a) {
   const uint32_t plane_bytes = (uint32_t)a.npix_alloc * 16u;
   const uint32_t bar = smem_u32(&bar_storage);
 
-  if (tid == 0) mbar_init(bar, 1);
+  const uint32_t ldbar = smem_u32(&ldbar_storage);
+  if (tid == 0) { mbar_init(bar, 1); mbar_init(ldbar, 1); if (a.use_tma) tma::prefetch_map(&tmap); }
   if (warp == 0) tmem_alloc(smem_u32(&tmem_base_smem), TMEM_COLS);
   // weights (already in operand layout) and a zeroed input area (halo and slack stay zero for the whole kernel)
   for (uint32_t i = tid; i < W_BYTES / 16; i += NT) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w)[i];
@@ -116,12 +121,36 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a) {
   const uint32_t tmem_base = tmem_base_smem;
   const uint32_t idesc = make_idesc(128, COUT, 0, 0);
   const uint32_t a_base = smem_u32(in_smem), b_base = smem_u32(w_smem);
-  uint32_t parity = 0;
+  uint32_t parity = 0, ldparity = 0;
   const int ngroups = (a.F + a.G - 1) / a.G;
 
   for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
     const int f0 = grp * a.G, nf = min(a.G, a.F - f0);
     // ---- stage the group's frames: global NHWC -> planes, ReLU on the way in --------------------------
+    if (a.use_tma) {
+      // ---- TMA: one bulk tensor copy per 8-channel chunk lands the whole group, zero halo included (box starts at (-1,-1)) ----
+      const uint32_t bytes = (uint32_t)(a.G * R) * 16u;
+      if (tid == 0) {
+        tma::arrive_expect_tx(ldbar, bytes * NCH);
+#pragma unroll
+        for (int ch = 0; ch < NCH; ++ch) tma::load_4d(a_base + (uint32_t)ch * plane_bytes, &tmap, ch * 8, -1, -1, f0, ldbar);
+      }
+      if (!mbar_wait(ldbar, ldparity)) { if (a.error_flag) *a.error_flag = 6; }
+      ldparity ^= 1;
+      if (a.relu_in) {      // ReLU in place (generic proxy), made visible to the tensor core by the proxy fence below
+        const int n16 = a.G * R;
+        for (int i = tid; i < n16 * NCH; i += NT) {
+          const int ch = i / n16, pos = i - ch * n16;
+          uint4* p = reinterpret_cast<uint4*>(in_smem + (size_t)ch * plane_bytes + (size_t)pos * 16);
+          uint4 v = *p;
+          __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+          const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
+          *p = v;
+        }
+      }
+    } else {
     const int per_frame = a.H * a.W * NCH, nwork = a.G * per_frame;
     for (int i0 = tid; i0 < nwork; i0 += NT * 4) {       // 4 independent 16-byte loads in flight per thread
       uint4 v[4]; uint32_t dst[4];
@@ -148,6 +177,7 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a) {
         }
         *reinterpret_cast<uint4*>(in_smem + dst[u]) = v[u];
       }
+    }
     }
     fence_async_smem();
     __syncthreads();
@@ -253,21 +283,21 @@ static TcPlan tc_plan(int H, int W, int cin, int cout) {
 bool conv_tc_fits(int H, int W, int cin, int cout) { return tc_plan(H, W, cin, cout).smem <= 220 * 1024; }
 
 template <int CIN, int COUT, int MODE>
-static int launch_one(const tc::ConvTcArgs& a, size_t smem, int ngroups, cudaStream_t st) {
+static int launch_one(const tc::ConvTcArgs& a, const CUtensorMap& tmap, size_t smem, int ngroups, cudaStream_t st) {
   static size_t configured = 0;      // largest dynamic size this instantiation has been opted in for
   if (smem > configured) {
     CB_CUDA(cudaFuncSetAttribute(tc::conv3x3_tc_kernel<CIN, COUT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
   int grid = std::min(ngroups, 3 * 148);
-  tc::conv3x3_tc_kernel<CIN, COUT, MODE><<<grid, tc::NT, smem, st>>>(a);
+  tc::conv3x3_tc_kernel<CIN, COUT, MODE><<<grid, tc::NT, smem, st>>>(a, tmap);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
 
 template <int MODE>
-static int dispatch(int cin, int cout, const tc::ConvTcArgs& a, size_t smem, int ngroups, cudaStream_t st) {
-#define CB_TC_CASE(ci, co) if (cin == ci && cout == co) return launch_one<ci, co, MODE>(a, smem, ngroups, st);
+static int dispatch(int cin, int cout, const tc::ConvTcArgs& a, const CUtensorMap& tmap, size_t smem, int ngroups, cudaStream_t st) {
+#define CB_TC_CASE(ci, co) if (cin == ci && cout == co) return launch_one<ci, co, MODE>(a, tmap, smem, ngroups, st);
   CB_TC_CASE(16, 16) CB_TC_CASE(16, 32) CB_TC_CASE(32, 16) CB_TC_CASE(32, 32) CB_TC_CASE(32, 64) CB_TC_CASE(64, 32) CB_TC_CASE(64, 64)
   CB_TC_CASE(16, 64) CB_TC_CASE(64, 16)
 #undef CB_TC_CASE
@@ -281,9 +311,11 @@ int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16*
   if (F <= 0) return CB_OK;
   TcPlan p = tc_plan(H, W, cin, cout);
   if (p.smem > 220 * 1024) { set_error("conv_tc: frame does not fit shared memory"); return CB_EINVAL; }
-  tc::ConvTcArgs a{in, w, bias, aux0, aux1, out, F, H, W, p.G, p.npix_alloc, relu_in ? 1 : 0, error_flag};
+  CUtensorMap tmap; memset(&tmap, 0, sizeof tmap);
+  const bool use_tma = W + 2 <= 256 && H + 2 <= 256 && tma::make_nhwc_map(&tmap, in, F, H, W, cin, W + 2, H + 2, p.G);
+  tc::ConvTcArgs a{in, w, bias, aux0, aux1, out, F, H, W, p.G, p.npix_alloc, relu_in ? 1 : 0, use_tma ? 1 : 0, error_flag};
   int ngroups = (F + p.G - 1) / p.G;
-  return mode == 0 ? dispatch<0>(cin, cout, a, p.smem, ngroups, st) : dispatch<1>(cin, cout, a, p.smem, ngroups, st);
+  return mode == 0 ? dispatch<0>(cin, cout, a, tmap, p.smem, ngroups, st) : dispatch<1>(cin, cout, a, tmap, p.smem, ngroups, st);
 }
 
 }  // namespace cb
