@@ -16,6 +16,9 @@
 // writes ONE fp32 partial [9][Cin+1][Cout] at the end; a second kernel adds the partials in CTA order,
 // so the result is bitwise reproducible (no atomics; the item -> CTA map depends on the shape only).
 #include "common.cuh"
+#include "tma.cuh"
+
+#include <cstring>
 
 namespace cb {
 namespace tcw {
@@ -59,7 +62,7 @@ struct WgradTcArgs {
   const bf16* x;      // [F, H, W, CIN]  layer input (pre-activation when relu_in)
   const bf16* dy;     // [F, H, W, COUT]
   float* partial;     // [gridDim.x][9][CIN+1][COUT]
-  int F, H, W, G, R, nbands, npix_alloc, kext, relu_in, stage_planes;
+  int F, H, W, G, R, nbands, npix_alloc, kext, relu_in, stage_planes, use_tma, dy_rows;
   int* error_flag;
 };
 
@@ -75,13 +78,13 @@ constexpr int NLOAD = 256;       // warps 0-7: stage operands (warps 0-3 later r
 // (dj, chunk); the M walk of ONE MMA then covers the three taps (di, 0..2) at rows dj*CIN + c -- 3 instead of 9
 // MMAs per 16 positions, and 49 instead of 17 useful rows of 64.
 template <int CIN, int COUT, int UM, bool ST3>
-__global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcArgs a) {
+__global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcArgs a, const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap ymap) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr int XCH = CIN / 8, YCH = COUT / 8, XPL = ST3 ? 3 * XCH : XCH;      // X planes per stage
   constexpr int NACC = ST3 ? 3 : 9;
   constexpr uint32_t TCOLS = (NACC * COUT <= 128) ? 128u : ((NACC * COUT <= 256) ? 256u : 512u);
   static_assert(!ST3 || 3 * CIN + 1 <= UM, "3-tap stacking needs 3*CIN+1 rows");
-  __shared__ __align__(8) uint64_t bars[5];          // full[2], empty[2], done
+  __shared__ __align__(8) uint64_t bars[7];          // full[2], empty[2], done, raw[2] (TMA landed)
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5;
   const int Wp = a.W + 2, Rb = (a.R + 2) * Wp;          // positions per frame region of a band
@@ -90,7 +93,7 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
   // per stage: planes [0, XCH) X | XCH: ones (bias row) | [XCH+1, XCH+1+YCH) DY | padding planes (zeros)
   const uint32_t bar0 = smem_u32(&bars[0]);
   if (tid == 0) {
-    for (int i = 0; i < 5; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
+    for (int i = 0; i < 7; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   if (warp == NLOAD / 32) {
@@ -99,12 +102,12 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
   }
   // total allocation: the last stage's A descriptor may walk UM/8 planes from its start
   const uint32_t total_bytes = stage_bytes + (uint32_t)max(a.stage_planes, UM / 8) * P;
-  for (uint32_t i = tid; i < total_bytes / 16; i += NLOAD + 32) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
+  for (uint32_t i = tid; i < total_bytes / 16; i += NLOAD + 64) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
   __syncthreads();
   {
     const uint32_t one2 = 0x3F803F80u;    // two bf16 ones
     for (int st = 0; st < 2; ++st)
-      for (uint32_t i = tid; i < P / 16; i += NLOAD + 32) reinterpret_cast<uint4*>(smem + (size_t)st * stage_bytes + (size_t)XPL * P)[i] = make_uint4(one2, one2, one2, one2);
+      for (uint32_t i = tid; i < P / 16; i += NLOAD + 64) reinterpret_cast<uint4*>(smem + (size_t)st * stage_bytes + (size_t)XPL * P)[i] = make_uint4(one2, one2, one2, one2);
   }
   asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -118,11 +121,28 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
     // ================= loaders =================
     for (int it = 0; it < my_items; ++it) {
       const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
-      if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 2; }
+      if (!a.use_tma && use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 2; }
       uint8_t* xs = smem + (size_t)s * stage_bytes;
       uint8_t* ys = xs + (size_t)(XPL + 1) * P;
       const int grp = item / a.nbands, band = item - grp * a.nbands;
       const int f0 = grp * a.G, nf = min(a.G, a.F - f0), yb = band * a.R;
+      if (a.use_tma) {
+        // operands were landed by the TMA producer thread; only the ReLU (in place) is left to these warps
+        if (!mbar_wait(bar0 + 8u * (5 + s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 7; }
+        if (a.relu_in) {
+          const int n16 = a.G * Rb;
+          for (int i = tid; i < n16 * XPL; i += NLOAD) {
+            const int pl = i / n16, pos = i - pl * n16;
+            uint4* p = reinterpret_cast<uint4*>(xs + (size_t)pl * P + (size_t)pos * 16);
+            uint4 v = *p;
+            __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+            const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
+            *p = v;
+          }
+        }
+      } else {
       const int xn = a.G * Rb * XCH;
       for (int i0 = tid; i0 < xn; i0 += NLOAD * 4) {
         uint4 v[4]; uint32_t dst[4];
@@ -175,6 +195,7 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
 #pragma unroll
         for (int u = 0; u < 4; ++u) if (dst[u] != 0xFFFFFFFFu) *reinterpret_cast<uint4*>(ys + dst[u]) = v[u];
       }
+      }
       asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
       asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
       if (tid == 0) mbar_arrive(bar0 + 8u * s);
@@ -204,6 +225,24 @@ __global__ void __launch_bounds__(NLOAD + 32) wgrad3x3_tc_kernel(const WgradTcAr
         }
       }
     }
+    }
+  } else if (tid == NLOAD + 32) {
+    // ================= TMA producer: runs one stage ahead of the tensor core =================
+    if (a.use_tma) {
+      tma::prefetch_map(&xmap); tma::prefetch_map(&ymap);
+      const uint32_t xbytes = (uint32_t)(a.G * Rb) * 16u, ybytes = (uint32_t)(a.G * a.dy_rows * Wp) * 16u;
+      for (int it = 0; it < my_items; ++it) {
+        const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
+        if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 7; }
+        const int grp = item / a.nbands, band = item - grp * a.nbands, f0 = grp * a.G, yb = band * a.R;
+        const uint32_t xs = smem_u32(smem + (size_t)s * stage_bytes), ys = xs + (uint32_t)(XPL + 1) * P, rb = bar0 + 8u * (5 + s);
+        tma::arrive_expect_tx(rb, xbytes * XPL + ybytes * YCH);
+        for (int pl = 0; pl < XPL; ++pl) {       // plane (dj, ch): X shifted by dj positions = box started dj columns further right
+          const int dj = ST3 ? pl / XCH : 0, ch = ST3 ? pl % XCH : pl;
+          tma::load_4d(xs + (uint32_t)pl * P, &xmap, ch * 8, -1 + dj, yb - 1, f0, rb);
+        }
+        for (int ch = 0; ch < YCH; ++ch) tma::load_4d(ys + (uint32_t)ch * P, &ymap, ch * 8, 0, yb, f0, rb);
+      }
     }
   } else if (tid == NLOAD) {
     // ================= MMA issuer =================
@@ -279,13 +318,13 @@ static WPlan wgrad_plan(int H, int W, int cin, int cout) {
 }
 
 template <int CIN, int COUT>
-static int launch_w(const tcw::WgradTcArgs& a, size_t smem, int grid, cudaStream_t st) {
+static int launch_w(const tcw::WgradTcArgs& a, const CUtensorMap& xmap, const CUtensorMap& ymap, size_t smem, int grid, cudaStream_t st) {
   static size_t configured = 0;
   if (smem > configured) {
     CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     configured = smem;
   }
-  tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true><<<grid, tcw::NLOAD + 32, smem, st>>>(a);
+  tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true><<<grid, tcw::NLOAD + 64, smem, st>>>(a, xmap, ymap);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
@@ -297,12 +336,18 @@ int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, con
   if (p.smem > 224 * 1024) { set_error("wgrad_tc: plan does not fit shared memory"); return CB_EINVAL; }
   const int nitems = ((F + p.G - 1) / p.G) * p.nbands;
   const int grid = std::min(nitems, WGRAD_TC_MAX_CTAS);
-  tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, p.stage_planes, error_flag};
+  // TMA boxes: X [8][W+2][R+2][G] started at (-1+dj, yb-1); DY [8][W+2][rows][G] started at (0, yb) with rows = R for banded
+  // plans (G = 1: the rows below the band must stay zero) and R+2 = H+2 for whole frames (out-of-bounds rows are zero-filled)
+  const int dy_rows = p.nbands > 1 ? p.R : p.R + 2;
+  CUtensorMap xmap, ymap; memset(&xmap, 0, sizeof xmap); memset(&ymap, 0, sizeof ymap);
+  const bool use_tma = g.W + 2 <= 256 && p.R + 2 <= 256 && tma::make_nhwc_map(&xmap, x, F, g.H, g.W, g.Cin, g.W + 2, p.R + 2, p.G) &&
+                       tma::make_nhwc_map(&ymap, dy, F, g.H, g.W, g.Cout, g.W + 2, dy_rows, p.G);
+  tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, p.stage_planes, use_tma ? 1 : 0, dy_rows, error_flag};
   int rc;
-  if (g.Cin == 16 && g.Cout == 16) rc = launch_w<16, 16>(a, p.smem, grid, st);
-  else if (g.Cin == 16 && g.Cout == 32) rc = launch_w<16, 32>(a, p.smem, grid, st);
-  else if (g.Cin == 32 && g.Cout == 16) rc = launch_w<32, 16>(a, p.smem, grid, st);
-  else rc = launch_w<32, 32>(a, p.smem, grid, st);
+  if (g.Cin == 16 && g.Cout == 16) rc = launch_w<16, 16>(a, xmap, ymap, p.smem, grid, st);
+  else if (g.Cin == 16 && g.Cout == 32) rc = launch_w<16, 32>(a, xmap, ymap, p.smem, grid, st);
+  else if (g.Cin == 32 && g.Cout == 16) rc = launch_w<32, 16>(a, xmap, ymap, p.smem, grid, st);
+  else rc = launch_w<32, 32>(a, xmap, ymap, p.smem, grid, st);
   if (rc) return rc;
   tcw::wgrad_tc_reduce_kernel<<<(9 * (g.Cin + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, grad);
   CB_CUDA(cudaGetLastError());
