@@ -22,6 +22,8 @@
 //   GAE ......................... pinned: lambda=1 brute-force discounted return, lambda=0
 //   IMPALA / PPO losses ......... pinned: finite differences, ratio-1 invariants, sign tests
 //   clip + Adam ................. pinned: first-step closed form, constant-gradient closed form
+//   clip + RMSprop (A22) ........ pinned: first-step and constant-gradient closed forms, lr = 0
+//   env-split minibatches (A21) . pinned: mb = 1 identity, equality with per-group single steps run by hand
 //   permutation ................. pinned: bijection + brute-force reference of the index rule
 // =============================================================================================
 #include <cmath>
@@ -50,6 +52,8 @@ typedef struct {
   double vf_coef, ent_coef;                       // c1, c2
   double lr, beta1, beta2, adam_eps, max_grad_norm;
   int loss_reduction;                             // 0 mean, 1 sum (reading A4)
+  int optimizer;                                  // 0 Adam (A12), 1 RMSprop (Table 3; reading A22)
+  double rms_decay, rms_eps;                      // 0.99, 0.01
 } orc_hparams;
 
 enum { ORC_N_STATS = 8 };  // loss, pg_loss, v_loss, entropy, grad_norm, approx_kl, clip_frac, mean_rho
@@ -525,6 +529,21 @@ double clip_adam(size_t P, float* theta, float* m, float* v, const double* g, ui
   return n;
 }
 
+// Reading A22, RMSprop as the paper's IMPALA optimizer (Table 3: "RMSprop eps 0.01, decay 0.99"; the
+// paper's stack is optax): nu <- decay nu + (1-decay) g^2;  theta <- theta - lr g / sqrt(nu + eps)   (eps INSIDE the root,
+// nu_0 = 0, no momentum, no centering), after the same global-norm clip as O9.  nu lives in the adam_v buffer.
+double clip_rmsprop(size_t P, float* theta, float* nu, const double* g, double lr, double decay, double eps, double max_norm) {
+  double ss = 0.0; for (size_t i = 0; i < P; ++i) ss += g[i] * g[i];
+  double n = std::sqrt(ss), scale = max_norm / std::max(n, max_norm);
+  for (size_t i = 0; i < P; ++i) {
+    double gi = g[i] * scale;
+    double ni = decay * (double)nu[i] + (1.0 - decay) * gi * gi;
+    double th = (double)theta[i] - lr * gi / std::sqrt(ni + eps);
+    nu[i] = (float)ni; theta[i] = (float)th;
+  }
+  return n;
+}
+
 // forward over F frames -> double logits [F,A], values [F]
 void forward_many(const orc_arch& a, const Layout& L, const double* P, const uint8_t* obs, int F,
                   double* logits, double* values) {
@@ -626,6 +645,11 @@ void orc_ppo_loss(int m, int A, const double* logits, const double* V, const int
                   const double* logp_old, double eps, double c1, double c2, int norm_adv, double* stats, double* dlogits, double* dV) {
   ppo_loss(m, A, logits, V, act, adv, ret, logp_old, eps, c1, c2, norm_adv, stats, dlogits, dV);
 }
+double orc_clip_rmsprop(size_t P, float* theta, float* nu, const double* g, double lr, double decay, double eps, double max_norm) {
+  return clip_rmsprop(P, theta, nu, g, lr, decay, eps, max_norm);
+}
+// linear decay of the learning rate to 0 over `total` updates (Tables 2-3 "Anneal lr: linear"): lr_k = lr0 (1 - k/total)
+double orc_linear_lr(double lr0, uint64_t k, uint64_t total) { return total ? lr0 * (1.0 - (double)std::min(k, total) / (double)total) : lr0; }
 double orc_clip_adam(size_t P, float* theta, float* m, float* v, const double* g, uint64_t k, double lr, double b1, double b2,
                      double eps, double max_norm) { return clip_adam(P, theta, m, v, g, k, lr, b1, b2, eps, max_norm); }
 
@@ -687,20 +711,37 @@ int orc_learner_step(const orc_arch* a, const orc_hparams* hp, float* params, fl
   }
   vec G(P);
   if (hp->algo == 0) {
-    vec logpi(N), vs(N), pg(N), rho(N);
-    for (int n = 0; n < N; ++n) { log_softmax(&lg[(size_t)n * A], A, lp.data()); logpi[n] = lp[actions[n]]; }
-    vtrace(T, B, V.data(), r.data(), dones, logpi.data(), logmu.data(), hp->gamma, hp->lambda_, hp->rho_bar, hp->c_bar, hp->rho_pg_bar, vs.data(), pg.data(), rho.data());
-    if (out_t0) std::copy(vs.begin(), vs.end(), out_t0);
-    if (out_t1) std::copy(pg.begin(), pg.end(), out_t1);
-    double st[ORC_N_STATS]; vec dl((size_t)N * A), dV(N);
-    impala_loss(N, A, lg.data(), V.data(), actions, vs.data(), pg.data(), rho.data(), hp->vf_coef, hp->ent_coef, hp->loss_reduction, st, dl.data(), dV.data());
-    std::fill(G.begin(), G.end(), 0.0);
-    backward_many(*a, L, Pd.data(), obs, nullptr, N, dl.data(), dV.data(), G.data());   // bootstrap frames get no gradient
-    if (out_grad) std::copy(G.begin(), G.end(), out_grad);
-    *opt_step += 1;
-    st[4] = clip_adam(P, params, adam_m, adam_v, G.data(), *opt_step, hp->lr, hp->beta1, hp->beta2, hp->adam_eps, hp->max_grad_norm);
-    for (int i = 0; i < ORC_N_STATS; ++i) stats[i] = (float)st[i];
-    return 1;
+    // Reading A21 ("IMPALA ... 4 gradient updates per rollout", 401): the rollout is split by ENVIRONMENT into
+    // `minibatches` groups of B/mb whole trajectories; each group is one complete update (forward with the current parameters,
+    // V-trace, loss averaged over its T*B/mb samples, backward, clip, optimizer), applied in group order.  mb = 1 is the
+    // single full-batch step of BASELINE.json configs 0/2/4.
+    int mb = hp->minibatches < 1 ? 1 : hp->minibatches; int Bm = B / mb, Nm = T * Bm, Fm = (T + 1) * Bm;
+    size_t fs = (size_t)a->in_c * a->in_h * a->in_w;
+    for (int k = 0; k < mb; ++k) {
+      std::vector<int32_t> fidx(Fm), act_m(Nm); std::vector<uint8_t> d_m(Nm); vec r_m(Nm), lmu_m(Nm);
+      for (int t = 0; t <= T; ++t) for (int b = 0; b < Bm; ++b) fidx[(size_t)t * Bm + b] = t * B + k * Bm + b;
+      for (int t = 0; t < T; ++t) for (int b = 0; b < Bm; ++b) { size_t src = (size_t)t * B + k * Bm + b, dst = (size_t)t * Bm + b;
+        act_m[dst] = actions[src]; d_m[dst] = dones[src]; r_m[dst] = r[src]; lmu_m[dst] = logmu[src]; }
+      if (mb > 1 || k > 0) Pd.assign(params, params + P);
+      vec lgm((size_t)Fm * A), Vm(Fm);
+      if (mb == 1) { lgm = lg; Vm = V; }
+      else for (int f = 0; f < Fm; ++f) net_forward(*a, L, Pd.data(), obs + fs * fidx[f], &lgm[(size_t)f * A], &Vm[f], nullptr);
+      vec logpi(Nm), vs(Nm), pg(Nm), rho(Nm);
+      for (int n = 0; n < Nm; ++n) { log_softmax(&lgm[(size_t)n * A], A, lp.data()); logpi[n] = lp[act_m[n]]; }
+      vtrace(T, Bm, Vm.data(), r_m.data(), d_m.data(), logpi.data(), lmu_m.data(), hp->gamma, hp->lambda_, hp->rho_bar, hp->c_bar, hp->rho_pg_bar, vs.data(), pg.data(), rho.data());
+      if (out_t0 && mb == 1) std::copy(vs.begin(), vs.end(), out_t0);
+      if (out_t1 && mb == 1) std::copy(pg.begin(), pg.end(), out_t1);
+      double st[ORC_N_STATS]; vec dl((size_t)Nm * A), dV(Nm);
+      impala_loss(Nm, A, lgm.data(), Vm.data(), act_m.data(), vs.data(), pg.data(), rho.data(), hp->vf_coef, hp->ent_coef, hp->loss_reduction, st, dl.data(), dV.data());
+      std::fill(G.begin(), G.end(), 0.0);
+      backward_many(*a, L, Pd.data(), obs, fidx.data(), Nm, dl.data(), dV.data(), G.data());   // bootstrap frames get no gradient
+      if (out_grad) std::copy(G.begin(), G.end(), out_grad);
+      *opt_step += 1;
+      if (hp->optimizer == 1) st[4] = clip_rmsprop(P, params, adam_v, G.data(), hp->lr, hp->rms_decay, hp->rms_eps, hp->max_grad_norm);
+      else st[4] = clip_adam(P, params, adam_m, adam_v, G.data(), *opt_step, hp->lr, hp->beta1, hp->beta2, hp->adam_eps, hp->max_grad_norm);
+      for (int i = 0; i < ORC_N_STATS; ++i) stats[(size_t)k * ORC_N_STATS + i] = (float)st[i];
+    }
+    return mb;
   }
   // PPO (Alg. 1 l.11-20)
   vec adv(N), ret(N);

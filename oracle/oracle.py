@@ -38,7 +38,8 @@ class HParams(C.Structure):
                 ("perm_seed", C.c_uint64),
                 ("vf_coef", C.c_double), ("ent_coef", C.c_double),
                 ("lr", C.c_double), ("beta1", C.c_double), ("beta2", C.c_double), ("adam_eps", C.c_double),
-                ("max_grad_norm", C.c_double), ("loss_reduction", C.c_int)]
+                ("max_grad_norm", C.c_double), ("loss_reduction", C.c_int),
+                ("optimizer", C.c_int), ("rms_decay", C.c_double), ("rms_eps", C.c_double)]
 
 
 def make_arch(kind, channels, fc, n_actions=18, in_c=4, in_h=84, in_w=84):
@@ -55,7 +56,8 @@ def make_hparams(algo="impala", T=20, B=128, **kw):
     h.algo = 1 if ppo else 0; h.T = T; h.B = B
     h.gamma = 0.99; h.lambda_ = 0.95 if ppo else 1.0
     h.rho_bar = h.c_bar = h.rho_pg_bar = 1.0
-    h.clip_eps = 0.1; h.epochs = 4; h.minibatches = 4; h.norm_adv = 1; h.perm_seed = 1
+    h.clip_eps = 0.1; h.epochs = 4; h.minibatches = 4 if ppo else 1; h.norm_adv = 1; h.perm_seed = 1
+    h.optimizer = 0; h.rms_decay = 0.99; h.rms_eps = 0.01          # Table 3; optimizer 1 = RMSprop (A22)
     h.vf_coef = 0.5; h.ent_coef = 0.01
     h.lr = 2.5e-4 if ppo else 6e-4; h.beta1 = 0.9; h.beta2 = 0.999; h.adam_eps = 1e-5
     h.max_grad_norm = 0.5 if ppo else 40.0; h.loss_reduction = 0
@@ -77,6 +79,8 @@ def lib():
         _lib.orc_fixed_log.restype = C.c_double; _lib.orc_fixed_log.argtypes = [C.c_double]
         _lib.orc_gumbel_from_u32.restype = C.c_float; _lib.orc_gumbel_from_u32.argtypes = [C.c_uint32]
         _lib.orc_clip_adam.restype = C.c_double
+        _lib.orc_clip_rmsprop.restype = C.c_double
+        _lib.orc_linear_lr.restype = C.c_double
         _lib.orc_impala_objective_f64.restype = C.c_double
         _lib.orc_ppo_objective_f64.restype = C.c_double
     return _lib
@@ -235,6 +239,17 @@ def clip_adam(theta, m, v, g, k, lr, b1=0.9, b2=0.999, eps=1e-5, max_norm=40.0):
     return theta, m, v, float(n)
 
 
+def clip_rmsprop(theta, nu, g, lr, decay=0.99, eps=0.01, max_norm=40.0):
+    """A22.  Returns (theta', nu', pre-clip norm); inputs untouched."""
+    theta = _c(theta, np.float32).copy(); nu = _c(nu, np.float32).copy(); g = _c(g, np.float64)
+    n = lib().orc_clip_rmsprop(C.c_size_t(theta.size), _p(theta), _p(nu), _p(g), C.c_double(lr), C.c_double(decay), C.c_double(eps), C.c_double(max_norm))
+    return theta, nu, float(n)
+
+
+def linear_lr(lr0, k, total):
+    return float(lib().orc_linear_lr(C.c_double(lr0), C.c_uint64(k), C.c_uint64(total)))
+
+
 def impala_objective_f64(arch, hp, params64, params_tgt64, obs, actions, rewards, dones, behaviour_logits, want_grad=False):
     params64 = _c(params64, np.float64); params_tgt64 = _c(params_tgt64, np.float64)
     obs = _c(obs, np.uint8); actions = _c(actions, np.int32); rewards = _c(rewards, np.float32)
@@ -261,7 +276,7 @@ def learner_step(arch, hp, params, adam_m, adam_v, opt_step, obs, actions, rewar
     obs = _c(obs, np.uint8); actions = _c(actions, np.int32); rewards = _c(rewards, np.float32)
     dones = _c(dones, np.uint8); bl = _c(behaviour_logits, np.float32)
     assert obs.shape[0] == (T + 1) * B or obs.shape[:2] == (T + 1, B)
-    n_upd = 1 if hp.algo == 0 else hp.epochs * hp.minibatches
+    n_upd = max(1, hp.minibatches) if hp.algo == 0 else hp.epochs * hp.minibatches
     stats = np.zeros((n_upd, N_STATS), np.float32); step = C.c_uint64(opt_step)
     F, N = (T + 1) * B, T * B
     dbg = dict(logits=np.empty((F, A)), values=np.empty(F), t0=np.empty(N), t1=np.empty(N), grad=np.empty(params.size)) if debug else {}

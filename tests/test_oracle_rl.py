@@ -321,3 +321,60 @@ def test_data_parallel_gradient_identity():
         _, gi = O.impala_objective_f64(oa, hp2, p, p, obs[:, s], act[:, s], rew[:, s], dones[:, s], bl[:, s], want_grad=True)
         gs.append(gi)
     np.testing.assert_allclose(g_all, 0.5 * (gs[0] + gs[1]), rtol=1e-10, atol=1e-14)
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT row f1: RMSprop (A22), env-split IMPALA minibatches (A21), linear LR anneal
+# ---------------------------------------------------------------------------------------------------
+def test_rmsprop_first_step_and_constant_gradient_closed_forms():
+    g = synth.rng(5).standard_normal(300) * 0.01
+    th0 = np.zeros(300, np.float32) + 0.5
+    lr, d, eps = 6e-4, 0.99, 0.01
+    th, nu, n = O.clip_rmsprop(th0, np.zeros(300, np.float32), g, lr, d, eps, max_norm=40.0)
+    assert n == pytest.approx(np.linalg.norm(g), rel=1e-12)
+    np.testing.assert_allclose(th.astype(np.float64) - 0.5, -lr * g / np.sqrt((1 - d) * g * g + eps), rtol=0, atol=1e-7)
+    np.testing.assert_allclose(nu, (1 - d) * g * g, rtol=1e-6)
+    # constant gradient for k steps: nu_k = (1 - d^k) g^2
+    th, nu = th0, np.zeros(300, np.float32)
+    for k in range(1, 6):
+        th, nu, _ = O.clip_rmsprop(th, nu, g, lr, d, eps, 40.0)
+        np.testing.assert_allclose(nu, (1 - d ** k) * g * g, rtol=2e-6)
+    # lr = 0 leaves the parameters bit-identical; above the clip threshold the update ignores the gradient's scale
+    th_z, _, _ = O.clip_rmsprop(th0, np.zeros(300, np.float32), g, 0.0, d, eps, 40.0)
+    assert th_z.tobytes() == th0.tobytes()
+    a, _, _ = O.clip_rmsprop(th0, np.zeros(300, np.float32), g * 1e3, lr, d, eps, 0.5)
+    b, _, _ = O.clip_rmsprop(th0, np.zeros(300, np.float32), g * 1e4, lr, d, eps, 0.5)
+    np.testing.assert_allclose(a, b, rtol=0, atol=1e-7)
+
+
+def test_linear_lr_anneal():
+    # Tables 2-3 "linear decay to 0"
+    assert O.linear_lr(6e-4, 0, 100) == 6e-4 and O.linear_lr(6e-4, 100, 100) == 0.0
+    assert O.linear_lr(6e-4, 25, 100) == pytest.approx(4.5e-4, rel=1e-12) and O.linear_lr(6e-4, 500, 100) == 0.0
+
+
+def test_impala_env_split_minibatches_equal_sequential_single_steps():
+    """A21: mb env-groups = mb full learner steps on the groups, in order, with the parameters flowing."""
+    arch = synth.ArchSpec("impala", (3, 4, 5), 12, 5, 2, 20, 20)
+    oa = O.make_arch(arch.kind, arch.channels, arch.fc, arch.n_actions, arch.in_c, arch.in_h, arch.in_w)
+    T, B, mb = 3, 6, 3
+    rewards, dones = synth.gen_rewards_dones(T, B, 1)
+    obs = synth.gen_obs_uniform((T + 1) * B, 2, arch).reshape(T + 1, B, arch.in_c, arch.in_h, arch.in_w)
+    bl, act = synth.gen_behaviour(T, B, arch.n_actions, 3)
+    p0 = synth.gen_params(arch, 4, bias_scale=0.05); P = p0.size
+    for opt in (0, 1):
+        hp = O.make_hparams("impala", T, B, minibatches=mb, optimizer=opt)
+        out = O.learner_step(oa, hp, p0, np.zeros(P, np.float32), np.zeros(P, np.float32), 0, obs, act, rewards, dones, bl)
+        assert out["stats"].shape[0] == mb and out["opt_step"] == mb
+        p, m, v, k = p0, np.zeros(P, np.float32), np.zeros(P, np.float32), 0
+        Bm = B // mb
+        for g in range(mb):
+            sl = slice(g * Bm, (g + 1) * Bm)
+            h1 = O.make_hparams("impala", T, Bm, minibatches=1, optimizer=opt)
+            o1 = O.learner_step(oa, h1, p, m, v, k, np.ascontiguousarray(obs[:, sl]), np.ascontiguousarray(act[:, sl]),
+                                     np.ascontiguousarray(rewards[:, sl]), np.ascontiguousarray(dones[:, sl]), np.ascontiguousarray(bl[:, sl]))
+            p, m, v, k = o1["params"], o1["m"], o1["v"], o1["opt_step"]
+            np.testing.assert_array_equal(out["stats"][g], o1["stats"][0])
+        assert out["params"].tobytes() == p.tobytes() and out["v"].tobytes() == v.tobytes()
+        if opt == 1:
+            assert not out["m"].any()          # RMSprop keeps its state in the second buffer only
