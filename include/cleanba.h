@@ -57,11 +57,14 @@ typedef struct {
   float gamma, lambda_;             /* V-trace lambda (1) or GAE lambda (0.95) */
   float rho_bar, c_bar, rho_pg_bar; /* IMPALA */
   float clip_eps;                   /* PPO */
-  int epochs, minibatches, norm_adv; /* PPO */
+  int epochs, minibatches, norm_adv; /* PPO.  IMPALA: minibatches = number of env groups (A21,
+                                      * PAPER.md:213, 401): each group of B/minibatches whole trajectories is one update */
   uint64_t perm_seed;               /* PPO minibatch permutation (A17) */
   float vf_coef, ent_coef;          /* c1, c2 */
   float lr, beta1, beta2, adam_eps, max_grad_norm;
   int loss_reduction;               /* 0 = mean over samples, 1 = sum (A4) */
+  int optimizer;                    /* 0 = Adam (A12), 1 = RMSprop (Table 3; A22): state in adam_v only */
+  float rms_decay, rms_eps;         /* 0.99, 0.01; eps sits inside the square root */
 } cb_hparams;
 
 typedef struct cb_net cb_net; /* opaque: layer table, parameter offsets, device workspaces */
@@ -96,8 +99,8 @@ int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int 
                       int32_t* actions, void* stream);
 
 /* ---- learner side (Alg. 1 l.11-20) -------------------------------------- */
-/* One learner call: IMPALA = one V-trace gradient update; PPO = GAE, then epochs x minibatches
- * updates over a seeded permutation.  Updated in place (dev fp32 [P]): params, adam_m, adam_v.
+/* One learner call: IMPALA = `minibatches` V-trace gradient updates, one per group of envs in order (1 = one
+ * full-batch update); PPO = GAE, then epochs x minibatches updates over a seeded permutation.  Updated in place (dev fp32 [P]): params, adam_m, adam_v.
  * opt_step: host counter, incremented once per gradient update (Adam's k, from 1).
  * obs: dev uint8 [T+1,B,in_c,in_h,in_w]; actions: dev int32 [T,B]; rewards: dev fp32 [T,B];
  * dones: dev uint8 [T,B], 1 <=> the step taken at t ended the episode (A1);
@@ -157,6 +160,14 @@ typedef struct {
 } cb_prof_entry;
 int cb_profile_begin(int only_class);
 int cb_profile_end(cb_prof_entry* out, int max);
+
+/* A22: global-norm clip + RMSprop: nu <- decay nu + (1-decay) g^2; theta <- theta - lr g / sqrt(nu + eps).  Same buffer rules
+ * and scratch as cb_clip_adam. */
+int cb_clip_rmsprop(size_t P, float* params, float* nu, const float* grad, float lr, float decay, float eps, float max_norm,
+                    float* grad_norm, void* scratch, void* stream);
+/* Linear decay of the learning rate to 0 over `total` updates (Tables 2-3): lr0 (1 - min(k,total)/total).
+ * Host arithmetic: the caller passes the result as cb_hparams.lr of update k. */
+float cb_linear_lr(float lr0, uint64_t k, uint64_t total);
 
 const char* cb_last_error(void);
 

@@ -19,7 +19,7 @@ ALGO = {"impala": 0, "ppo": 1}
 EXPORTS = ["cb_net_create", "cb_net_destroy", "cb_param_count", "cb_param_layout", "cb_net_init", "cb_policy_forward",
            "cb_learner_step", "cb_learner_view", "cb_sample_actions", "cb_logprob_entropy", "cb_vtrace", "cb_gae",
            "cb_permutation", "cb_clip_adam_scratch_bytes", "cb_clip_adam", "cb_last_error",
-           "cb_launch_count", "cb_profile_begin", "cb_profile_end"]
+           "cb_launch_count", "cb_profile_begin", "cb_profile_end", "cb_clip_rmsprop", "cb_linear_lr"]
 
 
 class CArch(C.Structure):
@@ -35,7 +35,8 @@ class CHParams(C.Structure):
                 ("perm_seed", C.c_uint64),
                 ("vf_coef", C.c_float), ("ent_coef", C.c_float),
                 ("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("adam_eps", C.c_float),
-                ("max_grad_norm", C.c_float), ("loss_reduction", C.c_int)]
+                ("max_grad_norm", C.c_float), ("loss_reduction", C.c_int),
+                ("optimizer", C.c_int), ("rms_decay", C.c_float), ("rms_eps", C.c_float)]
 
 
 class CleanbaError(RuntimeError):
@@ -57,6 +58,8 @@ def lib():
         L.cb_clip_adam_scratch_bytes.argtypes = [C.c_size_t]
         L.cb_last_error.restype = C.c_char_p
         L.cb_launch_count.restype = C.c_uint64
+        L.cb_linear_lr.restype = C.c_float
+        L.cb_linear_lr.argtypes = [C.c_float, C.c_uint64, C.c_uint64]
         L.cb_net_destroy.restype = None
         L.cb_net_destroy.argtypes = [C.c_void_p]
         _lib = L
@@ -75,7 +78,8 @@ def make_hparams(algo="impala", precision="bf16", T=20, B=128, **kw):
     h.algo = 1 if ppo else 0; h.precision = PREC.get(precision, precision); h.T = T; h.B = B
     h.gamma = 0.99; h.lambda_ = 0.95 if ppo else 1.0
     h.rho_bar = h.c_bar = h.rho_pg_bar = 1.0
-    h.clip_eps = 0.1; h.epochs = 4; h.minibatches = 4; h.norm_adv = 1; h.perm_seed = 1
+    h.clip_eps = 0.1; h.epochs = 4; h.minibatches = 4 if ppo else 1; h.norm_adv = 1; h.perm_seed = 1
+    h.optimizer = 0; h.rms_decay = 0.99; h.rms_eps = 0.01        # optimizer 1 = the paper's RMSprop (Table 3)
     h.vf_coef = 0.5; h.ent_coef = 0.01
     h.lr = 2.5e-4 if ppo else 6e-4; h.beta1 = 0.9; h.beta2 = 0.999; h.adam_eps = 1e-5
     h.max_grad_norm = 0.5 if ppo else 40.0; h.loss_reduction = 0
@@ -165,7 +169,7 @@ class Net:
         for t, n in ((params, "params"), (adam_m, "adam_m"), (adam_v, "adam_v"), (rewards, "rewards"), (behaviour_logits, "behaviour_logits")):
             _dev(t, torch.float32, n)
         _dev(obs, torch.uint8, "obs"); _dev(dones, torch.uint8, "dones"); _dev(actions, torch.int32, "actions")
-        n_upd = hp.epochs * hp.minibatches if hp.algo == 1 else 1
+        n_upd = hp.epochs * hp.minibatches if hp.algo == 1 else max(1, hp.minibatches)
         if stats is None:
             stats = torch.zeros((n_upd, N_STATS), dtype=torch.float32, device=obs.device)
         k = C.c_uint64(opt_step)
@@ -242,6 +246,23 @@ def clip_adam(params, adam_m, adam_v, grad, k, lr, beta1=0.9, beta2=0.999, eps=1
     _check(lib().cb_clip_adam(C.c_size_t(P), _ptr(params), _ptr(adam_m), _ptr(adam_v), _ptr(grad), C.c_uint64(k), C.c_float(lr), C.c_float(beta1),
                               C.c_float(beta2), C.c_float(eps), C.c_float(max_norm), _ptr(gn), _ptr(scratch), _stream()))
     return gn
+
+
+def clip_rmsprop(params, nu, grad, lr, decay=0.99, eps=0.01, max_norm=40.0, scratch=None):
+    """In place on params / nu; returns the pre-clip gradient norm as a cuda fp32 [1] tensor (A22)."""
+    torch = _torch(); P = params.numel()
+    for t, n in ((params, "params"), (nu, "nu"), (grad, "grad")):
+        _dev(t, torch.float32, n)
+    if scratch is None:
+        scratch = torch.empty((int(lib().cb_clip_adam_scratch_bytes(C.c_size_t(P))) + 7) // 8, dtype=torch.float64, device=params.device)
+    gn = torch.empty((1,), dtype=torch.float32, device=params.device)
+    _check(lib().cb_clip_rmsprop(C.c_size_t(P), _ptr(params), _ptr(nu), _ptr(grad), C.c_float(lr), C.c_float(decay), C.c_float(eps), C.c_float(max_norm),
+                                 _ptr(gn), _ptr(scratch), _stream()))
+    return gn
+
+
+def linear_lr(lr0, k, total):
+    return float(lib().cb_linear_lr(C.c_float(lr0), C.c_uint64(k), C.c_uint64(total)))
 
 
 # ---- instrumentation ----------------------------------------------------------------------------------

@@ -144,9 +144,10 @@ static void free_workspace(Workspace& ws) {
   cudaFree(ws.partial); ws.partial = nullptr; ws.frames = 0;
 }
 static void free_scratch(Workspace& ws) {
-  void* ps[] = {ws.logpi, ws.logmu, ws.ent, ws.t0, ws.t1, ws.rho, ws.values, ws.terms, ws.red, ws.advstat, ws.perm, ws.permj};
+  void* ps[] = {ws.logpi, ws.logmu, ws.ent, ws.t0, ws.t1, ws.rho, ws.values, ws.terms, ws.red, ws.advstat, ws.perm, ws.permj, ws.act_m, ws.rew_m, ws.dones_m, ws.logmu_m};
   for (void* p : ps) cudaFree(p);
   ws.logpi = ws.logmu = ws.ent = ws.t0 = ws.t1 = ws.rho = ws.values = ws.terms = ws.advstat = nullptr; ws.red = nullptr; ws.perm = nullptr; ws.permj = nullptr;
+  ws.act_m = nullptr; ws.rew_m = nullptr; ws.dones_m = nullptr; ws.logmu_m = nullptr;
   ws.learn_frames = ws.learn_N = ws.learn_epochs = 0;
 }
 
@@ -199,7 +200,8 @@ int ensure_learner_scratch(cb_net* net, int prec, int F, int N, int epochs) {
   CB_ALLOC(ws.logpi, n4); CB_ALLOC(ws.logmu, n4); CB_ALLOC(ws.ent, n4); CB_ALLOC(ws.t0, n4); CB_ALLOC(ws.t1, n4); CB_ALLOC(ws.rho, n4);
   CB_ALLOC(ws.values, (size_t)F * (net->arch.n_actions + 1) * 4);
   CB_ALLOC(ws.terms, n4 * 5); CB_ALLOC(ws.red, 64); CB_ALLOC(ws.advstat, 16);
-  CB_ALLOC(ws.perm, n4 * epochs); CB_ALLOC(ws.permj, n4 * epochs);
+  CB_ALLOC(ws.perm, std::max(n4 * epochs, (size_t)F * 4)); CB_ALLOC(ws.permj, n4 * epochs);
+  CB_ALLOC(ws.act_m, n4); CB_ALLOC(ws.rew_m, n4); CB_ALLOC(ws.dones_m, (size_t)N); CB_ALLOC(ws.logmu_m, n4);
   ws.learn_frames = F; ws.learn_N = N; ws.learn_epochs = epochs;
   return CB_OK;
 }
@@ -319,23 +321,48 @@ int cb_learner_step(cb_net* net, float* params, float* adam_m, float* adam_v, ui
   const int N = T * B, F = (T + 1) * B;
   const bool ppo = hp->algo == CB_ALGO_PPO;
   if (ppo && (hp->epochs < 1 || hp->minibatches < 1 || N % hp->minibatches != 0)) { set_error("PPO needs epochs >= 1 and minibatches dividing T*B"); return CB_EINVAL; }
+  const int mb = ppo ? hp->minibatches : (hp->minibatches < 1 ? 1 : hp->minibatches);
+  if (!ppo && B % mb != 0) { set_error("IMPALA needs minibatches dividing B (env groups, A21)"); return CB_EINVAL; }
+  if (hp->optimizer != 0 && hp->optimizer != 1) { set_error("bad optimizer"); return CB_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream; int rc;
   if ((rc = ensure_workspace(net, prec, F))) return rc;
   if ((rc = ensure_learner_scratch(net, prec, F, N, ppo ? hp->epochs : 1))) return rc;
   Workspace& ws = net->ws[prec];
-  net->last_prec = prec; net->last_F = F; net->last_N = N; net->last_ppo = ppo;
+  net->last_prec = prec; net->last_F = F; net->last_N = N; net->last_ppo = ppo || mb > 1;
   if ((rc = pack_weights(net, prec, params, st))) return rc;
   if ((rc = forward(net, prec, obs, nullptr, F, st))) return rc;
   float* head = (float*)ws.act[net->head_t];
   if ((rc = launch_logprob(behaviour_logits, A, N, A, actions, nullptr, ws.logmu, nullptr, st))) return rc;
-  if (!ppo) {
+  auto optimizer_step = [&](float* stats_row) -> int {
+    *opt_step += 1;
+    if (hp->optimizer == 1)
+      return launch_clip_rmsprop(net->P, params, adam_v, ws.gradbuf, hp->lr, hp->rms_decay, hp->rms_eps, hp->max_grad_norm, ws.gnorm, stats_row + 4, ws.adam_scratch, st);
+    return launch_clip_adam(net->P, params, adam_m, adam_v, ws.gradbuf, *opt_step, hp->lr, hp->beta1, hp->beta2, hp->adam_eps, hp->max_grad_norm, ws.gnorm, stats_row + 4, ws.adam_scratch, st);
+  };
+  if (!ppo && mb == 1) {
     if ((rc = launch_logprob(head, A + 1, N, A, actions, nullptr, ws.logpi, nullptr, st))) return rc;
     if ((rc = launch_vtrace(T, B, head + A, A + 1, rewards, dones, ws.logpi, ws.logmu, hp->gamma, hp->lambda_, hp->rho_bar, hp->c_bar, hp->rho_pg_bar, ws.t0, ws.t1, ws.rho, st))) return rc;
     if ((rc = launch_impala_loss(prec, N, A, head, actions, ws.t0, ws.t1, ws.rho, hp->vf_coef, hp->ent_coef, hp->loss_reduction, ws.grad[G_HEAD], ws.terms, ws.red, stats, st))) return rc;
     if ((rc = backward(net, prec, obs, nullptr, N, ws.gradbuf, st))) return rc;
-    *opt_step += 1;
-    if ((rc = launch_clip_adam(net->P, params, adam_m, adam_v, ws.gradbuf, *opt_step, hp->lr, hp->beta1, hp->beta2, hp->adam_eps, hp->max_grad_norm, ws.gnorm, stats + 4, ws.adam_scratch, st))) return rc;
+    if ((rc = optimizer_step(stats))) return rc;
     return 1;
+  }
+  if (!ppo) {
+    // A21: one complete update per group of B/mb envs, in group order, each with the parameters the previous one left
+    const int Bm = B / mb, Nm = T * Bm, Fm = (T + 1) * Bm;
+    CB_CUDA(cudaMemcpyAsync(ws.values, head, (size_t)F * (A + 1) * 4, cudaMemcpyDeviceToDevice, st));      // cb_learner_view(0)
+    for (int k = 0; k < mb; ++k) {
+      float* st_out = stats + (size_t)k * CB_N_STATS;
+      if ((rc = launch_gather_traj(T, B, k * Bm, Bm, actions, rewards, dones, ws.logmu, ws.perm, ws.act_m, ws.rew_m, ws.dones_m, ws.logmu_m, st))) return rc;
+      if (k > 0) if ((rc = pack_weights(net, prec, params, st))) return rc;
+      if ((rc = forward(net, prec, obs, ws.perm, Fm, st))) return rc;
+      if ((rc = launch_logprob(head, A + 1, Nm, A, ws.act_m, nullptr, ws.logpi, nullptr, st))) return rc;
+      if ((rc = launch_vtrace(T, Bm, head + A, A + 1, ws.rew_m, ws.dones_m, ws.logpi, ws.logmu_m, hp->gamma, hp->lambda_, hp->rho_bar, hp->c_bar, hp->rho_pg_bar, ws.t0, ws.t1, ws.rho, st))) return rc;
+      if ((rc = launch_impala_loss(prec, Nm, A, head, ws.act_m, ws.t0, ws.t1, ws.rho, hp->vf_coef, hp->ent_coef, hp->loss_reduction, ws.grad[G_HEAD], ws.terms, ws.red, st_out, st))) return rc;
+      if ((rc = backward(net, prec, obs, ws.perm, Nm, ws.gradbuf, st))) return rc;
+      if ((rc = optimizer_step(st_out))) return rc;
+    }
+    return mb;
   }
   // PPO (Alg. 1 l.11-20): values and old log-probs from the iteration-start parameters
   CB_CUDA(cudaMemcpyAsync(ws.values, head, (size_t)F * (A + 1) * 4, cudaMemcpyDeviceToDevice, st));
@@ -350,8 +377,7 @@ int cb_learner_step(cb_net* net, float* params, float* adam_m, float* adam_v, ui
       float* st_out = stats + (size_t)upd * CB_N_STATS;
       if ((rc = launch_ppo_loss(prec, m, A, head, idx, actions, ws.t0, ws.t1, ws.logmu, hp->clip_eps, hp->vf_coef, hp->ent_coef, hp->norm_adv, ws.grad[G_HEAD], ws.terms, ws.red, ws.advstat, st_out, st))) return rc;
       if ((rc = backward(net, prec, obs, idx, m, ws.gradbuf, st))) return rc;
-      *opt_step += 1;
-      if ((rc = launch_clip_adam(net->P, params, adam_m, adam_v, ws.gradbuf, *opt_step, hp->lr, hp->beta1, hp->beta2, hp->adam_eps, hp->max_grad_norm, ws.gnorm, st_out + 4, ws.adam_scratch, st))) return rc;
+      if ((rc = optimizer_step(st_out))) return rc;
     }
   return upd;
 }
@@ -401,6 +427,16 @@ int cb_permutation(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* st
   int rc = launch_permutation(seed, epoch, 1, N, perm, jb, (cudaStream_t)stream);
   cudaFreeAsync(jb, (cudaStream_t)stream);
   return rc;
+}
+int cb_clip_rmsprop(size_t P, float* params, float* nu, const float* grad, float lr, float decay, float eps, float max_norm, float* grad_norm,
+                    void* scratch, void* stream) {
+  if (!params || !nu || !grad || !scratch) { set_error("bad argument"); return CB_EINVAL; }
+  if (misaligned(params, 16) || misaligned(nu, 16) || misaligned(grad, 16) || misaligned(scratch, 8)) { set_error("buffers must be 16-byte aligned"); return CB_EINVAL; }
+  return launch_clip_rmsprop(P, params, nu, grad, lr, decay, eps, max_norm, grad_norm, nullptr, scratch, (cudaStream_t)stream);
+}
+float cb_linear_lr(float lr0, uint64_t k, uint64_t total) {
+  if (total == 0) return lr0;
+  return (float)((double)lr0 * (1.0 - (double)std::min(k, total) / (double)total));
 }
 size_t cb_clip_adam_scratch_bytes(size_t P) { return clip_adam_scratch_bytes(P); }
 int cb_clip_adam(size_t P, float* params, float* adam_m, float* adam_v, const float* grad, uint64_t k, float lr, float beta1, float beta2,

@@ -84,7 +84,8 @@ struct Workspace {     // one per precision mode
   float* terms = nullptr;            // [5, N] per-sample loss terms
   double* red = nullptr;             // reduction scratch
   float* advstat = nullptr;          // [2] mean, 1/(std+eps)
-  int32_t* perm = nullptr;           // [epochs, N]
+  int32_t* perm = nullptr;           // [epochs, N]  (IMPALA env groups: frame indices [(T+1) * B/mb])
+  int32_t* act_m = nullptr; float* rew_m = nullptr; uint8_t* dones_m = nullptr; float* logmu_m = nullptr;   // env-group copies [T, B/mb]
   uint32_t* permj = nullptr;
   void* adam_scratch = nullptr;
   float* gnorm = nullptr;
@@ -179,6 +180,10 @@ int launch_impala_loss(int prec, int N, int A, const float* head, const int32_t*
 int launch_ppo_loss(int prec, int m, int A, const float* head, const int32_t* idx, const int32_t* act, const float* adv,
                     const float* ret, const float* logp_old, float eps, float c1, float c2, int norm_adv, void* dhead,
                     float* terms, double* red, float* advstat, float* stats, cudaStream_t st);
+int launch_clip_rmsprop(size_t P, float* params, float* nu, const float* g, float lr, float decay, float eps, float max_norm, float* grad_norm,
+                        float* stats_slot, void* scratch, cudaStream_t st);
+int launch_gather_traj(int T, int B, int b0, int Bm, const int32_t* act, const float* rew, const uint8_t* dones, const float* logmu, int32_t* fidx,
+                       int32_t* act_m, float* rew_m, uint8_t* dones_m, float* logmu_m, cudaStream_t st);
 size_t clip_adam_scratch_bytes(size_t P);
 int launch_clip_adam(size_t P, float* params, float* m, float* v, const float* g, uint64_t k, float lr, float b1, float b2,
                      float eps, float max_norm, float* grad_norm, float* stats_slot, void* scratch, cudaStream_t st);

@@ -486,6 +486,53 @@ __global__ void __launch_bounds__(256) adam_kernel(size_t P, float* __restrict__
   }
 }
 
+// A22: RMSprop with eps inside the root; nu_0 = 0
+__global__ void __launch_bounds__(256) rmsprop_kernel(size_t P, float* __restrict__ th, float* __restrict__ nu, const float* __restrict__ g,
+                                                      const double* __restrict__ norm, float max_norm, float decay, float omd, float lr, float eps) {
+  const double n = *norm;
+  const float scale = (float)((double)max_norm / fmax(n, (double)max_norm));
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < P; i += (size_t)gridDim.x * blockDim.x) {
+    const float gi = g[i] * scale;
+    const float ni = fmaf(decay, nu[i], omd * gi * gi);
+    nu[i] = ni;
+    th[i] -= lr * gi / sqrtf(ni + eps);
+  }
+}
+
+int launch_clip_rmsprop(size_t P, float* params, float* nu, const float* g, float lr, float decay, float eps, float max_norm, float* grad_norm,
+                        float* stats_slot, void* scratch, cudaStream_t st) {
+  if (P == 0) return CB_OK;
+  int nparts = (int)((P + NORM_CHUNK - 1) / NORM_CHUNK);
+  double* partial = (double*)scratch + 1; double* norm = (double*)scratch;
+  { ProfScope ps(K_SQNORM, st, 2, 0.0, (double)P * 4);
+  sqnorm_partial_kernel<<<nparts, 256, 0, st>>>(P, g, partial);
+  sqnorm_final_kernel<<<1, 256, 0, st>>>(nparts, partial, norm, grad_norm, stats_slot); }
+  ProfScope ps(K_ADAM, st, 1, 0.0, (double)P * 20);
+  int grid = (int)std::min<size_t>((P + 255) / 256, (size_t)148 * 8);
+  rmsprop_kernel<<<grid, 256, 0, st>>>(P, params, nu, g, norm, max_norm, decay, (float)(1.0 - (double)decay), lr, eps);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+// env group [b0, b0+Bm) of a [T,B] rollout: frame indices of its (T+1) x Bm observations (t-major) and contiguous copies
+// of its per-step data (A21)
+__global__ void gather_traj_kernel(int T, int B, int b0, int Bm, const int32_t* __restrict__ act, const float* __restrict__ rew,
+                                   const uint8_t* __restrict__ dones, const float* __restrict__ logmu, int32_t* __restrict__ fidx,
+                                   int32_t* __restrict__ act_m, float* __restrict__ rew_m, uint8_t* __restrict__ dones_m, float* __restrict__ logmu_m) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (T + 1) * Bm) return;
+  const int t = i / Bm, b = i - t * Bm, src = t * B + b0 + b;
+  fidx[i] = src;
+  if (t < T) { act_m[i] = act[src]; rew_m[i] = rew[src]; dones_m[i] = dones[src]; logmu_m[i] = logmu[src]; }
+}
+int launch_gather_traj(int T, int B, int b0, int Bm, const int32_t* act, const float* rew, const uint8_t* dones, const float* logmu, int32_t* fidx,
+                       int32_t* act_m, float* rew_m, uint8_t* dones_m, float* logmu_m, cudaStream_t st) {
+  ProfScope ps(K_HEAD_MISC, st);
+  gather_traj_kernel<<<((T + 1) * Bm + 127) / 128, 128, 0, st>>>(T, B, b0, Bm, act, rew, dones, logmu, fidx, act_m, rew_m, dones_m, logmu_m);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
 size_t clip_adam_scratch_bytes(size_t P) { return (((P + NORM_CHUNK - 1) / NORM_CHUNK) + 2) * sizeof(double); }
 
 int launch_clip_adam(size_t P, float* params, float* m, float* v, const float* g, uint64_t k, float lr, float b1, float b2, float eps,

@@ -101,3 +101,11 @@ def test_batch_bookkeeping_worked_example():
     # 8 envs x 128 steps = 1024, 4 minibatches of 256, K = 4 epochs -> 16 updates
     hp = binding.make_hparams("ppo", T=128, B=8)
     assert hp.T * hp.B == 1024 and hp.T * hp.B // hp.minibatches == 256 and hp.epochs * hp.minibatches == 16
+
+
+def test_impala_defaults_and_linear_lr_host():
+    i = binding.make_hparams("impala")
+    assert i.minibatches == 1 and i.optimizer == 0 and (i.rms_decay, i.rms_eps) == pytest.approx((0.99, 0.01))     # Table 3
+    # cb_linear_lr is host arithmetic: compare with the oracle's closed form
+    for k, total in [(0, 100), (25, 100), (100, 100), (500, 100), (3, 0)]:
+        assert binding.linear_lr(6e-4, k, total) == pytest.approx(oracle.linear_lr(float(np.float32(6e-4)), k, total), rel=1e-6, abs=1e-12)

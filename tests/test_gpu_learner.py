@@ -269,3 +269,57 @@ def test_errors_on_bad_shapes():
         net.learner_step(torch.zeros(net.P, device="cuda"), torch.zeros(net.P, device="cuda"), torch.zeros(net.P, device="cuda"), 0,
                          torch.zeros((4, 3, 4, 84, 84), dtype=torch.uint8, device="cuda"), torch.zeros((3, 3), dtype=torch.int32, device="cuda"),
                          z, torch.zeros(9, dtype=torch.uint8, device="cuda"), torch.zeros((3, 3, 18), device="cuda"), hp)
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT row f1: the paper's IMPALA schedule -- env-split minibatches (A21) with RMSprop (A22)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("prec,opt", [("fp32", 1), ("fp32", 0), ("bf16", 1)])
+def test_learner_impala_env_split_rmsprop(prec, opt):
+    arch, T, B, mb = TINY_IMPALA, 5, 12, 4
+    hp, ho = _hp_pair("impala", prec, T, B, minibatches=mb, optimizer=opt)
+    ho.rms_decay, ho.rms_eps = float(hp.rms_decay), float(hp.rms_eps)
+    bt = _batch(arch, T, B, 91, False)
+    params = synth.gen_params(arch, 92, bias_scale=0.05, head_scale=0.1); P = params.size
+    g = synth.rng(93)
+    m = np.zeros(P, np.float32) if opt == 1 else (g.standard_normal(P) * 1e-3).astype(np.float32)
+    v = (g.random(P) * 1e-5 + 1e-6).astype(np.float32)          # warm second-moment state: the comparison is not a sign test
+    k0 = 50
+    net = binding.Net(arch)
+    dp, dm, dv = dev(params), dev(m), dev(v)
+    k1, stats = net.learner_step(dp, dm, dv, k0, *[dev(bt[k]) for k in ("obs", "actions", "rewards", "dones", "behaviour_logits")], hp)
+    torch.cuda.synchronize()
+    ref = oracle.learner_step(orc_arch(arch), ho, params, m, v, k0, bt["obs"], bt["actions"], bt["rewards"], bt["dones"], bt["behaviour_logits"])
+    assert k1 == ref["opt_step"] == k0 + mb and host(stats).shape == ref["stats"].shape == (mb, 8)
+    rt = RTOL[prec]
+    for u in range(mb):
+        gs, rs = host(stats)[u].astype(np.float64), ref["stats"][u].astype(np.float64)
+        scale = abs(rs[1]) + abs(rs[2]) + 0.01 * abs(rs[3]) + 1e-3 + (0.1 if prec == "fp32" else 5.0)
+        srt = rt if u == 0 else 10 * rt
+        for i in (0, 1, 2, 3, 7):
+            assert abs(gs[i] - rs[i]) <= srt * max(abs(gs[i]), abs(rs[i])) + srt * scale, (u, oracle.STAT_NAMES[i], gs[i], rs[i])
+        if prec == "fp32":
+            assert abs(gs[4] - rs[4]) <= 1e-3 * rs[4], (u, gs[4], rs[4])
+    for name, off, dims in net.param_layout():
+        n = int(np.prod(dims)); gp, rp = host(dp)[off:off + n].astype(np.float64), ref["params"][off:off + n].astype(np.float64)
+        small = name.endswith(".b") or name in ("pi.w", "v.w")
+        slack = (1.0 if prec == "bf16" else 0.02) * hp.lr * mb * np.sqrt(n) if small else 0.0
+        assert np.linalg.norm(gp - rp) <= PTOL[prec] * np.linalg.norm(rp) + slack, (name, rel_l2(gp, rp))
+    if opt == 1:
+        assert host(dm).tobytes() == m.tobytes()                  # RMSprop never touches the first-moment buffer
+    assert rel_l2(host(dv), ref["v"]) < (1e-4 if prec == "fp32" else 1.5e-1)      # nu accumulates g^2: twice the relative error of the bf16 gradient
+
+
+@pytest.mark.parametrize("P", [5, 4099, 1094115])
+def test_clip_rmsprop_parity(P):
+    g = synth.rng(P)
+    th = (g.standard_normal(P) * 0.05).astype(np.float32); grad = (g.standard_normal(P) * 3.0 / np.sqrt(P)).astype(np.float32)
+    nu = (g.random(P) * 1e-4).astype(np.float32)
+    dth, dnu = dev(th), dev(nu)
+    gn = binding.clip_rmsprop(dth, dnu, dev(grad), 6e-4, 0.99, 0.01, 0.5)
+    rth, rnu, rn = oracle.clip_rmsprop(th, nu, grad.astype(np.float64), 6e-4, float(np.float32(0.99)), float(np.float32(0.01)), 0.5)
+    assert abs(float(host(gn)[0]) - rn) <= 1e-6 * rn
+    close(host(dnu), rnu, 1e-5, what="nu")
+    du_g, du_r = host(dth).astype(np.float64) - th, rth.astype(np.float64) - th
+    assert (np.abs(du_g - du_r) <= 1e-4 * np.abs(du_r) + 1.2e-8).all()       # 1.2e-8: two ulps of a parameter of size 0.05-0.1 in fp32
+    assert rel_l2(host(dth), rth) < 1e-6
