@@ -163,7 +163,7 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
 }
 
-constexpr int WNLOAD = 256;     // warps 0-7 stage (warps 0-1 later drain TMEM); warp 8: one thread issues the MMAs
+constexpr int WNLOAD = 512;     // warps 0-15 stage (the gather is latency-bound: more loads in flight); warps 0-1 later drain TMEM; warp 16 issues the MMAs
 
 // Two stages of (X plane, DY planes): the loaders fill one while the tensor core reads the other.  UMMA M = 64:
 // accumulator row r = 8*dj + c sits in TMEM lane 32*(r/16) + r%16.

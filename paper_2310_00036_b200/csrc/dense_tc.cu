@@ -168,6 +168,7 @@ __global__ void colsum_kernel(const bf16* __restrict__ dy, int F, int N, float* 
   int n = blockIdx.x * blockDim.x + threadIdx.x;
   if (n >= N) return;
   float s = 0.f;
+#pragma unroll 16
   for (int f = 0; f < F; ++f) s += __bfloat162float(dy[(size_t)f * N + n]);
   out[n] = s;
 }

@@ -277,7 +277,8 @@ __global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nc
   const int rows = g.Cin + 1, per = 9 * rows * g.Cout;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < per; i += gridDim.x * blockDim.x) {
     float s = 0.f;
-    for (int z = 0; z < nctas; ++z) s += partial[(size_t)z * per + i];
+#pragma unroll 8
+    for (int z = 0; z < nctas; ++z) s += partial[(size_t)z * per + i];      // loads independent, adds in CTA order
     int o = i % g.Cout, q = i / g.Cout, row = q % rows, tap = q / rows;
     if (row == g.Cin) { if (tap == 0) grad[pm.b(o)] = s; continue; }
     grad[pm.w(o, row, tap / 3, tap % 3, g)] = s;
