@@ -87,6 +87,7 @@ struct ConvTcArgs {
   const bf16* aux1;    // dgrad: gradient added after gating; nullable
   bf16* out;           // [F, H, W, COUT]
   int F, H, W, G, npix_alloc, relu_in, use_tma;
+  int RB, nbands;      // rows per band (= H when the whole frame is staged) and bands per frame (banded: G = 1, TMA only)
   int* error_flag;
 };
 
@@ -103,7 +104,7 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, cons
   __shared__ __align__(8) uint64_t ldbar_storage;
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5, wg = warp >> 2, lane_row = tid & 127;
-  const int Wp = a.W + 2, R = (a.H + 2) * Wp;
+  const int Wp = a.W + 2, R = (a.RB + 2) * Wp;      // R = staged positions per frame (band with its halo)
   uint8_t* w_smem = smem;
   uint8_t* in_smem = smem + ((W_BYTES + 127u) & ~127u);
   const uint32_t plane_bytes = (uint32_t)a.npix_alloc * 16u;
@@ -122,10 +123,11 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, cons
   const uint32_t idesc = make_idesc(128, COUT, 0, 0);
   const uint32_t a_base = smem_u32(in_smem), b_base = smem_u32(w_smem);
   uint32_t parity = 0, ldparity = 0;
-  const int ngroups = (a.F + a.G - 1) / a.G;
+  const int ngroups = ((a.F + a.G - 1) / a.G) * a.nbands;
 
   for (int grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
-    const int f0 = grp * a.G, nf = min(a.G, a.F - f0);
+    const int fg = grp / a.nbands, yb = (grp - fg * a.nbands) * a.RB;
+    const int f0 = fg * a.G, nf = min(a.G, a.F - f0);
     // ---- stage the group's frames: global NHWC -> planes, ReLU on the way in --------------------------
     if (a.use_tma) {
       // ---- TMA: one bulk tensor copy per 8-channel chunk lands the whole group, zero halo included (box starts at (-1,-1)) ----
@@ -133,7 +135,7 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, cons
       if (tid == 0) {
         tma::arrive_expect_tx(ldbar, bytes * NCH);
 #pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) tma::load_4d(a_base + (uint32_t)ch * plane_bytes, &tmap, ch * 8, -1, -1, f0, ldbar);
+        for (int ch = 0; ch < NCH; ++ch) tma::load_4d(a_base + (uint32_t)ch * plane_bytes, &tmap, ch * 8, -1, yb - 1, f0, ldbar);
       }
       if (!mbar_wait(ldbar, ldparity)) { if (a.error_flag) *a.error_flag = 6; }
       ldparity ^= 1;
@@ -181,7 +183,7 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, cons
     }
     fence_async_smem();
     __syncthreads();
-    const int ntiles = (nf * R + 127) / 128;
+    const int ntiles = ((nf - 1) * R + a.RB * Wp + 127) / 128;      // positions up to the last computed row of the last frame
     for (int t0 = 0; t0 < ntiles; t0 += TILES_PER_BATCH) {
       const int nt = min(TILES_PER_BATCH, ntiles - t0);
       if (tid == 0) {
@@ -210,8 +212,8 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, cons
       for (int s = wg; s < nt; s += 2) {
         const int q = (t0 + s) * 128 + lane_row;
         const int j = q / R, rem = q - j * R;
-        const int y = rem / Wp, x = rem - y * Wp;
-        const bool valid = j < nf && y < a.H && x < a.W;
+        const int yl = rem / Wp, x = rem - yl * Wp, y = yb + yl;
+        const bool valid = j < nf && yl < a.RB && y < a.H && x < a.W;
         const size_t o = (((size_t)(f0 + j) * a.H + y) * a.W + x) * COUT;
 #pragma unroll
         for (int c0 = 0; c0 < COUT; c0 += 16) {
@@ -266,7 +268,7 @@ bool conv_tc_supported(const Geom& g) {
   return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && okc(g.Cin) && okc(g.Cout) && g.H == g.Ho && g.W == g.Wo;
 }
 
-struct TcPlan { int G, npix_alloc; size_t smem; };
+struct TcPlan { int G, npix_alloc, RB, nbands; size_t smem; };
 static TcPlan tc_plan(int H, int W, int cin, int cout) {
   const int Wp = W + 2, R = (H + 2) * Wp;
   const size_t wbytes = ((size_t)9 * cin * cout * 2 + 127) & ~(size_t)127;
@@ -276,7 +278,17 @@ static TcPlan tc_plan(int H, int W, int cin, int cout) {
   if (G > 8) G = 8;
   int npix = ((G * R + 127) / 128) * 128 + 2 * Wp + 2;
   npix = (npix + 7) / 8 * 8;
-  return {G, npix, wbytes + (size_t)npix * cin * 2};
+  TcPlan p{G, npix, H, 1, wbytes + (size_t)npix * cin * 2};
+  if (p.smem > 200 * 1024) {      // a whole frame does not fit: row bands of RB rows (+2 halo rows), one frame at a time
+    const long avail = 200 * 1024 - (long)wbytes;
+    int rows = (int)(avail / ((long)cin * 2) - 2 * Wp - 136) / Wp - 2;
+    if (rows < 1) rows = 1;
+    p.nbands = (H + rows - 1) / rows; p.RB = (H + p.nbands - 1) / p.nbands; p.G = 1;
+    npix = (((p.RB + 2) * Wp + 127) / 128) * 128 + 2 * Wp + 2;
+    p.npix_alloc = (npix + 7) / 8 * 8;
+    p.smem = wbytes + (size_t)p.npix_alloc * cin * 2;
+  }
+  return p;
 }
 
 // the staged frame group (with halo) plus the weight image must fit one CTA's shared memory
@@ -312,9 +324,10 @@ int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16*
   TcPlan p = tc_plan(H, W, cin, cout);
   if (p.smem > 220 * 1024) { set_error("conv_tc: frame does not fit shared memory"); return CB_EINVAL; }
   CUtensorMap tmap; memset(&tmap, 0, sizeof tmap);
-  const bool use_tma = W + 2 <= 256 && H + 2 <= 256 && tma::make_nhwc_map(&tmap, in, F, H, W, cin, W + 2, H + 2, p.G);
-  tc::ConvTcArgs a{in, w, bias, aux0, aux1, out, F, H, W, p.G, p.npix_alloc, relu_in ? 1 : 0, use_tma ? 1 : 0, error_flag};
-  int ngroups = (F + p.G - 1) / p.G;
+  const bool use_tma = W + 2 <= 256 && p.RB + 2 <= 256 && tma::make_nhwc_map(&tmap, in, F, H, W, cin, W + 2, p.RB + 2, p.G);
+  if (!use_tma && p.nbands > 1) { set_error("conv_tc: banded staging needs TMA"); return CB_EINVAL; }
+  tc::ConvTcArgs a{in, w, bias, aux0, aux1, out, F, H, W, p.G, p.npix_alloc, relu_in ? 1 : 0, use_tma ? 1 : 0, p.RB, p.nbands, error_flag};
+  int ngroups = ((F + p.G - 1) / p.G) * p.nbands;
   return mode == 0 ? dispatch<0>(cin, cout, a, tmap, p.smem, ngroups, st) : dispatch<1>(cin, cout, a, tmap, p.smem, ngroups, st);
 }
 

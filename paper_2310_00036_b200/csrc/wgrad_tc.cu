@@ -63,6 +63,7 @@ struct WgradTcArgs {
   const bf16* dy;     // [F, H, W, COUT]
   float* partial;     // [gridDim.x][9][CIN+1][COUT]
   int F, H, W, G, R, nbands, npix_alloc, kext, relu_in, stage_planes, use_tma, dy_rows;
+  int c_off, cin_total;      // the kernel handles input channels [c_off, c_off + CIN) of a layer with cin_total channels
   int* error_flag;
 };
 
@@ -156,7 +157,7 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
             int y = yb - 1 + lr, x = xp - 1;
             dst[u] = (uint32_t)ch * P + (uint32_t)pos * 16u;
             if (j < nf && (unsigned)y < (unsigned)a.H && (unsigned)x < (unsigned)a.W)
-              v[u] = *reinterpret_cast<const uint4*>(a.x + (((size_t)(f0 + j) * a.H + y) * a.W + x) * CIN + ch * 8);
+              v[u] = *reinterpret_cast<const uint4*>(a.x + (((size_t)(f0 + j) * a.H + y) * a.W + x) * a.cin_total + a.c_off + ch * 8);
           }
         }
 #pragma unroll
@@ -239,7 +240,7 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
         tma::arrive_expect_tx(rb, xbytes * XPL + ybytes * YCH);
         for (int pl = 0; pl < XPL; ++pl) {       // plane (dj, ch): X shifted by dj positions = box started dj columns further right
           const int dj = ST3 ? pl / XCH : 0, ch = ST3 ? pl % XCH : pl;
-          tma::load_4d(xs + (uint32_t)pl * P, &xmap, ch * 8, -1 + dj, yb - 1, f0, rb);
+          tma::load_4d(xs + (uint32_t)pl * P, &xmap, a.c_off + ch * 8, -1 + dj, yb - 1, f0, rb);
         }
         for (int ch = 0; ch < YCH; ++ch) tma::load_4d(ys + (uint32_t)ch * P, &ymap, ch * 8, 0, yb, f0, rb);
       }
@@ -273,23 +274,24 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
 }
 
 // sums the per-CTA partials in CTA order and scatters to the canonical gradient
-__global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nctas, Geom g, ParamMap pm, float* __restrict__ grad) {
-  const int rows = g.Cin + 1, per = 9 * rows * g.Cout;
+__global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nctas, Geom g, ParamMap pm, int cin_k, int c_off, float* __restrict__ grad) {
+  const int rows = cin_k + 1, per = 9 * rows * g.Cout;      // cin_k = channels handled by the kernel launch that wrote `partial`
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < per; i += gridDim.x * blockDim.x) {
     float s = 0.f;
 #pragma unroll 8
     for (int z = 0; z < nctas; ++z) s += partial[(size_t)z * per + i];      // loads independent, adds in CTA order
     int o = i % g.Cout, q = i / g.Cout, row = q % rows, tap = q / rows;
-    if (row == g.Cin) { if (tap == 0) grad[pm.b(o)] = s; continue; }
-    grad[pm.w(o, row, tap / 3, tap % 3, g)] = s;
+    if (row == cin_k) { if (tap == 0 && c_off == 0) grad[pm.b(o)] = s; continue; }
+    grad[pm.w(o, c_off + row, tap / 3, tap % 3, g)] = s;
   }
 }
 
 }  // namespace tcw
 
 bool wgrad_tc_supported(const Geom& g) {
-  auto okc = [](int c) { return c == 16 || c == 32; };
-  return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && okc(g.Cin) && okc(g.Cout) && g.H == g.Ho && g.W == g.Wo;
+  // Cin = 64 runs as two launches over 32 input channels each; Cin = 16 supports Cout <= 32
+  const bool okc = (g.Cin == 16 && (g.Cout == 16 || g.Cout == 32)) || ((g.Cin == 32 || g.Cin == 64) && (g.Cout == 16 || g.Cout == 32 || g.Cout == 64));
+  return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && okc && g.H == g.Ho && g.W == g.Wo;
 }
 
 constexpr int WGRAD_TC_MAX_CTAS = 148;
@@ -333,7 +335,8 @@ static int launch_w(const tcw::WgradTcArgs& a, const CUtensorMap& xmap, const CU
 int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
                     int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
-  WPlan p = wgrad_plan(g.H, g.W, g.Cin, g.Cout);
+  const int cin_k = g.Cin == 64 ? 32 : g.Cin;      // channels per kernel launch
+  WPlan p = wgrad_plan(g.H, g.W, cin_k, g.Cout);
   if (p.smem > 224 * 1024) { set_error("wgrad_tc: plan does not fit shared memory"); return CB_EINVAL; }
   const int nitems = ((F + p.G - 1) / p.G) * p.nbands;
   const int grid = std::min(nitems, WGRAD_TC_MAX_CTAS);
@@ -343,15 +346,19 @@ int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, con
   CUtensorMap xmap, ymap; memset(&xmap, 0, sizeof xmap); memset(&ymap, 0, sizeof ymap);
   const bool use_tma = g.W + 2 <= 256 && p.R + 2 <= 256 && tma::make_nhwc_map(&xmap, x, F, g.H, g.W, g.Cin, g.W + 2, p.R + 2, p.G) &&
                        tma::make_nhwc_map(&ymap, dy, F, g.H, g.W, g.Cout, g.W + 2, dy_rows, p.G);
-  tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, p.stage_planes, use_tma ? 1 : 0, dy_rows, error_flag};
-  int rc;
-  if (g.Cin == 16 && g.Cout == 16) rc = launch_w<16, 16>(a, xmap, ymap, p.smem, grid, st);
-  else if (g.Cin == 16 && g.Cout == 32) rc = launch_w<16, 32>(a, xmap, ymap, p.smem, grid, st);
-  else if (g.Cin == 32 && g.Cout == 16) rc = launch_w<32, 16>(a, xmap, ymap, p.smem, grid, st);
-  else rc = launch_w<32, 32>(a, xmap, ymap, p.smem, grid, st);
-  if (rc) return rc;
-  tcw::wgrad_tc_reduce_kernel<<<(9 * (g.Cin + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, grad);
-  CB_CUDA(cudaGetLastError());
+  for (int c_off = 0; c_off < g.Cin; c_off += cin_k) {
+    tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, p.stage_planes, use_tma ? 1 : 0, dy_rows,
+                       c_off, g.Cin, error_flag};
+    int rc;
+    if (cin_k == 16 && g.Cout == 16) rc = launch_w<16, 16>(a, xmap, ymap, p.smem, grid, st);
+    else if (cin_k == 16) rc = launch_w<16, 32>(a, xmap, ymap, p.smem, grid, st);
+    else if (g.Cout == 16) rc = launch_w<32, 16>(a, xmap, ymap, p.smem, grid, st);
+    else if (g.Cout == 32) rc = launch_w<32, 32>(a, xmap, ymap, p.smem, grid, st);
+    else rc = launch_w<32, 64>(a, xmap, ymap, p.smem, grid, st);
+    if (rc) return rc;
+    tcw::wgrad_tc_reduce_kernel<<<(9 * (cin_k + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, cin_k, c_off, grad);
+    CB_CUDA(cudaGetLastError());
+  }
   return CB_OK;
 }
 

@@ -323,3 +323,10 @@ def test_clip_rmsprop_parity(P):
     du_g, du_r = host(dth).astype(np.float64) - th, rth.astype(np.float64) - th
     assert (np.abs(du_g - du_r) <= 1e-4 * np.abs(du_r) + 1.2e-8).all()       # 1.2e-8: two ulps of a parameter of size 0.05-0.1 in fp32
     assert rel_l2(host(dth), rth) < 1e-6
+
+
+def test_learner_impala_wide_small():
+    """configs[4] at reduced size: the 32/64/64 network exercises the row-banded conv staging (64 channels at 42x42),
+    the 64-output weight gradients and the Cin = 64 gradients computed as two 32-channel launches."""
+    net, got, ref, ctx = _run_learner(synth.IMPALA_WIDE, "impala", "bf16", 2, 2, 1005, blobs=True, warm=True)
+    _check_learner(synth.IMPALA_WIDE, got, ref, ctx, "bf16", False)
