@@ -272,22 +272,24 @@ struct TcPlan { int G, npix_alloc, RB, nbands; size_t smem; };
 static TcPlan tc_plan(int H, int W, int cin, int cout) {
   const int Wp = W + 2, R = (H + 2) * Wp;
   const size_t wbytes = ((size_t)9 * cin * cout * 2 + 127) & ~(size_t)127;
-  const size_t budget = 72 * 1024;          // three CTAs per SM where the frame allows it
-  int G = (int)((budget > wbytes ? budget - wbytes : 0) / ((size_t)R * cin * 2));
-  if (G < 1) G = 1;
-  if (G > 8) G = 8;
-  int npix = ((G * R + 127) / 128) * 128 + 2 * Wp + 2;
-  npix = (npix + 7) / 8 * 8;
-  TcPlan p{G, npix, H, 1, wbytes + (size_t)npix * cin * 2};
-  if (p.smem > 200 * 1024) {      // a whole frame does not fit: row bands of RB rows (+2 halo rows), one frame at a time
-    const long avail = 200 * 1024 - (long)wbytes;
-    int rows = (int)(avail / ((long)cin * 2) - 2 * Wp - 136) / Wp - 2;
-    if (rows < 1) rows = 1;
-    p.nbands = (H + rows - 1) / rows; p.RB = (H + p.nbands - 1) / p.nbands; p.G = 1;
-    npix = (((p.RB + 2) * Wp + 127) / 128) * 128 + 2 * Wp + 2;
-    p.npix_alloc = (npix + 7) / 8 * 8;
-    p.smem = wbytes + (size_t)p.npix_alloc * cin * 2;
+  // shared-memory target per CTA: three CTAs per SM (72 KB) unless the weight image alone is large (two CTAs, 110 KB);
+  // co-resident CTAs overlap each other's staging / MMA / epilogue phases
+  const size_t budget = wbytes <= 40 * 1024 ? 72 * 1024 : 110 * 1024;
+  auto alloc_pix = [&](int positions) { int n = ((positions + 127) / 128) * 128 + 2 * Wp + 2; return (n + 7) / 8 * 8; };
+  TcPlan p;
+  p.G = (int)((budget - wbytes) / ((size_t)R * cin * 2)); if (p.G > 8) p.G = 8;
+  p.RB = H; p.nbands = 1;
+  while (p.G > 1 && wbytes + (size_t)alloc_pix(p.G * R) * cin * 2 > budget) --p.G;
+  if (p.G < 1 || wbytes + (size_t)alloc_pix(p.G * R) * cin * 2 > budget) {
+    p.G = 1;
+    if (wbytes + (size_t)alloc_pix(R) * cin * 2 > budget) {      // one frame is too big: row bands of RB rows (+2 halo rows)
+      long rows = ((long)(budget - wbytes) / ((long)cin * 2) - 2 * Wp - 140) / Wp - 2;
+      if (rows < 4) rows = 4;
+      p.nbands = (int)((H + rows - 1) / rows); p.RB = (H + p.nbands - 1) / p.nbands;
+    }
   }
+  p.npix_alloc = alloc_pix(p.nbands > 1 ? (p.RB + 2) * Wp : p.G * R);
+  p.smem = wbytes + (size_t)p.npix_alloc * cin * 2;
   return p;
 }
 
