@@ -157,6 +157,7 @@ int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* 
 // dense_tc.cu
 bool dense_tc_supported(const Geom& g);
 int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wf, const float* bias, bf16* out, bool relu_in, float* partial, int* error_flag, cudaStream_t st);
+int launch_dense_dgrad_tc(const Geom& g, int F, const bf16* dy, const bf16* wf, const bf16* mask, bf16* dx, int* error_flag, cudaStream_t st);
 int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* A, const bf16* dy, bool relu_in, float* grad, int* error_flag, cudaStream_t st);
 
 // rl.cu

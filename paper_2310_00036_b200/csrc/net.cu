@@ -348,6 +348,12 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         if (rc) return rc;
         continue;
       }
+      if (std::is_same<AT, bf16>::value && !L.f32_out && dense_tc_supported(g) && op.add < 0 && (g.H * g.W * g.Cin) % 16 == 0) {
+        int rc = launch_dense_dgrad_tc(g, F, (const bf16*)ws.grad[op.dy], (const bf16*)ws.wf + L.wf_off,
+                                       op.mask_t >= 0 ? (const bf16*)ws.act[op.mask_t] : nullptr, (bf16*)ws.grad[op.dx], ws.errflag, st);
+        if (rc) return rc;
+        continue;
+      }
       if (g.Ho == 1 && g.Wo == 1 && g.kh == g.H && g.kw == g.W && g.p == 0) {
         int Nf = g.H * g.W * g.Cin;
         DgradFullProblem<AT> pf{F, Nf, g.Cout, g.Cout, g.Cin, (const AT*)ws.grad[op.dy], (const AT*)ws.wd + L.wd_off,
