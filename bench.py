@@ -321,6 +321,13 @@ def main():
             dist.destroy_process_group()
         return
     peaks = load_peaks()
+    traffic = None      # dram bytes per launch of the dominant class from the committed `ncu --set full` summary (profiles/), if any
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")      # config,kernel_class,dram_bytes_per_launch (see profiles/traffic.md)
+    if os.path.exists(tpath):
+        for line in open(tpath).read().splitlines()[1:]:
+            f = line.split(",")
+            if len(f) == 3 and f[0] == str(args.config) and f[1] == dom["name"]:
+                traffic = float(f[2])
     bound = "tensor" if dom["flops"] > 0 else "hbm"
     per_launch_s = dom["ms"] / 1e3 / max(dom["launches"], 1)
     if bound == "tensor":
@@ -340,7 +347,7 @@ def main():
         "clocks": clk, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
         "roofline": {"bound": bound, "kernel": dom["name"], "achieved": achieved, "peak": peak, "unit": runit, "frac": achieved / peak,
-                     "traffic": None, "peak_source": f"{peaks['src']} ({'sustained bf16' if bound == 'tensor' else 'copy'})",
+                     "traffic": traffic, "peak_source": f"{peaks['src']} ({'sustained bf16' if bound == 'tensor' else 'copy'})",
                      "launches": dom["launches"], "ms_per_launch": 1e3 * per_launch_s, "share_of_step": dom["ms"] / (1e3 * t_local)},
         "kernel_breakdown_ms_per_step": {e["name"]: round(e["ms"], 4) for e in sorted(prof_all, key=lambda e: -e["ms"])},
         "kernel_breakdown_total_ms": total_ms, "loss": loss_last, "inference": inference,
