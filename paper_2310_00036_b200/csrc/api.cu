@@ -36,7 +36,7 @@ struct Builder {
     L.pm = {off, off + nw, 0, 0, cout};
     ptensor(name + ".w", off, {cout, C, kh, kw}, C * kh * kw); ptensor(name + ".b", off + nw, {cout}, C * kh * kw);
     off += nw + cout;
-    L.in_t = in; L.skip_t = skip; L.relu_in = relu_in; L.u8_in = in < 0; L.f32_out = false;
+    L.in_t = in; L.skip_t = skip; L.relu_in = relu_in; L.gate_in = relu_in; L.relu_out = false; L.u8_in = in < 0; L.f32_out = false;
     L.out_t = tensor((size_t)L.g.Ho * L.g.Wo * cout);
     L.wf_off = L.wd_off = net->wf_total; net->wf_total += (nw + 7) / 8 * 8;
     L.bias_off = net->bias_total; net->bias_total += (cout + 3) / 4 * 4;
@@ -49,7 +49,7 @@ struct Builder {
   void wgrad(int li, int dy) { net->bwd.push_back({OP_WGRAD, li, -1, -1, 0, 0, 0, dy, -1, -1, -1}); }
   void dgrad(int li, int dy, int dx, int add) {
     const Layer& L = net->layers[li];
-    net->bwd.push_back({OP_DGRAD, li, -1, -1, 0, 0, 0, dy, dx, L.relu_in ? L.in_t : -1, add});
+    net->bwd.push_back({OP_DGRAD, li, -1, -1, 0, 0, 0, dy, dx, L.gate_in ? L.in_t : -1, add});
     need(dx, (size_t)L.g.H * L.g.W * L.g.Cin); need(dy, (size_t)L.g.Ho * L.g.Wo * L.g.Cout);
   }
 };
@@ -80,6 +80,8 @@ static int build_program(cb_net* net) {
         st.l[2 * k] = b.conv(nm, p, a.channels[s], 3, 3, 1, 1, true, -1);
         snprintf(nm, sizeof nm, "stage%d.block%d.conv2", s, k);
         st.l[2 * k + 1] = b.conv(nm, net->layers[st.l[2 * k]].out_t, a.channels[s], 3, 3, 1, 1, true, p);
+        // h = conv1(relu(p)) is only ever consumed as relu(h): conv1 stores relu(h), conv2 loads it as is
+        net->layers[st.l[2 * k]].relu_out = true; net->layers[st.l[2 * k + 1]].relu_in = false;
         p = net->layers[st.l[2 * k + 1]].out_t;
       }
       b.cur = p; stages.push_back(st);
@@ -100,7 +102,7 @@ static int build_program(cb_net* net) {
     b.ptensor("pi.w", L.pm.w_off, {A, a.fc}, a.fc); b.ptensor("pi.b", L.pm.b_off, {A}, a.fc);
     b.ptensor("v.w", L.pm.w2_off, {1, a.fc}, a.fc); b.ptensor("v.b", L.pm.b2_off, {1}, a.fc);
     b.off = L.pm.b2_off + 1;
-    L.in_t = net->hid_t; L.skip_t = -1; L.relu_in = true; L.u8_in = false; L.f32_out = true;
+    L.in_t = net->hid_t; L.skip_t = -1; L.relu_in = true; L.gate_in = true; L.relu_out = false; L.u8_in = false; L.f32_out = true;
     L.out_t = b.tensor((size_t)A + 1, true);
     size_t nw = (size_t)(A + 1) * a.fc;
     L.wf_off = L.wd_off = net->wf_total; net->wf_total += (nw + 7) / 8 * 8;

@@ -43,7 +43,9 @@ struct Layer {
   Geom g;
   ParamMap pm;
   int in_t, out_t, skip_t;   // activation tensor ids (-1 = observations / none)
-  bool relu_in;              // the layer consumes relu(in)
+  bool relu_in;              // the layer applies ReLU to its input when loading it
+  bool gate_in;              // the input reaches the layer through a ReLU (applied here or stored by the producer): its sign gates dgrad
+  bool relu_out;             // the layer stores relu(output): every consumer reads it through a ReLU anyway (first conv of a residual block)
   bool u8_in;                // first layer: uint8 NCHW observations, scaled by 1/255 (O1)
   bool f32_out;              // heads: fp32 output in every mode
   size_t wf_off, wd_off, bias_off;   // offsets (elements) into the packed weight / bias buffers
@@ -136,7 +138,7 @@ int backward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx
 bool conv_tc_supported(const Geom& g);
 bool conv_tc_fits(int H, int W, int cin, int cout);
 int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16* in, const bf16* w, const float* bias, const bf16* aux0,
-                   const bf16* aux1, bf16* out, bool relu_in, int* error_flag, cudaStream_t st);
+                   const bf16* aux1, bf16* out, bool relu_in, bool relu_out, int* error_flag, cudaStream_t st);
 
 // wgrad_tc.cu
 bool wgrad_tc_supported(const Geom& g);

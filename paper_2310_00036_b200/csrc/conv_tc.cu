@@ -86,7 +86,7 @@ struct ConvTcArgs {
   const bf16* aux0;    // forward: skip tensor (added) | dgrad: pre-activation whose sign gates the result; nullable
   const bf16* aux1;    // dgrad: gradient added after gating; nullable
   bf16* out;           // [F, H, W, COUT]
-  int F, H, W, G, npix_alloc, relu_in, use_tma;
+  int F, H, W, G, npix_alloc, relu_in, use_tma, relu_out;
   int RB, nbands;      // rows per band (= H when the whole frame is staged) and bands per frame (banded: G = 1, TMA only)
   int* error_flag;
 };
@@ -229,6 +229,10 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, cons
 #pragma unroll
               for (int i = 0; i < 8; ++i) { v[i] += __bfloat162float(h0[i]); v[8 + i] += __bfloat162float(h1[i]); }
             }
+            if (a.relu_out) {
+#pragma unroll
+              for (int i = 0; i < 16; ++i) v[i] = fmaxf(v[i], 0.f);
+            }
           } else {
             if (a.aux0) {
               uint4 s0 = *reinterpret_cast<const uint4*>(a.aux0 + o + c0), s1 = *reinterpret_cast<const uint4*>(a.aux0 + o + c0 + 8);
@@ -321,14 +325,14 @@ static int dispatch(int cin, int cout, const tc::ConvTcArgs& a, const CUtensorMa
 
 // mode 0: forward (cin = g.Cin, cout = g.Cout);  mode 1: dgrad (cin = g.Cout, cout = g.Cin, weights packed flipped/transposed)
 int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16* in, const bf16* w, const float* bias, const bf16* aux0,
-                   const bf16* aux1, bf16* out, bool relu_in, int* error_flag, cudaStream_t st) {
+                   const bf16* aux1, bf16* out, bool relu_in, bool relu_out, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
   TcPlan p = tc_plan(H, W, cin, cout);
   if (p.smem > 220 * 1024) { set_error("conv_tc: frame does not fit shared memory"); return CB_EINVAL; }
   CUtensorMap tmap; memset(&tmap, 0, sizeof tmap);
   const bool use_tma = W + 2 <= 256 && p.RB + 2 <= 256 && tma::make_nhwc_map(&tmap, in, F, H, W, cin, W + 2, p.RB + 2, p.G);
   if (!use_tma && p.nbands > 1) { set_error("conv_tc: banded staging needs TMA"); return CB_EINVAL; }
-  tc::ConvTcArgs a{in, w, bias, aux0, aux1, out, F, H, W, p.G, p.npix_alloc, relu_in ? 1 : 0, use_tma ? 1 : 0, p.RB, p.nbands, error_flag};
+  tc::ConvTcArgs a{in, w, bias, aux0, aux1, out, F, H, W, p.G, p.npix_alloc, relu_in ? 1 : 0, use_tma ? 1 : 0, relu_out ? 1 : 0, p.RB, p.nbands, error_flag};
   int ngroups = ((F + p.G - 1) / p.G) * p.nbands;
   return mode == 0 ? dispatch<0>(cin, cout, a, tmap, p.smem, ngroups, st) : dispatch<1>(cin, cout, a, tmap, p.smem, ngroups, st);
 }

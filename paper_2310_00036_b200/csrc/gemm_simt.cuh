@@ -40,7 +40,7 @@ template <typename AT, typename OT, bool U8>
 struct FwdProblem {
   static constexpr bool A_K_FAST = true;
   int M, N, K, kchunk;
-  ConvInput<AT, U8> in; const AT* w; const float* bias; const AT* skip; OT* y; float in_scale;
+  ConvInput<AT, U8> in; const AT* w; const float* bias; const AT* skip; OT* y; float in_scale; bool relu_out;
   typedef Pix RowA; typedef Tap ColA;
   __device__ RowA rowA(int m) const { Pix r; r.ok = m < M; int q = in.g.Ho * in.g.Wo; r.f = m / q; int rem = m - r.f * q; r.oy = rem / in.g.Wo; r.ox = rem - r.oy * in.g.Wo; return r; }
   __device__ ColA colA(int k) const { Tap t; t.ok = k < K; t.c = k % in.g.Cin; int q = k / in.g.Cin; t.dj = q % in.g.kw; t.di = q / in.g.kw; return t; }
@@ -50,6 +50,7 @@ struct FwdProblem {
     float v = acc * in_scale + bias[n];
     size_t i = (size_t)m * N + n;
     if (skip) v += ldv(skip, i);
+    if (relu_out) v = fmaxf(v, 0.f);
     stv(y, i, v);
   }
 };

@@ -249,19 +249,19 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     int rc;
     if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out && conv_tc_fits(g.H, g.W, g.Cin, g.Cout)) {
       rc = launch_conv_tc(0, F, g.H, g.W, g.Cin, g.Cout, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (const bf16*)skip, nullptr,
-                          (bf16*)ws.act[L.out_t], L.relu_in, ws.errflag, st);
+                          (bf16*)ws.act[L.out_t], L.relu_in, L.relu_out, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
       rc = launch_dense_fwd_tc(g, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.wf + L.wf_off, bias, (bf16*)ws.act[L.out_t], L.relu_in, ws.partial, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(g)) {
       rc = launch_conv0_fwd(g, F, obs, frame_idx, ws.w0img, bias, (bf16*)ws.act[L.out_t], ws.errflag, st);
     } else if (L.u8_in) {
-      FwdProblem<AT, AT, true> p{M, N, K, K, {g, obs, frame_idx, false}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f / 255.0f};
+      FwdProblem<AT, AT, true> p{M, N, K, K, {g, obs, frame_idx, false}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f / 255.0f, L.relu_out};
       rc = launch_gemm(p, 1, st);
     } else if (L.f32_out) {
-      FwdProblem<AT, float, false> p{M, N, K, K, {g, ws.act[L.in_t], nullptr, L.relu_in}, wf, bias, skip, (float*)ws.act[L.out_t], 1.0f};
+      FwdProblem<AT, float, false> p{M, N, K, K, {g, ws.act[L.in_t], nullptr, L.relu_in}, wf, bias, skip, (float*)ws.act[L.out_t], 1.0f, L.relu_out};
       rc = launch_gemm(p, 1, st);
     } else {
-      FwdProblem<AT, AT, false> p{M, N, K, K, {g, ws.act[L.in_t], nullptr, L.relu_in}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f};
+      FwdProblem<AT, AT, false> p{M, N, K, K, {g, ws.act[L.in_t], nullptr, L.relu_in}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f, L.relu_out};
       rc = launch_gemm(p, 1, st);
     }
     if (rc) return rc;
@@ -344,7 +344,7 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
       if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && conv_tc_fits(g.H, g.W, g.Cout, g.Cin)) {
         int rc = launch_conv_tc(1, F, g.H, g.W, g.Cout, g.Cin, (const bf16*)ws.grad[op.dy], ws.wtc_d + L.wf_off, nullptr,
                                 op.mask_t >= 0 ? (const bf16*)ws.act[op.mask_t] : nullptr, op.add >= 0 ? (const bf16*)ws.grad[op.add] : nullptr,
-                                (bf16*)ws.grad[op.dx], false, ws.errflag, st);
+                                (bf16*)ws.grad[op.dx], false, false, ws.errflag, st);
         if (rc) return rc;
         continue;
       }
