@@ -191,14 +191,20 @@ __global__ void dense_reduce_kernel(const float* __restrict__ part, int S, int F
   }
 }
 
-// db[n] = sum_f dY[f][n], serial in f (fixed order), one thread per n
+// db[n] = sum_f dY[f][n]: 16 lanes per column, lane k sums frames [k*q, (k+1)*q) in order, then the 16 sums are added in
+// lane order (fixed association => reproducible)
 __global__ void colsum_kernel(const bf16* __restrict__ dy, int F, int N, float* __restrict__ out) {
-  int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n >= N) return;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x, n = t >> 4, part = t & 15;
+  const int q = (F + 15) / 16, f0 = part * q, f1 = min(F, f0 + q);
   float s = 0.f;
-#pragma unroll 16
-  for (int f = 0; f < F; ++f) s += __bfloat162float(dy[(size_t)f * N + n]);
-  out[n] = s;
+  if (n < N) {
+#pragma unroll 8
+    for (int f = f0; f < f1; ++f) s += __bfloat162float(dy[(size_t)f * N + n]);
+  }
+  float tot = s;
+#pragma unroll
+  for (int k = 1; k < 16; ++k) tot += __shfl_down_sync(0xffffffffu, s, k);
+  if (part == 0 && n < N) out[n] = tot;
 }
 
 }  // namespace dn
@@ -237,7 +243,7 @@ int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* 
   dn::Args a{A, dy, nullptr, nullptr, nullptr, grad, F, K, N, relu_in ? 1 : 0, nullptr, 1, g.H, g.W, g.Cin, pm.w_off, error_flag};
   int rc = launch_d<1, 64>(a, dim3((K + 127) / 128, (N + 63) / 64), st);
   if (rc) return rc;
-  dn::colsum_kernel<<<(N + 127) / 128, 128, 0, st>>>(dy, F, N, grad + pm.b_off);
+  dn::colsum_kernel<<<(16 * N + 255) / 256, 256, 0, st>>>(dy, F, N, grad + pm.b_off);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }

@@ -274,16 +274,25 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
 }
 
 // sums the per-CTA partials in CTA order and scatters to the canonical gradient
+// RL lanes per element: lane k adds the partials of CTAs [k*q, (k+1)*q) in order, then the RL sums are added in lane
+// order -- a fixed association, so the result is reproducible, with 1/RL of the dependent-load latency.
+constexpr int RL = 16;
 __global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nctas, Geom g, ParamMap pm, int cin_k, int c_off, float* __restrict__ grad) {
   const int rows = cin_k + 1, per = 9 * rows * g.Cout;      // cin_k = channels handled by the kernel launch that wrote `partial`
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < per; i += gridDim.x * blockDim.x) {
-    float s = 0.f;
-#pragma unroll 8
-    for (int z = 0; z < nctas; ++z) s += partial[(size_t)z * per + i];      // loads independent, adds in CTA order
-    int o = i % g.Cout, q = i / g.Cout, row = q % rows, tap = q / rows;
-    if (row == cin_k) { if (tap == 0 && c_off == 0) grad[pm.b(o)] = s; continue; }
-    grad[pm.w(o, c_off + row, tap / 3, tap % 3, g)] = s;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x, i = t / RL, part = t % RL;
+  const int q = (nctas + RL - 1) / RL, z0 = part * q, z1 = min(nctas, z0 + q);
+  float s = 0.f;
+  if (i < per) {
+#pragma unroll 10
+    for (int z = z0; z < z1; ++z) s += partial[(size_t)z * per + i];
   }
+  float tot = s;
+#pragma unroll
+  for (int k = 1; k < RL; ++k) tot += __shfl_down_sync(0xffffffffu, s, k);      // lane `part == 0` collects s_0 + s_1 + ... in order
+  if (part != 0 || i >= per) return;
+  int o = i % g.Cout, qq = i / g.Cout, row = qq % rows, tap = qq / rows;
+  if (row == cin_k) { if (tap == 0 && c_off == 0) grad[pm.b(o)] = tot; return; }
+  grad[pm.w(o, c_off + row, tap / 3, tap % 3, g)] = tot;
 }
 
 }  // namespace tcw
@@ -356,7 +365,7 @@ int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, con
     else if (g.Cout == 32) rc = launch_w<32, 32>(a, xmap, ymap, p.smem, grid, st);
     else rc = launch_w<32, 64>(a, xmap, ymap, p.smem, grid, st);
     if (rc) return rc;
-    tcw::wgrad_tc_reduce_kernel<<<(9 * (cin_k + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, cin_k, c_off, grad);
+    tcw::wgrad_tc_reduce_kernel<<<(tcw::RL * 9 * (cin_k + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, cin_k, c_off, grad);
     CB_CUDA(cudaGetLastError());
   }
   return CB_OK;
