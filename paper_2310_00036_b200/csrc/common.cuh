@@ -152,7 +152,7 @@ size_t conv0_partial_elems(const Geom& g);
 size_t conv0_wimg_elems(const Geom& g);
 int launch_conv0_pack(const Geom& g, const ParamMap& pm, const float* params, bf16* wimg, cudaStream_t st);
 int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* wimg, const float* bias, bf16* out,
-                     int* error_flag, cudaStream_t st);
+                     bf16* pool_out, uint8_t* pool_arg, int* error_flag, cudaStream_t st);
 int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, const uint8_t* pool_arg,
                        const bf16* dpool, float* partial, float* grad, int* error_flag, cudaStream_t st);
 

@@ -24,6 +24,7 @@ struct Args {
   const bf16* dy; float* partial;                 // wgrad: dy [F,H,W,COUT], partial [grid][3][24][COUT]
   const uint8_t* pool_arg; const bf16* dpool;     // wgrad, fused max-pool adjoint: dy is gathered from dpool [F,Ho,Wo,COUT] through pool_arg
   int F, H, W, CIN, R, nbands, npix_alloc, kext;
+  bf16* pool_out; uint8_t* pool_arg_out; int Rp;  // forward, fused 3x3 s2 SAME max-pool: pooled map + arg-max positions; Rp pooled rows per band
   int* error_flag;
 };
 
@@ -88,28 +89,34 @@ __device__ __forceinline__ uint4 pool_gather(const Args& a, int f, int y, int x,
 constexpr int TMEM_COLS = 256;
 
 template <int COUT>
-__global__ void __launch_bounds__(128) conv0_fwd_kernel(const Args a) {
+__global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr uint32_t W_BYTES = 6u * 2u * COUT * 16u;
   constexpr int TILES_PER_BATCH = TMEM_COLS / COUT;
   __shared__ __align__(8) uint64_t bar_storage;
   __shared__ uint32_t tmem_base_smem;
-  const int tid = threadIdx.x, warp = tid >> 5, Wp = a.W + 2;
+  const int tid = threadIdx.x, warp = tid >> 5, wg = warp >> 2, lane_row = tid & 127, Wp = a.W + 2;      // two warpgroups
   uint8_t* w_smem = smem; uint8_t* xs = smem + W_BYTES;
   const uint32_t bar = smem_u32(&bar_storage);
   if (tid == 0) mbar_init(bar, 1);
   if (warp == 0) tmem_alloc(smem_u32(&tmem_base_smem), TMEM_COLS);
-  for (uint32_t i = tid; i < W_BYTES / 16; i += 128) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w)[i];
-  for (int i = tid; i < a.npix_alloc; i += 128) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
+  for (uint32_t i = tid; i < W_BYTES / 16; i += 256) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w)[i];
+  for (int i = tid; i < a.npix_alloc; i += 256) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
   tc_fence_before(); __syncthreads(); tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem, idesc = make_idesc(128, COUT, 0, 0);
   const uint32_t a_base = smem_u32(xs), b_base = smem_u32(w_smem);
   uint32_t parity = 0;
   const int nitems = a.F * a.nbands;
   for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
-    const int f = item / a.nbands, yb = (item - f * a.nbands) * a.R;
+    const int f = item / a.nbands, band = item - f * a.nbands;
+    const bool fused = a.pool_out != nullptr;
+    const int Ho = (a.H + 1) / 2, Wo = (a.W + 1) / 2;
+    int th_ = (Ho - 1) * 2 + 3 - a.H; if (th_ < 0) th_ = 0; const int ph = th_ / 2;
+    int tw_ = (Wo - 1) * 2 + 3 - a.W; if (tw_ < 0) tw_ = 0; const int pw = tw_ / 2;
+    const int py0 = band * a.Rp;                                   // fused: first pooled row of the band
+    const int yb = fused ? max(0, 2 * py0 - ph) : band * a.R;      // first conv row computed by this item
     const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
-    stage_band(a, xs, fr, yb, tid);
+    stage_band(a, xs, fr, yb, tid, 256);
     fence_async_smem();
     __syncthreads();
     const int ntiles = (a.R * Wp + 127) / 128;
@@ -132,14 +139,14 @@ __global__ void __launch_bounds__(128) conv0_fwd_kernel(const Args a) {
       if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 3; }
       parity ^= 1;
       tc_fence_after();
-      for (int s = 0; s < nt; ++s) {
-        const int q = (t0 + s) * 128 + tid, yl = q / Wp, x = q - yl * Wp, y = yb + yl;
+      for (int s = wg; s < nt; s += 2) {      // each warpgroup drains every second accumulator tile
+        const int q = (t0 + s) * 128 + lane_row, yl = q / Wp, x = q - yl * Wp, y = yb + yl;
         const bool valid = yl < a.R && y < a.H && x < a.W;
         const size_t o = (((size_t)f * a.H + y) * a.W + x) * COUT;
 #pragma unroll
         for (int c0 = 0; c0 < COUT; c0 += 16) {
           float v[16];
-          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(s * COUT + c0), v);
+          tmem_ld16(tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(s * COUT + c0), v);
           if (!valid) continue;
           uint4 o0, o1;
           __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
@@ -147,12 +154,50 @@ __global__ void __launch_bounds__(128) conv0_fwd_kernel(const Args a) {
           for (int i = 0; i < 16; ++i) v[i] = fmaf(v[i], 1.0f / 255.0f, a.bias[c0 + i]);
 #pragma unroll
           for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
-          *reinterpret_cast<uint4*>(a.out + o + c0) = o0;
-          *reinterpret_cast<uint4*>(a.out + o + c0 + 8) = o1;
+          if (fused) {      // keep the band of conv outputs (already rounded to bf16, as the unfused path stores them) in shared memory
+            bf16* ct = reinterpret_cast<bf16*>(xs + (size_t)a.npix_alloc * 16) + ((size_t)yl * a.W + x) * COUT + c0;
+            *reinterpret_cast<uint4*>(ct) = o0; *reinterpret_cast<uint4*>(ct + 8) = o1;
+          } else {
+            *reinterpret_cast<uint4*>(a.out + o + c0) = o0;
+            *reinterpret_cast<uint4*>(a.out + o + c0 + 8) = o1;
+          }
         }
       }
       tc_fence_before();
       __syncthreads();
+    }
+    if (fused) {
+      // ---- max-pool 3x3 stride 2 SAME (A10) over the band; first maximum in row-major window order (A11) ----
+      const bf16* ct = reinterpret_cast<const bf16*>(xs + (size_t)a.npix_alloc * 16);
+      constexpr int C8 = COUT / 8;
+      const int pr = min(a.Rp, Ho - py0);
+      for (int i = tid; i < pr * Wo * C8; i += 256) {
+        const int c8 = i % C8, q = i / C8, ox = q % Wo, oy = py0 + q / Wo;
+        float best[8]; uint32_t bk[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { best[k] = -INFINITY; bk[k] = 15; }
+        for (int di = 0; di < 3; ++di) {
+          const int iy = oy * 2 + di - ph; if ((unsigned)iy >= (unsigned)a.H) continue;
+          for (int dj = 0; dj < 3; ++dj) {
+            const int ix = ox * 2 + dj - pw; if ((unsigned)ix >= (unsigned)a.W) continue;
+            const uint4 u = *reinterpret_cast<const uint4*>(ct + ((size_t)(iy - yb) * a.W + ix) * COUT + c8 * 8);
+            const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&u);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              const float2 t = __bfloat1622float2(h[k]);
+              if (t.x > best[2 * k]) { best[2 * k] = t.x; bk[2 * k] = (uint32_t)(di * 3 + dj); }
+              if (t.y > best[2 * k + 1]) { best[2 * k + 1] = t.y; bk[2 * k + 1] = (uint32_t)(di * 3 + dj); }
+            }
+          }
+        }
+        const size_t o = (((size_t)f * Ho + oy) * Wo + ox) * COUT + c8 * 8;
+        uint4 r; __nv_bfloat162* o2 = reinterpret_cast<__nv_bfloat162*>(&r);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) o2[k] = __floats2bfloat162_rn(best[2 * k], best[2 * k + 1]);
+        *reinterpret_cast<uint4*>(a.pool_out + o) = r;
+        uint2 pk; pk.x = bk[0] | (bk[1] << 8) | (bk[2] << 16) | (bk[3] << 24); pk.y = bk[4] | (bk[5] << 8) | (bk[6] << 16) | (bk[7] << 24);
+        *reinterpret_cast<uint2*>(a.pool_arg_out + o) = pk;
+      }
     }
   }
   tc_fence_before(); __syncthreads();
@@ -299,18 +344,26 @@ static int set_smem(K kernel, size_t smem, size_t* configured) {
 }
 
 int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* wimg, const float* bias, bf16* out,
-                     int* error_flag, cudaStream_t st) {
+                     bf16* pool_out, uint8_t* pool_arg, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
   const int Wp = g.W + 2;
-  int R = std::min(g.H, (90 * 1024 / 16 - 2 * Wp - 130) / Wp - 2); if (R < 1) R = 1;
-  const int nb = (g.H + R - 1) / R; R = (g.H + nb - 1) / nb;
+  int R, nb, Rp = 0; size_t ctile = 0;
+  if (pool_out) {      // fused max-pool: a band of Rp pooled rows needs 2 Rp + 1 conv rows, kept in shared memory as bf16
+    const int Ho = (g.H + 1) / 2;
+    Rp = g.Cout == 16 ? 10 : 5; if (Rp > Ho) Rp = Ho;
+    R = 2 * Rp + 1; nb = (Ho + Rp - 1) / Rp;
+    ctile = (size_t)R * g.W * g.Cout * 2;
+  } else {
+    R = std::min(g.H, (90 * 1024 / 16 - 2 * Wp - 130) / Wp - 2); if (R < 1) R = 1;
+    nb = (g.H + R - 1) / R; R = (g.H + nb - 1) / nb;
+  }
   const int npix = ((R * Wp + 127) / 128) * 128 + 2 * Wp + 8;
-  const size_t smem = (size_t)6 * 2 * g.Cout * 16 + (size_t)npix * 16;
-  tc0::Args a{obs, frame_idx, wimg, bias, out, nullptr, nullptr, nullptr, nullptr, F, g.H, g.W, g.Cin, R, nb, npix, 0, error_flag};
+  const size_t smem = (size_t)6 * 2 * g.Cout * 16 + (size_t)npix * 16 + ctile;
+  tc0::Args a{obs, frame_idx, wimg, bias, out, nullptr, nullptr, nullptr, nullptr, F, g.H, g.W, g.Cin, R, nb, npix, 0, pool_out, pool_arg, Rp, error_flag};
   const int grid = std::min(F * nb, 296);
   static size_t c16 = 0, c32 = 0; int rc;
-  if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_fwd_kernel<16>, smem, &c16))) return rc; tc0::conv0_fwd_kernel<16><<<grid, 128, smem, st>>>(a); }
-  else { if ((rc = set_smem(tc0::conv0_fwd_kernel<32>, smem, &c32))) return rc; tc0::conv0_fwd_kernel<32><<<grid, 128, smem, st>>>(a); }
+  if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_fwd_kernel<16>, smem, &c16))) return rc; tc0::conv0_fwd_kernel<16><<<grid, 256, smem, st>>>(a); }
+  else { if ((rc = set_smem(tc0::conv0_fwd_kernel<32>, smem, &c32))) return rc; tc0::conv0_fwd_kernel<32><<<grid, 256, smem, st>>>(a); }
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
@@ -326,7 +379,7 @@ int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* 
   const int npix = (kext + 2 * Wp + 40 + 7) / 8 * 8;
   const size_t smem = (size_t)2 * (1 + ych) * npix * 16;
   const int grid = std::min(F * nb, CONV0_MAX_CTAS);
-  tc0::Args a{obs, frame_idx, nullptr, nullptr, nullptr, dy, partial, pool_arg, dpool, F, g.H, g.W, g.Cin, R, nb, npix, kext, error_flag};
+  tc0::Args a{obs, frame_idx, nullptr, nullptr, nullptr, dy, partial, pool_arg, dpool, F, g.H, g.W, g.Cin, R, nb, npix, kext, nullptr, nullptr, 0, error_flag};
   static size_t c16 = 0, c32 = 0; int rc;
   if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_wgrad_kernel<16>, smem, &c16))) return rc; tc0::conv0_wgrad_kernel<16><<<grid, tc0::WNLOAD + 32, smem, st>>>(a); }
   else { if ((rc = set_smem(tc0::conv0_wgrad_kernel<32>, smem, &c32))) return rc; tc0::conv0_wgrad_kernel<32><<<grid, tc0::WNLOAD + 32, smem, st>>>(a); }

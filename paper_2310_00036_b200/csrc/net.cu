@@ -227,8 +227,11 @@ static inline int grid_for(size_t total) { return (int)std::min<size_t>((total +
 
 template <typename AT>
 static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads) {
-  for (const Op& op : net->fwd) {
+  bool pool_fused = false;      // the first layer's kernel also produced the pooled map: skip the following POOL op
+  for (size_t oi = 0; oi < net->fwd.size(); ++oi) {
+    const Op& op = net->fwd[oi];
     if (skip_heads && op.kind == OP_CONV && net->layers[op.layer].f32_out) continue;
+    if (op.kind == OP_POOL && pool_fused) { pool_fused = false; continue; }
     if (op.kind == OP_POOL) {
       size_t total = (size_t)F * pool_out(op.H) * pool_out(op.W) * op.C;
       ProfScope ps(K_POOL_FWD, st, 1, 0.0, (double)sizeof(AT) * (total + (double)F * op.H * op.W * op.C));
@@ -253,7 +256,10 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     } else if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
       rc = launch_dense_fwd_tc(g, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.wf + L.wf_off, bias, (bf16*)ws.act[L.out_t], L.relu_in, ws.partial, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(g)) {
-      rc = launch_conv0_fwd(g, F, obs, frame_idx, ws.w0img, bias, (bf16*)ws.act[L.out_t], ws.errflag, st);
+      const Op* nx = oi + 1 < net->fwd.size() ? &net->fwd[oi + 1] : nullptr;
+      pool_fused = nx && nx->kind == OP_POOL && nx->in_t == L.out_t && nx->C % 8 == 0 && g.W % 2 == 0;
+      rc = launch_conv0_fwd(g, F, obs, frame_idx, ws.w0img, bias, (bf16*)ws.act[L.out_t], pool_fused ? (bf16*)ws.act[nx->out_t] : nullptr,
+                            pool_fused ? (uint8_t*)ws.act[nx->mask_t] : nullptr, ws.errflag, st);
     } else if (L.u8_in) {
       FwdProblem<AT, AT, true> p{M, N, K, K, {g, obs, frame_idx, false}, wf, bias, skip, (AT*)ws.act[L.out_t], 1.0f / 255.0f, L.relu_out};
       rc = launch_gemm(p, 1, st);
