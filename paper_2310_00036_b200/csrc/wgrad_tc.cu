@@ -118,9 +118,10 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
   const int ngroups = (a.F + a.G - 1) / a.G, nitems = ngroups * a.nbands;
   const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
+  const bool direct = a.use_tma && !a.relu_in;      // nothing to do between the TMA landing and the MMAs: the issuer waits on raw[] itself
   if (warp < NLOAD / 32) {
     // ================= loaders =================
-    for (int it = 0; it < my_items; ++it) {
+    for (int it = 0; it < (direct ? 0 : my_items); ++it) {
       const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
       if (!a.use_tma && use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 2; }
       uint8_t* xs = smem + (size_t)s * stage_bytes;
@@ -251,7 +252,7 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
     uint32_t accumulate = 0;
     for (int it = 0; it < my_items; ++it) {
       const int s = it & 1, use = it >> 1;
-      if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
+      if (!mbar_wait(bar0 + 8u * (direct ? 5 + s : s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
       asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
       const uint32_t x_base = smem_u32(smem + (size_t)s * stage_bytes), y_base = x_base + (uint32_t)(XPL + 1) * P;
       for (int k0 = 0; k0 < a.kext; k0 += 16) {
