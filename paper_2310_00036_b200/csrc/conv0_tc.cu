@@ -52,38 +52,54 @@ __device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr
   }
 }
 
-// adjoint of the 3x3 stride-2 SAME max-pool, gather form, evaluated while staging dy: conv-output pixel (y,x)
-// receives dpool of every window (<= 4) whose stored arg-max position is this pixel (A11); sums in fp32, in
-// window order, then rounds to bf16 exactly like the stand-alone pool_bwd_v8_kernel.
-__device__ __forceinline__ uint4 pool_gather(const Args& a, int f, int y, int x, int ch, int cout) {
-  const int Ho = (a.H + 1) / 2, Wo = (a.W + 1) / 2;
-  int th = (Ho - 1) * 2 + 3 - a.H; if (th < 0) th = 0; const int ph = th / 2;
-  int tw = (Wo - 1) * 2 + 3 - a.W; if (tw < 0) tw = 0; const int pw = tw / 2;
-  float g[8];
+// adjoint of the 3x3 stride-2 SAME max-pool, scatter form, evaluated while staging dy (A11): every pooled
+// element adds its gradient to the conv-output pixel its stored arg-max names.  Windows whose (oy, ox)
+// parities agree are disjoint (stride 4 between them, width 3), so the four parity classes are applied as
+// four barrier-separated phases of plain shared-memory read-modify-writes: no atomics, fixed order,
+// bitwise reproducible.  A pixel elected by several windows is rounded to bf16 after each addition.
+struct PoolGeom { int Ho, Wo, ph, pw, oy_lo, noy[2], nox[2]; };
+__device__ __forceinline__ PoolGeom pool_geom(const Args& a, int yb) {
+  PoolGeom q; q.Ho = (a.H + 1) / 2; q.Wo = (a.W + 1) / 2;
+  int th = (q.Ho - 1) * 2 + 3 - a.H; if (th < 0) th = 0; q.ph = th / 2;
+  int tw = (q.Wo - 1) * 2 + 3 - a.W; if (tw < 0) tw = 0; q.pw = tw / 2;
+  int lo = yb + q.ph - 2; lo = lo <= 0 ? 0 : (lo + 1) / 2;
+  const int yend = min(yb + a.R, a.H) - 1;
+  const int hi = min((yend + q.ph) / 2, q.Ho - 1);
+  q.oy_lo = lo;
+  for (int par = 0; par < 2; ++par) {
+    const int first = lo + (((lo & 1) != par) ? 1 : 0);
+    q.noy[par] = hi >= first ? (hi - first) / 2 + 1 : 0;
+    q.nox[par] = (q.Wo - par + 1) / 2;
+  }
+  return q;
+}
+// item i of phase p -> (oy, ox, ch); returns false past the end
+__device__ __forceinline__ bool pool_item(const PoolGeom& q, int p, int i, int ych, int& oy, int& ox, int& ch) {
+  const int pa = p >> 1, pb = p & 1, n = q.noy[pa] * q.nox[pb] * ych;
+  if (i >= n) return false;
+  ch = i % ych; const int r = i / ych; const int ix = r % q.nox[pb], iy = r / q.nox[pb];
+  const int first = q.oy_lo + (((q.oy_lo & 1) != pa) ? 1 : 0);
+  oy = first + 2 * iy; ox = pb + 2 * ix;
+  return true;
+}
+__device__ __forceinline__ void pool_scatter(const Args& a, const PoolGeom& q, uint8_t* ys, uint32_t P, int yb, int oy, int ox, int ch,
+                                             uint2 pk, uint4 dv) {
+  const int Wp = a.W + 2, rows = min(a.R, a.H - yb);
+  const int y0 = oy * 2 - q.ph - yb, x0 = ox * 2 - q.pw;
+  uint8_t* base = ys + (size_t)ch * P;
+  const uint16_t* h = reinterpret_cast<const uint16_t*>(&dv);
 #pragma unroll
-  for (int k = 0; k < 8; ++k) g[k] = 0.f;
-  int oy_lo = (y + ph - 2 + 1) / 2; if (y + ph - 2 < 0) oy_lo = 0;
-  int ox_lo = (x + pw - 2 + 1) / 2; if (x + pw - 2 < 0) ox_lo = 0;
-  const int oy_hi = min((y + ph) / 2, Ho - 1), ox_hi = min((x + pw) / 2, Wo - 1);
-  for (int oy = oy_lo; oy <= oy_hi; ++oy)
-    for (int ox = ox_lo; ox <= ox_hi; ++ox) {
-      const uint32_t me = (uint32_t)((y - (oy * 2 - ph)) * 3 + (x - (ox * 2 - pw)));
-      const size_t o = (((size_t)f * Ho + oy) * Wo + ox) * cout + ch * 8;
-      const uint2 pk = *reinterpret_cast<const uint2*>(a.pool_arg + o);
-      const uint4 dv = *reinterpret_cast<const uint4*>(a.dpool + o);
-      const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&dv);
-#pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const float2 t = __bfloat1622float2(h[k]);
-        const uint32_t w = k < 2 ? pk.x : pk.y; const int sh = (k & 1) * 16;
-        if (((w >> sh) & 255u) == me) g[2 * k] += t.x;
-        if (((w >> (sh + 8)) & 255u) == me) g[2 * k + 1] += t.y;
-      }
+  for (int k = 0; k < 8; ++k) {
+    const uint32_t arg = ((k < 4 ? pk.x : pk.y) >> (8 * (k & 3))) & 255u;
+    const int wy = (int)((arg * 11u) >> 5), wx = (int)arg - 3 * wy;
+    const int yl = y0 + wy;
+    if ((unsigned)yl < (unsigned)rows) {
+      uint16_t* p = reinterpret_cast<uint16_t*>(base + (size_t)(yl * Wp + x0 + wx) * 16) + k;
+      const float o = __uint_as_float((uint32_t)(*p) << 16), t = __uint_as_float((uint32_t)h[k] << 16);
+      const __nv_bfloat16 r = __float2bfloat16_rn(o + t);
+      *p = *reinterpret_cast<const uint16_t*>(&r);
     }
-  uint4 r; __nv_bfloat162* o2 = reinterpret_cast<__nv_bfloat162*>(&r);
-#pragma unroll
-  for (int k = 0; k < 4; ++k) o2[k] = __floats2bfloat162_rn(g[2 * k], g[2 * k + 1]);
-  return r;
+  }
 }
 
 constexpr int TMEM_COLS = 256;
@@ -122,19 +138,22 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
     const int ntiles = (a.R * Wp + 127) / 128;
     for (int t0 = 0; t0 < ntiles; t0 += TILES_PER_BATCH) {
       const int nt = min(TILES_PER_BATCH, ntiles - t0);
-      if (tid == 0) {
+      if (warp == 0) {        // the whole warp runs the loop, one elected lane issues
         tc_fence_after();
+        const uint32_t a_lo = ((a_base >> 4) & 0x3FFFu) | (1u << 16), a_hi = 8u | (1u << 14);               // LBO 16 B, SBO 128 B
+        const uint32_t b_lo = ((b_base >> 4) & 0x3FFFu) | ((uint32_t)COUT << 16), b_hi = 8u | (1u << 14);   // LBO COUT*16 B, SBO 128 B
         for (int s = 0; s < nt; ++s) {
           const uint32_t q0 = (uint32_t)(t0 + s) * 128u;
 #pragma unroll
           for (int slot = 0; slot < 6; ++slot) {
             const uint32_t shift = (uint32_t)((slot >> 1) * Wp + (slot & 1) * 2);
-            uint64_t ad = make_desc(a_base + (q0 + shift) * 16u, 16u, 128u);
-            uint64_t bd = make_desc(b_base + (uint32_t)slot * 2u * COUT * 16u, (uint32_t)COUT * 16u, 128u);
-            mma_f16(tmem_base + (uint32_t)(s * COUT), ad, bd, idesc, slot ? 1u : 0u);
+            const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(a_lo + q0 + shift);
+            const uint64_t bd = ((uint64_t)b_hi << 32) | (uint64_t)(b_lo + (uint32_t)slot * 2u * COUT);
+            if (elect_one()) mma_f16(tmem_base + (uint32_t)(s * COUT), ad, bd, idesc, slot ? 1u : 0u);
           }
         }
-        mma_commit(bar);
+        if (elect_one()) mma_commit(bar);
+        __syncwarp();
       }
       if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 3; }
       parity ^= 1;
@@ -240,19 +259,44 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
   if (warp < WNLOAD / 32) {
     for (int it = 0; it < my_items; ++it) {
       const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
+      const int f = item / a.nbands, yb = (item - f * a.nbands) * a.R;
+      // the pooled gradients of this thread's first item of each phase are fetched before anything waits
+      PoolGeom q; bool pf_ok[4] = {false, false, false, false}; int pf_oy[4], pf_ox[4], pf_ch[4]; uint2 pf_pk[4]; uint4 pf_dv[4];
+      if (a.pool_arg != nullptr) {
+        q = pool_geom(a, yb);
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+          pf_ok[p] = pool_item(q, p, tid, YCH, pf_oy[p], pf_ox[p], pf_ch[p]);
+          if (pf_ok[p]) {
+            const size_t o = (((size_t)f * q.Ho + pf_oy[p]) * q.Wo + pf_ox[p]) * COUT + pf_ch[p] * 8;
+            pf_pk[p] = *reinterpret_cast<const uint2*>(a.pool_arg + o); pf_dv[p] = *reinterpret_cast<const uint4*>(a.dpool + o);
+          }
+        }
+      }
       if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 4; }
       uint8_t* xs = smem + (size_t)s * STAGE; uint8_t* ys = xs + P;
-      const int f = item / a.nbands, yb = (item - f * a.nbands) * a.R;
       const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
       stage_band(a, xs, fr, yb, tid, WNLOAD);
-      for (int i = tid; i < a.kext * YCH; i += WNLOAD) {
-        int ch = i % YCH, pos = i / YCH, yl = pos / Wp, x = pos - yl * Wp, y = yb + yl;
-        uint4 v = make_uint4(0, 0, 0, 0);
-        if (yl < a.R && y < a.H && x < a.W) {
-          if (a.pool_arg == nullptr) v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)f * a.H + y) * a.W + x) * COUT + ch * 8);
-          else v = pool_gather(a, f, y, x, ch, COUT);
+      if (a.pool_arg == nullptr) {
+        for (int i = tid; i < a.kext * YCH; i += WNLOAD) {
+          int ch = i % YCH, pos = i / YCH, yl = pos / Wp, x = pos - yl * Wp, y = yb + yl;
+          uint4 v = make_uint4(0, 0, 0, 0);
+          if (yl < a.R && y < a.H && x < a.W) v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)f * a.H + y) * a.W + x) * COUT + ch * 8);
+          *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
         }
-        *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
+      } else {
+        for (int i = tid; i < a.kext * YCH; i += WNLOAD)
+          *reinterpret_cast<uint4*>(ys + (size_t)(i % YCH) * P + (size_t)(i / YCH) * 16) = make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+          asm volatile("bar.sync 1, %0;\n" :: "n"(WNLOAD) : "memory");
+          if (pf_ok[p]) pool_scatter(a, q, ys, P, yb, pf_oy[p], pf_ox[p], pf_ch[p], pf_pk[p], pf_dv[p]);
+          for (int i = tid + WNLOAD; ; i += WNLOAD) {
+            int oy, ox, ch; if (!pool_item(q, p, i, YCH, oy, ox, ch)) break;
+            const size_t o = (((size_t)f * q.Ho + oy) * q.Wo + ox) * COUT + ch * 8;
+            pool_scatter(a, q, ys, P, yb, oy, ox, ch, *reinterpret_cast<const uint2*>(a.pool_arg + o), *reinterpret_cast<const uint4*>(a.dpool + o));
+          }
+        }
       }
       fence_async_smem();
       asm volatile("bar.sync 1, %0;\n" :: "n"(WNLOAD) : "memory");
@@ -275,26 +319,30 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
         }
       }
     }
-  } else if (tid == WNLOAD) {
+  } else {      // warp WNLOAD / 32: the whole warp runs the loop, one elected lane issues
     const uint32_t idesc = make_idesc(64, COUT, 1, 1);
+    const uint32_t a_hi = 1u | (1u << 14), b_hi = ((P >> 4) & 0x3FFFu) | (1u << 14);     // A: SBO = 16 B (M walk); B: SBO = plane
     uint32_t accumulate = 0;
     for (int it = 0; it < my_items; ++it) {
       const int s = it & 1, use = it >> 1;
       if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 4; }
       tc_fence_after();
       const uint32_t x_base = smem_u32(smem + (size_t)s * STAGE), y_base = x_base + P;
+      const uint32_t x_lo = ((x_base >> 4) & 0x3FFFu) | (8u << 16), y_lo = ((y_base >> 4) & 0x3FFFu) | (8u << 16);
       for (int k0 = 0; k0 < a.kext; k0 += 16) {
-        const uint64_t bd = make_desc(y_base + (uint32_t)k0 * 16u, 128u, P);
+        const uint64_t bd = ((uint64_t)b_hi << 32) | (uint64_t)(y_lo + (uint32_t)k0);
 #pragma unroll
         for (int di = 0; di < 3; ++di) {
-          const uint64_t ad = make_desc(x_base + (uint32_t)(k0 + di * Wp) * 16u, 128u, 16u);
-          mma_f16(tmem_base + (uint32_t)(di * COUT), ad, bd, idesc, accumulate);
+          const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(x_lo + (uint32_t)(k0 + di * Wp));
+          if (elect_one()) mma_f16(tmem_base + (uint32_t)(di * COUT), ad, bd, idesc, accumulate);
         }
         accumulate = 1;
       }
-      mma_commit(bar0 + 8u * (2 + s));
+      if (elect_one()) mma_commit(bar0 + 8u * (2 + s));
+      __syncwarp();
     }
-    mma_commit(bar0 + 8u * 4);
+    if (elect_one()) mma_commit(bar0 + 8u * 4);
+    __syncwarp();
   }
   tc_fence_before(); __syncthreads();
   if (warp == WNLOAD / 32) tmem_dealloc(tmem_base, TCOLS);

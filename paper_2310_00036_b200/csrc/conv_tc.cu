@@ -40,6 +40,12 @@ __device__ __forceinline__ void mma_f16(uint32_t tmem_d, uint64_t adesc, uint64_
   asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
                :: "r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
+// one lane of a converged warp: tcgen05 instructions then issue from the uniform datapath (see tc_ptx.cuh)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred = 0;
+  asm volatile("{\n\t.reg .b32 rx;\n\t.reg .pred px;\n\telect.sync rx|px, %1;\n\t@px mov.s32 %0, 1;\n\t}\n" : "+r"(pred) : "r"(0xFFFFFFFFu));
+  return pred != 0;
+}
 __device__ __forceinline__ void mma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" :: "r"(bar) : "memory");
 }
@@ -186,24 +192,25 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, cons
     const int ntiles = ((nf - 1) * R + a.RB * Wp + 127) / 128;      // positions up to the last computed row of the last frame
     for (int t0 = 0; t0 < ntiles; t0 += TILES_PER_BATCH) {
       const int nt = min(TILES_PER_BATCH, ntiles - t0);
-      if (tid == 0) {
+      if (tid < 32) {        // the whole warp runs the loop, one elected lane issues
         tc_fence_after();
+        const uint32_t a_lo = ((a_base >> 4) & 0x3FFFu) | (((plane_bytes >> 4) & 0x3FFFu) << 16), d_hi = 8u | (1u << 14);   // LBO = plane, SBO = 128 B
+        const uint32_t b_lo = ((b_base >> 4) & 0x3FFFu) | ((uint32_t)COUT << 16);                                        // LBO = COUT*16 B
         for (int s = 0; s < nt; ++s) {
           const uint32_t q0 = (uint32_t)(t0 + s) * 128u;
-          uint32_t first = 1;
 #pragma unroll
           for (int tap = 0; tap < 9; ++tap) {
             const uint32_t shift = (uint32_t)((tap / 3) * Wp + (tap % 3));
 #pragma unroll
             for (int ks = 0; ks < KSTEPS; ++ks) {
-              uint64_t ad = make_desc(a_base + (q0 + shift) * 16u + (uint32_t)(2 * ks) * plane_bytes, plane_bytes, 128u);
-              uint64_t bd = make_desc(b_base + (uint32_t)((tap * NCH + 2 * ks) * COUT) * 16u, (uint32_t)COUT * 16u, 128u);
-              mma_f16(tmem_base + (uint32_t)(s * COUT), ad, bd, idesc, first ? 0u : 1u);
-              first = 0;
+              const uint64_t ad = ((uint64_t)d_hi << 32) | (uint64_t)(a_lo + q0 + shift + (uint32_t)(2 * ks) * (plane_bytes >> 4));
+              const uint64_t bd = ((uint64_t)d_hi << 32) | (uint64_t)(b_lo + (uint32_t)((tap * NCH + 2 * ks) * COUT));
+              if (elect_one()) mma_f16(tmem_base + (uint32_t)(s * COUT), ad, bd, idesc, (tap | ks) ? 1u : 0u);
             }
           }
         }
-        mma_commit(bar);
+        if (elect_one()) mma_commit(bar);
+        __syncwarp();
       }
       if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 1; }
       parity ^= 1;

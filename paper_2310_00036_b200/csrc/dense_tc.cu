@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(NLOAD + 32) dense_tc_kernel(const Args a) {
         }
       }
     }
-  } else if (tid == NLOAD) {
+  } else {      // warp NLOAD / 32: the whole warp runs the loop, one elected lane issues
     const uint32_t idesc = make_idesc(128, BN, MODE == 1 ? 1 : 0, MODE == 2 ? 0 : 1);
     for (int t = 0; t < ntiles; ++t) {
       const int s = t % NSTAGE, use = t / NSTAGE;
@@ -171,11 +171,13 @@ __global__ void __launch_bounds__(NLOAD + 32) dense_tc_kernel(const Args a) {
       for (int ks = 0; ks < BK / 16; ++ks) {
         const uint64_t ad = MODE != 1 ? make_desc(ab + (uint32_t)(2 * ks) * PA, PA, 128u) : make_desc(ab + (uint32_t)ks * 256u, 128u, PA);
         const uint64_t bd = MODE == 2 ? make_desc(bb + (uint32_t)(2 * ks) * PBK, PBK, 128u) : make_desc(bb + (uint32_t)ks * 256u, 128u, PB);
-        mma_f16(tmem_base, ad, bd, idesc, (t | ks) ? 1u : 0u);
+        if (elect_one()) mma_f16(tmem_base, ad, bd, idesc, (t | ks) ? 1u : 0u);
       }
-      mma_commit(bar0 + 8u * (NSTAGE + s));
+      if (elect_one()) mma_commit(bar0 + 8u * (NSTAGE + s));
+      __syncwarp();
     }
-    if (ntiles > 0) mma_commit(bar0 + 8u * (2 * NSTAGE));
+    if (ntiles > 0 && elect_one()) mma_commit(bar0 + 8u * (2 * NSTAGE));
+    __syncwarp();
   }
   tc_fence_before(); __syncthreads();
   if (warp == NLOAD / 32) tmem_dealloc(tmem_base, TCOLS);

@@ -35,6 +35,13 @@ __device__ __forceinline__ void mma_f16(uint32_t tmem_d, uint64_t adesc, uint64_
   asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
                :: "r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
 }
+// one lane of a converged warp; the compiler then issues the tcgen05 instruction from the uniform datapath
+// instead of looping over the active lanes of a divergent branch (which costs ~50 clk per MMA)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred = 0;
+  asm volatile("{\n\t.reg .b32 rx;\n\t.reg .pred px;\n\telect.sync rx|px, %1;\n\t@px mov.s32 %0, 1;\n\t}\n" : "+r"(pred) : "r"(0xFFFFFFFFu));
+  return pred != 0;
+}
 __device__ __forceinline__ void mma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" :: "r"(bar) : "memory");
 }
@@ -246,28 +253,32 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
         for (int ch = 0; ch < YCH; ++ch) tma::load_4d(ys + (uint32_t)ch * P, &ymap, ch * 8, 0, yb, f0, rb);
       }
     }
-  } else if (tid == NLOAD) {
-    // ================= MMA issuer =================
+  } else if (warp == NLOAD / 32) {
+    // ================= MMA issuer: the whole warp runs the loop, one elected lane issues =================
     const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(COUT >> 3) << 17) | ((uint32_t)(UM >> 4) << 24);
+    const uint32_t desc_hi = ((P >> 4) & 0x3FFFu) | (1u << 14);        // SBO = plane stride, descriptor version bit 46
     uint32_t accumulate = 0;
     for (int it = 0; it < my_items; ++it) {
       const int s = it & 1, use = it >> 1;
       if (!mbar_wait(bar0 + 8u * (direct ? 5 + s : s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
       asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
       const uint32_t x_base = smem_u32(smem + (size_t)s * stage_bytes), y_base = x_base + (uint32_t)(XPL + 1) * P;
+      const uint32_t x_lo = ((x_base >> 4) & 0x3FFFu) | (8u << 16), y_lo = ((y_base >> 4) & 0x3FFFu) | (8u << 16);   // LBO = 128 B
       for (int k0 = 0; k0 < a.kext; k0 += 16) {
-        const uint64_t bd = make_desc(y_base + (uint32_t)k0 * 16u, 128u, P);
+        const uint64_t bd = ((uint64_t)desc_hi << 32) | (uint64_t)(y_lo + (uint32_t)k0);
 #pragma unroll
         for (int acc = 0; acc < NACC; ++acc) {
           const uint32_t shift = ST3 ? (uint32_t)(acc * Wp) : (uint32_t)((acc / 3) * Wp + (acc % 3));
-          const uint64_t ad = make_desc(x_base + ((uint32_t)k0 + shift) * 16u, 128u, P);
-          mma_f16(tmem_base + (uint32_t)(acc * COUT), ad, bd, idesc, accumulate);
+          const uint64_t ad = ((uint64_t)desc_hi << 32) | (uint64_t)(x_lo + (uint32_t)k0 + shift);
+          if (elect_one()) mma_f16(tmem_base + (uint32_t)(acc * COUT), ad, bd, idesc, accumulate);
         }
         accumulate = 1;
       }
-      mma_commit(bar0 + 8u * (2 + s));          // stage s may be refilled once these MMAs have read it
+      if (elect_one()) mma_commit(bar0 + 8u * (2 + s));          // stage s may be refilled once these MMAs have read it
+      __syncwarp();
     }
-    mma_commit(bar0 + 8u * 4);                  // everything issued so far has completed -> accumulators final
+    if (elect_one()) mma_commit(bar0 + 8u * 4);                  // everything issued so far has completed -> accumulators final
+    __syncwarp();
   }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
