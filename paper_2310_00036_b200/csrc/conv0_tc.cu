@@ -13,6 +13,7 @@
 //            per di) live in TMEM for the life of the CTA; per-CTA partials are summed in CTA order.
 #include "common.cuh"
 #include "tc_ptx.cuh"
+#include "pool.cuh"
 
 namespace cb {
 namespace tc0 {
@@ -95,9 +96,7 @@ __device__ __forceinline__ void pool_scatter(const Args& a, const PoolGeom& q, u
     const int yl = y0 + wy;
     if ((unsigned)yl < (unsigned)rows) {
       uint16_t* p = reinterpret_cast<uint16_t*>(base + (size_t)(yl * Wp + x0 + wx) * 16) + k;
-      const float o = __uint_as_float((uint32_t)(*p) << 16), t = __uint_as_float((uint32_t)h[k] << 16);
-      const __nv_bfloat16 r = __float2bfloat16_rn(o + t);
-      *p = *reinterpret_cast<const uint16_t*>(&r);
+      pool::add_bf16(p, h[k]);
     }
   }
 }
@@ -192,29 +191,23 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
       const int pr = min(a.Rp, Ho - py0);
       for (int i = tid; i < pr * Wo * C8; i += 256) {
         const int c8 = i % C8, q = i / C8, ox = q % Wo, oy = py0 + q / Wo;
-        float best[8]; uint32_t bk[8];
+        uint4 v[9]; uint32_t valid = 0;
 #pragma unroll
-        for (int k = 0; k < 8; ++k) { best[k] = -INFINITY; bk[k] = 15; }
         for (int di = 0; di < 3; ++di) {
-          const int iy = oy * 2 + di - ph; if ((unsigned)iy >= (unsigned)a.H) continue;
-          for (int dj = 0; dj < 3; ++dj) {
-            const int ix = ox * 2 + dj - pw; if ((unsigned)ix >= (unsigned)a.W) continue;
-            const uint4 u = *reinterpret_cast<const uint4*>(ct + ((size_t)(iy - yb) * a.W + ix) * COUT + c8 * 8);
-            const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&u);
+          const int iy = oy * 2 + di - ph;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-              const float2 t = __bfloat1622float2(h[k]);
-              if (t.x > best[2 * k]) { best[2 * k] = t.x; bk[2 * k] = (uint32_t)(di * 3 + dj); }
-              if (t.y > best[2 * k + 1]) { best[2 * k + 1] = t.y; bk[2 * k + 1] = (uint32_t)(di * 3 + dj); }
+          for (int dj = 0; dj < 3; ++dj) {
+            const int ix = ox * 2 + dj - pw;
+            if ((unsigned)iy < (unsigned)a.H && (unsigned)ix < (unsigned)a.W) {
+              v[di * 3 + dj] = *reinterpret_cast<const uint4*>(ct + ((size_t)(iy - yb) * a.W + ix) * COUT + c8 * 8);
+              valid |= 1u << (di * 3 + dj);
             }
           }
         }
         const size_t o = (((size_t)f * Ho + oy) * Wo + ox) * COUT + c8 * 8;
-        uint4 r; __nv_bfloat162* o2 = reinterpret_cast<__nv_bfloat162*>(&r);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) o2[k] = __floats2bfloat162_rn(best[2 * k], best[2 * k + 1]);
+        uint4 r; uint2 pk;
+        pool::window_max(v, valid, r, pk);
         *reinterpret_cast<uint4*>(a.pool_out + o) = r;
-        uint2 pk; pk.x = bk[0] | (bk[1] << 8) | (bk[2] << 16) | (bk[3] << 24); pk.y = bk[4] | (bk[5] << 8) | (bk[6] << 16) | (bk[7] << 24);
         *reinterpret_cast<uint2*>(a.pool_arg_out + o) = pk;
       }
     }
@@ -398,8 +391,10 @@ int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* fr
   int R, nb, Rp = 0; size_t ctile = 0;
   if (pool_out) {      // fused max-pool: a band of Rp pooled rows needs 2 Rp + 1 conv rows, kept in shared memory as bf16
     const int Ho = (g.H + 1) / 2;
-    Rp = g.Cout == 16 ? 10 : 5; if (Rp > Ho) Rp = Ho;
-    R = 2 * Rp + 1; nb = (Ho + Rp - 1) / Rp;
+    auto need = [&](int rp) { const int r = 2 * rp + 1; return (size_t)6 * 2 * g.Cout * 16 + (size_t)(((r * Wp + 127) / 128) * 128 + 2 * Wp + 8) * 16 + (size_t)r * g.W * g.Cout * 2; };
+    Rp = 1; while (Rp < Ho && need(Rp + 1) <= (size_t)110 * 1024) ++Rp;      // two CTAs per SM
+    nb = (Ho + Rp - 1) / Rp; Rp = (Ho + nb - 1) / nb;                          // equal bands
+    R = 2 * Rp + 1;
     ctile = (size_t)R * g.W * g.Cout * 2;
   } else {
     R = std::min(g.H, (90 * 1024 / 16 - 2 * Wp - 130) / Wp - 2); if (R < 1) R = 1;

@@ -2,6 +2,7 @@
 // (a9-a10) over the layer program built in api.cu.  Plain SIMT path; tcgen05 kernels live in
 // conv_tc.cu and are dispatched from here when the shape qualifies.
 #include "gemm_simt.cuh"
+#include "pool.cuh"
 
 #include <type_traits>
 
@@ -154,44 +155,81 @@ __global__ void pool_fwd_v8_kernel(const bf16* __restrict__ x, bf16* __restrict_
   size_t total = (size_t)F * Ho * Wo * C8;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
     int c8 = (int)(i % C8); size_t q = i / C8; int ox = (int)(q % Wo); q /= Wo; int oy = (int)(q % Ho); size_t f = q / Ho;
-    float best[8]; uint32_t bk[8];
+    uint4 v[9]; uint32_t valid = 0;
 #pragma unroll
-    for (int k = 0; k < 8; ++k) { best[k] = -INFINITY; bk[k] = 15; }
     for (int di = 0; di < 3; ++di) {
-      int iy = oy * 2 + di - ph; if ((unsigned)iy >= (unsigned)H) continue;
-      for (int dj = 0; dj < 3; ++dj) {
-        int ix = ox * 2 + dj - pw; if ((unsigned)ix >= (unsigned)W) continue;
-        float v[8]; bf8_to_f(*reinterpret_cast<const uint4*>(x + ((f * H + iy) * W + ix) * C + c8 * 8), v);
+      const int iy = oy * 2 + di - ph;
 #pragma unroll
-        for (int k = 0; k < 8; ++k) if (v[k] > best[k]) { best[k] = v[k]; bk[k] = (uint32_t)(di * 3 + dj); }   // strict >: first maximum
+      for (int dj = 0; dj < 3; ++dj) {
+        const int ix = ox * 2 + dj - pw;
+        if ((unsigned)iy < (unsigned)H && (unsigned)ix < (unsigned)W) {
+          v[di * 3 + dj] = *reinterpret_cast<const uint4*>(x + ((f * H + iy) * W + ix) * C + c8 * 8);
+          valid |= 1u << (di * 3 + dj);
+        }
       }
     }
-    *reinterpret_cast<uint4*>(y + i * 8) = f_to_bf8(best);
-    uint2 pk; pk.x = bk[0] | (bk[1] << 8) | (bk[2] << 16) | (bk[3] << 24); pk.y = bk[4] | (bk[5] << 8) | (bk[6] << 16) | (bk[7] << 24);
+    uint4 best; uint2 pk;
+    pool::window_max(v, valid, best, pk);      // packed bf16 max; first maximum in window order (A11)
+    *reinterpret_cast<uint4*>(y + i * 8) = best;
     *reinterpret_cast<uint2*>(arg + i * 8) = pk;
   }
 }
-__global__ void pool_bwd_v8_kernel(const uint8_t* __restrict__ arg, const bf16* __restrict__ dy, bf16* __restrict__ dx, int F, int C, int H, int W) {
-  int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W), C8 = C / 8;
-  size_t total = (size_t)F * H * W * C8;
-  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-    int c8 = (int)(i % C8); size_t q = i / C8; int ix = (int)(q % W); q /= W; int iy = (int)(q % H); size_t f = q / H;
-    float g[8];
+// Max-pool adjoint, scatter form: one CTA builds a band of `RB` input rows of one frame in shared memory.  Every
+// pooled element of the rows that reach into the band adds its gradient to the pixel its stored arg-max names.
+// Windows whose (oy, ox) parities agree are disjoint, so the four parity classes run as four barrier-separated
+// phases of plain read-modify-writes (no atomics, fixed order: bitwise reproducible); a pixel elected by several
+// windows is rounded to bf16 after each addition.  The finished band leaves as one linear copy.
+__global__ void __launch_bounds__(256) pool_bwd_scatter_kernel(const uint8_t* __restrict__ arg, const bf16* __restrict__ dy, bf16* __restrict__ dx,
+                                                               int F, int C, int H, int W, int RB, int nbands) {
+  extern __shared__ __align__(16) uint8_t tile[];
+  const int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W), C8 = C / 8, tid = threadIdx.x;
+  for (int item = blockIdx.x; item < F * nbands; item += gridDim.x) {
+    const int f = item / nbands, yb = (item - f * nbands) * RB, rows = min(RB, H - yb);
+    const int n16 = rows * W * C8;
+    int lo = yb + ph - 2; lo = lo <= 0 ? 0 : (lo + 1) / 2;
+    const int hi = min((yb + rows - 1 + ph) / 2, Ho - 1);
+    // this thread's first element of each phase is fetched before the tile is touched
+    uint2 pk[4]; uint4 dv[4]; int py[4], px[4], pc[4]; bool ok[4];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) g[k] = 0.f;
-    int oy_lo = (iy + ph - 2 + 1) / 2; if (iy + ph - 2 < 0) oy_lo = 0;
-    int ox_lo = (ix + pw - 2 + 1) / 2; if (ix + pw - 2 < 0) ox_lo = 0;
-    int oy_hi = min((iy + ph) / 2, Ho - 1), ox_hi = min((ix + pw) / 2, Wo - 1);
-    for (int oy = oy_lo; oy <= oy_hi; ++oy)
-      for (int ox = ox_lo; ox <= ox_hi; ++ox) {
-        const uint32_t me = (uint32_t)((iy - (oy * 2 - ph)) * 3 + (ix - (ox * 2 - pw)));   // my position inside this window
-        const size_t o = ((f * Ho + oy) * Wo + ox) * C + c8 * 8;
-        const uint2 pk = *reinterpret_cast<const uint2*>(arg + o);
-        float d[8]; bf8_to_f(*reinterpret_cast<const uint4*>(dy + o), d);
-#pragma unroll
-        for (int k = 0; k < 4; ++k) { if (((pk.x >> (8 * k)) & 255u) == me) g[k] += d[k]; if (((pk.y >> (8 * k)) & 255u) == me) g[4 + k] += d[4 + k]; }
+    for (int p = 0; p < 4; ++p) {
+      const int pa = p >> 1, pb = p & 1, first = lo + (((lo & 1) != pa) ? 1 : 0);
+      const int noy = hi >= first ? (hi - first) / 2 + 1 : 0, nox = (Wo - pb + 1) / 2;
+      ok[p] = tid < noy * nox * C8;
+      if (ok[p]) {
+        pc[p] = tid % C8; const int r = tid / C8; px[p] = pb + 2 * (r % nox); py[p] = first + 2 * (r / nox);
+        const size_t o = (((size_t)f * Ho + py[p]) * Wo + px[p]) * C + pc[p] * 8;
+        pk[p] = *reinterpret_cast<const uint2*>(arg + o); dv[p] = *reinterpret_cast<const uint4*>(dy + o);
       }
-    *reinterpret_cast<uint4*>(dx + i * 8) = f_to_bf8(g);
+    }
+    for (int i = tid; i < n16; i += 256) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      __syncthreads();
+      const int pa = p >> 1, pb = p & 1, first = lo + (((lo & 1) != pa) ? 1 : 0);
+      const int noy = hi >= first ? (hi - first) / 2 + 1 : 0, nox = (Wo - pb + 1) / 2, n = noy * nox * C8;
+      for (int i = tid; i < n; i += 256) {
+        int oy, ox, c8; uint2 k2; uint4 d4;
+        if (i == tid && ok[p]) { oy = py[p]; ox = px[p]; c8 = pc[p]; k2 = pk[p]; d4 = dv[p]; }
+        else {
+          c8 = i % C8; const int r = i / C8; ox = pb + 2 * (r % nox); oy = first + 2 * (r / nox);
+          const size_t o = (((size_t)f * Ho + oy) * Wo + ox) * C + c8 * 8;
+          k2 = *reinterpret_cast<const uint2*>(arg + o); d4 = *reinterpret_cast<const uint4*>(dy + o);
+        }
+        const int y0 = oy * 2 - ph - yb, x0 = ox * 2 - pw;
+        const uint16_t* h = reinterpret_cast<const uint16_t*>(&d4);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const uint32_t a = ((k < 4 ? k2.x : k2.y) >> (8 * (k & 3))) & 255u;
+          const int wy = (int)((a * 11u) >> 5), wx = (int)a - 3 * wy, yl = y0 + wy;
+          if ((unsigned)yl < (unsigned)rows)
+            pool::add_bf16(reinterpret_cast<uint16_t*>(tile) + ((size_t)(yl * W + x0 + wx) * C + c8 * 8 + k), h[k]);
+        }
+      }
+    }
+    __syncthreads();
+    uint4* out = reinterpret_cast<uint4*>(dx + ((size_t)f * H + yb) * W * C);
+    for (int i = tid; i < n16; i += 256) out[i] = reinterpret_cast<const uint4*>(tile)[i];
+    __syncthreads();
   }
 }
 
@@ -292,9 +330,16 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
       }
       size_t total = (size_t)F * op.H * op.W * op.C;
       ProfScope ps(K_POOL_BWD, st, 1, 0.0, (double)sizeof(AT) * (2.0 * total + (double)F * pool_out(op.H) * pool_out(op.W) * op.C));
-      if (std::is_same<AT, bf16>::value && op.C % 8 == 0)
-        pool_bwd_v8_kernel<<<grid_for(total / 8), 256, 0, st>>>((const uint8_t*)ws.act[op.mask_t], (const bf16*)ws.grad[op.dy], (bf16*)ws.grad[op.dx], F, op.C, op.H, op.W);
-      else
+      if (std::is_same<AT, bf16>::value && op.C % 8 == 0) {
+        const size_t row_bytes = (size_t)op.W * op.C * 2;
+        int RB = (int)std::min<size_t>((size_t)op.H, std::max<size_t>(2, (size_t)(40 * 1024) / row_bytes));
+        const int nb = (op.H + RB - 1) / RB; RB = (op.H + nb - 1) / nb;
+        const size_t smem = (size_t)RB * row_bytes;
+        static size_t configured = 48 * 1024;
+        if (smem > configured) { CB_CUDA(cudaFuncSetAttribute(pool_bwd_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); configured = smem; }
+        pool_bwd_scatter_kernel<<<std::min(F * nb, 148 * 8), 256, smem, st>>>((const uint8_t*)ws.act[op.mask_t], (const bf16*)ws.grad[op.dy], (bf16*)ws.grad[op.dx],
+                                                                             F, op.C, op.H, op.W, RB, nb);
+      } else
         pool_bwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (const AT*)ws.grad[op.dy], (AT*)ws.grad[op.dx], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());
       continue;
