@@ -70,6 +70,8 @@ struct WgradTcArgs {
   const bf16* dy;     // [F, H, W, COUT]
   float* partial;     // [gridDim.x][9][CIN+1][COUT]
   int F, H, W, G, R, nbands, npix_alloc, kext, relu_in, stage_planes, use_tma, dy_rows;
+  int repl;           // ST3 with TMA: only the dj = 0 planes are landed (the TMA unit moves about one 16-byte piece per clock, so three
+                      // shifted boxes would bound the kernel); the loader warps derive the dj = 1, 2 copies in shared memory
   int c_off, cin_total;      // the kernel handles input channels [c_off, c_off + CIN) of a layer with cin_total channels
   int* error_flag;
 };
@@ -125,7 +127,7 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
   const int ngroups = (a.F + a.G - 1) / a.G, nitems = ngroups * a.nbands;
   const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
 
-  const bool direct = a.use_tma && !a.relu_in;      // nothing to do between the TMA landing and the MMAs: the issuer waits on raw[] itself
+  const bool direct = a.use_tma && !a.relu_in && !a.repl;      // nothing to do between the TMA landing and the MMAs: the issuer waits on raw[] itself
   if (warp < NLOAD / 32) {
     // ================= loaders =================
     for (int it = 0; it < (direct ? 0 : my_items); ++it) {
@@ -138,7 +140,23 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
       if (a.use_tma) {
         // operands were landed by the TMA producer thread; only the ReLU (in place) is left to these warps
         if (!mbar_wait(bar0 + 8u * (5 + s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 7; }
-        if (a.relu_in) {
+        if (a.repl) {
+          const int n16 = a.G * Rb;
+          const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
+          for (int i = tid; i < n16 * XCH; i += NLOAD) {
+            const int ch = i / n16, pos = i - ch * n16;
+            uint8_t* p = xs + (size_t)ch * P + (size_t)pos * 16;
+            uint4 v = *reinterpret_cast<uint4*>(p);
+            if (a.relu_in) {
+              __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+#pragma unroll
+              for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
+              *reinterpret_cast<uint4*>(p) = v;
+            }
+            if (pos >= 1) *reinterpret_cast<uint4*>(p + (size_t)XCH * P - 16) = v;          // plane (1, ch), one position earlier
+            if (pos >= 2) *reinterpret_cast<uint4*>(p + (size_t)2 * XCH * P - 32) = v;      // plane (2, ch), two positions earlier
+          }
+        } else if (a.relu_in) {
           const int n16 = a.G * Rb;
           for (int i = tid; i < n16 * XPL; i += NLOAD) {
             const int pl = i / n16, pos = i - pl * n16;
@@ -245,8 +263,9 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcAr
         if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 7; }
         const int grp = item / a.nbands, band = item - grp * a.nbands, f0 = grp * a.G, yb = band * a.R;
         const uint32_t xs = smem_u32(smem + (size_t)s * stage_bytes), ys = xs + (uint32_t)(XPL + 1) * P, rb = bar0 + 8u * (5 + s);
-        tma::arrive_expect_tx(rb, xbytes * XPL + ybytes * YCH);
-        for (int pl = 0; pl < XPL; ++pl) {       // plane (dj, ch): X shifted by dj positions = box started dj columns further right
+        const int npl = a.repl ? XCH : XPL;
+        tma::arrive_expect_tx(rb, xbytes * (uint32_t)npl + ybytes * YCH);
+        for (int pl = 0; pl < npl; ++pl) {       // plane (dj, ch): X shifted by dj positions = box started dj columns further right
           const int dj = ST3 ? pl / XCH : 0, ch = ST3 ? pl % XCH : pl;
           tma::load_4d(xs + (uint32_t)pl * P, &xmap, a.c_off + ch * 8, -1 + dj, yb - 1, f0, rb);
         }
@@ -369,7 +388,7 @@ int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, con
                        tma::make_nhwc_map(&ymap, dy, F, g.H, g.W, g.Cout, g.W + 2, dy_rows, p.G);
   for (int c_off = 0; c_off < g.Cin; c_off += cin_k) {
     tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, p.stage_planes, use_tma ? 1 : 0, dy_rows,
-                       c_off, g.Cin, error_flag};
+                       use_tma ? 1 : 0, c_off, g.Cin, error_flag};
     int rc;
     if (cin_k == 16 && g.Cout == 16) rc = launch_w<16, 16>(a, xmap, ymap, p.smem, grid, st);
     else if (cin_k == 16) rc = launch_w<16, 32>(a, xmap, ymap, p.smem, grid, st);
