@@ -247,6 +247,38 @@ __global__ void wgrad_reduce_kernel(const float* __restrict__ partial, int split
   }
 }
 
+// ---- weight gradient of the two heads (a [fc x (A+1)] matrix): CTA z sums a fixed chunk of frames, thread k owns hidden unit k ----
+// partial layout = [z][fc + 1][N] (row fc = bias gradient), the layout wgrad_reduce_kernel sums in z order.
+constexpr int HEAD_WGRAD_SPLITS = 148;      // a constant, not the device's SM count: the summation order is a function of the shape only (A16)
+template <typename AT>
+__global__ void __launch_bounds__(256) heads_wgrad_kernel(const AT* __restrict__ hid, const AT* __restrict__ dy, float* __restrict__ partial, int F, int fc, int N, int chunk) {
+  __shared__ float dys[64 * 32];
+  const int f0 = blockIdx.x * chunk, f1 = min(F, f0 + chunk);
+  float* out = partial + (size_t)blockIdx.x * (fc + 1) * N;
+  for (int k0 = 0; k0 < fc + 1; k0 += 256) {
+    const int k = k0 + threadIdx.x;
+    float acc[32];
+#pragma unroll
+    for (int n = 0; n < 32; ++n) acc[n] = 0.f;
+    for (int fb = f0; fb < f1; fb += 64) {
+      const int nf = min(64, f1 - fb);
+      __syncthreads();
+      for (int i = threadIdx.x; i < nf * N; i += 256) dys[(i / N) * 32 + i % N] = (float)dy[(size_t)fb * N + i];
+      __syncthreads();
+      if (k <= fc)
+        for (int j = 0; j < nf; ++j) {
+          const float h = k < fc ? fmaxf((float)hid[(size_t)(fb + j) * fc + k], 0.f) : 1.f;
+#pragma unroll
+          for (int n = 0; n < 32; ++n) if (n < N) acc[n] = fmaf(h, dys[j * 32 + n], acc[n]);
+        }
+    }
+    if (k <= fc) {
+#pragma unroll
+      for (int n = 0; n < 32; ++n) if (n < N) out[(size_t)k * N + n] = acc[n];
+    }
+  }
+}
+
 // split-K policy: a function of the problem shape only (never of the device), so the summation
 // order -- and with it every bit of the gradient -- is fixed (A16).
 static inline void wgrad_split(long long K, int* splits, int* kchunk, long long tiles_mn = 1 << 20) {
@@ -258,6 +290,7 @@ static inline void wgrad_split(long long K, int* splits, int* kchunk, long long 
 
 size_t wgrad_partial_elems(const Geom& g, long long frames) {
   int s, ch; wgrad_split(frames * g.Ho * g.Wo, &s, &ch, (long long)((g.kh * g.kw * g.Cin + 1 + 127) / 128) * ((g.Cout + 63) / 64));
+  if (g.kh == 1 && g.kw == 1 && g.H == 1 && g.W == 1 && g.Cout <= 32) s = std::max(s, HEAD_WGRAD_SPLITS);      // heads_wgrad_kernel
   return (size_t)s * (g.kh * g.kw * g.Cin + 1) * g.Cout;
 }
 
@@ -285,6 +318,12 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     int M = F * g.Ho * g.Wo, N = g.Cout, K = g.kh * g.kw * g.Cin;
     const AT* wf = (const AT*)ws.wf + L.wf_off; const float* bias = ws.bias + L.bias_off;
     const AT* skip = L.skip_t >= 0 ? (const AT*)ws.act[L.skip_t] : nullptr;
+    if (L.f32_out && L.relu_in && g.kh == 1 && g.kw == 1 && g.H == 1 && g.W == 1 && N <= 32 && !skip) {      // the heads: one warp per frame (its own profile class)
+      int rc = launch_heads_sample(std::is_same<AT, bf16>::value ? CB_PREC_BF16_TC : CB_PREC_FP32_REF, ws.act[L.in_t], wf, bias, M, K, N - 1, 0, 0, 0,
+                                   (float*)ws.act[L.out_t], nullptr, nullptr, nullptr, st);
+      if (rc) return rc;
+      continue;
+    }
     double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
     ProfScope ps(K_CONV_FWD, st, 1, 2.0 * M * N * K, in_bytes + (double)M * N * (L.f32_out ? 4 : sizeof(AT)) * (skip ? 2 : 1) + (double)K * N * sizeof(AT));
     int rc;
@@ -378,6 +417,11 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
       if (L.u8_in) {
         WgradProblem<AT, AT, true> p{M, N, Kpix, kchunk, {g, obs, frame_idx, false}, (const AT*)ws.grad[op.dy], ws.partial};
         rc = launch_gemm(p, splits, st);
+      } else if (L.f32_out && L.relu_in && g.kh == 1 && g.kw == 1 && g.H == 1 && g.W == 1 && N <= 32) {      // the heads
+        const int chunk = (F + HEAD_WGRAD_SPLITS - 1) / HEAD_WGRAD_SPLITS;
+        splits = (F + chunk - 1) / chunk;
+        heads_wgrad_kernel<AT><<<splits, 256, 0, st>>>((const AT*)ws.act[L.in_t], (const AT*)ws.grad[op.dy], ws.partial, F, g.Cin, N, chunk);
+        rc = cudaGetLastError() == cudaSuccess ? CB_OK : CB_ECUDA;
       } else {
         WgradProblem<AT, AT, false> p{M, N, Kpix, kchunk, {g, ws.act[L.in_t], nullptr, L.relu_in}, (const AT*)ws.grad[op.dy], ws.partial};
         rc = launch_gemm(p, splits, st);
