@@ -335,9 +335,12 @@ __global__ void __launch_bounds__(PIPE_THREADS) conv3x3_tc_pipe_kernel(const Pip
   __shared__ __align__(16) float bias_s[64];
   const int tid = threadIdx.x, warp = tid >> 5, NS = pa.nstages;
   const int Wp = a.W + 2, R = (a.RB + 2) * Wp;
+  // stages hold whole pixels, one row of PITCH = 2*CIN bytes per position, in the 32B/64B/128B swizzle pattern the TMA writes and
+  // the A descriptor names; the pattern is a function of the absolute shared-memory address (stages are 1024-byte aligned), so a
+  // descriptor may start at any position: a tap is still a constant shift of the start address
+  constexpr uint32_t PITCH = 2u * CIN, SWZ = CIN == 16 ? 6u : (CIN == 32 ? 4u : 2u);
   uint8_t* w_smem = smem;
-  uint8_t* in_smem = smem + ((W_BYTES + 127u) & ~127u);
-  const uint32_t plane_bytes = (uint32_t)a.npix_alloc * 16u;
+  uint8_t* in_smem = smem + W_BYTES; in_smem += (1024u - (smem_u32(in_smem) & 1023u)) & 1023u;
   const uint32_t bar0 = smem_u32(&bars[0]);
   auto RAW = [&](int s) { return bar0 + 8u * (uint32_t)s; };
   auto FULL = [&](int s) { return bar0 + 8u * (uint32_t)(PIPE_MAX_STAGES + s); };
@@ -410,15 +413,15 @@ __global__ void __launch_bounds__(PIPE_THREADS) conv3x3_tc_pipe_kernel(const Pip
       if (elect_one()) {
         const uint32_t dst = smem_u32(in_smem) + (uint32_t)s * pa.stage_bytes;
         tma::arrive_expect_tx(RAW(s), bytes);
-#pragma unroll
-        for (int ch = 0; ch < NCH; ++ch) tma::load_4d(dst + (uint32_t)ch * plane_bytes, &tmap, ch * 8, -1, yb - 1, f0, RAW(s));
+        tma::load_4d(dst, &tmap, 0, -1, yb - 1, f0, RAW(s));
       }
       __syncwarp();
     }
   } else if (warp == PIPE_EPI_WARPS + 1) {
     // ================= MMA issuer =================
     const uint32_t idesc = make_idesc(128, COUT, 0, 0);
-    const uint32_t d_hi = 8u | (1u << 14);                                                                    // SBO = 128 B, version bit 46
+    const uint32_t d_hi = 8u | (1u << 14);                                                                    // B: SBO = 128 B, version bit 46
+    const uint32_t a_hi = ((8u * PITCH) >> 4) | (1u << 14) | (SWZ << 29);                                     // A: SBO = 8 rows, swizzle mode in bits 61-63
     const uint32_t b_lo = ((smem_u32(w_smem) >> 4) & 0x3FFFu) | ((uint32_t)COUT << 16);                       // LBO = COUT*16 B
     uint32_t bc = 0;
     for (int it = 0; it < my_items; ++it) {
@@ -427,7 +430,7 @@ __global__ void __launch_bounds__(PIPE_THREADS) conv3x3_tc_pipe_kernel(const Pip
       const int ntiles = ((nf - 1) * R + a.RB * Wp + 127) / 128;
       if (!mbar_wait(a.relu_in ? FULL(s) : RAW(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
       tc_fence_after();
-      const uint32_t a_lo = (((smem_u32(in_smem) + (uint32_t)s * pa.stage_bytes) >> 4) & 0x3FFFu) | (((plane_bytes >> 4) & 0x3FFFu) << 16);   // LBO = plane
+      const uint32_t a_lo = (((smem_u32(in_smem) + (uint32_t)s * pa.stage_bytes) >> 4) & 0x3FFFu) | (1u << 16);      // LBO unused (one swizzle row holds the K slice)
       for (int t0 = 0; t0 < ntiles; t0 += TB, ++bc) {
         const int nt = min(TB, ntiles - t0), b = (int)(bc % PIPE_TBUF);
         if (bc >= PIPE_TBUF && !mbar_wait(TEMPTY(b), ((bc / PIPE_TBUF) - 1) & 1u)) { if (a.error_flag) *a.error_flag = 3; }
@@ -439,7 +442,7 @@ __global__ void __launch_bounds__(PIPE_THREADS) conv3x3_tc_pipe_kernel(const Pip
             const uint32_t shift = (uint32_t)((tap / 3) * Wp + (tap % 3));
 #pragma unroll
             for (int ks = 0; ks < KSTEPS; ++ks) {
-              const uint64_t ad = ((uint64_t)d_hi << 32) | (uint64_t)(a_lo + q0 + shift + (uint32_t)(2 * ks) * (plane_bytes >> 4));
+              const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(a_lo + (q0 + shift) * (PITCH >> 4) + (uint32_t)(2 * ks));
               const uint64_t bd = ((uint64_t)d_hi << 32) | (uint64_t)(b_lo + (uint32_t)((tap * NCH + 2 * ks) * COUT));
               if (elect_one()) mma_f16(td, ad, bd, idesc, (tap | ks) ? 1u : 0u);
             }
@@ -458,16 +461,14 @@ __global__ void __launch_bounds__(PIPE_THREADS) conv3x3_tc_pipe_kernel(const Pip
     for (int it = 0; it < my_items; ++it) {
       const int s = it % NS, use = it / NS;
       if (!mbar_wait(RAW(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 7; }
-      uint8_t* st = in_smem + (size_t)s * pa.stage_bytes;
+      uint4* st = reinterpret_cast<uint4*>(in_smem + (size_t)s * pa.stage_bytes);
       const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
-      for (int i = t; i < n16 * NCH; i += 128) {
-        const int ch = i / n16, pos = i - ch * n16;
-        uint4* p = reinterpret_cast<uint4*>(st + (size_t)ch * plane_bytes + (size_t)pos * 16);
-        uint4 v = *p;
+      for (int i = t; i < n16 * NCH; i += 128) {      // elementwise: the swizzle does not matter
+        uint4 v = st[i];
         __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
 #pragma unroll
         for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
-        *p = v;
+        st[i] = v;
       }
       fence_async_smem();
       asm volatile("bar.sync 2, 128;\n" ::: "memory");
@@ -541,9 +542,9 @@ struct PipePlan { int G, npix_alloc, RB, nbands, nstages; size_t stage_bytes, sm
 static PipePlan pipe_plan(int F, int H, int W, int cin, int cout) {
   const int Wp = W + 2, R = (H + 2) * Wp;
   const size_t wbytes = ((size_t)9 * cin * cout * 2 + 127) & ~(size_t)127;
-  const size_t avail = (size_t)200 * 1024 - wbytes;
+  const size_t avail = (size_t)200 * 1024 - wbytes - 1024;      // 1 KB: the stages start on a 1024-byte boundary
   auto alloc_pix = [&](int positions) { int n = ((positions + 127) / 128) * 128 + 2 * Wp + 2; return (n + 7) / 8 * 8; };
-  auto bytes = [&](int positions) { return ((size_t)alloc_pix(positions) * cin * 2 + 127) & ~(size_t)127; };
+  auto bytes = [&](int positions) { return ((size_t)alloc_pix(positions) * cin * 2 + 1023) & ~(size_t)1023; };
   PipePlan p{1, 0, H, 1, 3, 0, 0, true};
   if (bytes(R) <= avail / 3) {
     // whole frames: the group size that minimises (items of the busiest CTA) x (tiles per item); a function of the shape only
@@ -563,8 +564,8 @@ static PipePlan pipe_plan(int F, int H, int W, int cin, int cout) {
     p.nbands = (int)((H + rows - 1) / rows); p.RB = (H + p.nbands - 1) / p.nbands;
     p.npix_alloc = alloc_pix((p.RB + 2) * Wp);
   }
-  p.stage_bytes = ((size_t)p.npix_alloc * cin * 2 + 127) & ~(size_t)127;
-  p.smem = wbytes + (size_t)p.nstages * p.stage_bytes;
+  p.stage_bytes = ((size_t)p.npix_alloc * cin * 2 + 1023) & ~(size_t)1023;
+  p.smem = wbytes + 1024 + (size_t)p.nstages * p.stage_bytes;
   p.ok = p.smem <= (size_t)220 * 1024;
   return p;
 }
@@ -601,7 +602,7 @@ int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16*
   CUtensorMap tmap; memset(&tmap, 0, sizeof tmap);
   {      // pipelined, TMA-fed kernel
     const PipePlan q = pipe_plan(F, H, W, cin, cout);
-    if (q.ok && W + 2 <= 256 && q.RB + 2 <= 256 && tma::make_nhwc_map(&tmap, in, F, H, W, cin, W + 2, q.RB + 2, q.G)) {
+    if (q.ok && W + 2 <= 256 && q.RB + 2 <= 256 && tma::make_nhwc_map(&tmap, in, F, H, W, cin, W + 2, q.RB + 2, q.G, cin, true)) {
       tc::PipeArgs pa{{in, w, bias, aux0, aux1, out, F, H, W, q.G, q.npix_alloc, relu_in ? 1 : 0, 1, relu_out ? 1 : 0, q.RB, q.nbands, error_flag},
                       q.nstages, (uint32_t)q.stage_bytes, (uint32_t)((0x100000000ull + (uint64_t)((q.RB + 2) * (W + 2)) - 1) / (uint64_t)((q.RB + 2) * (W + 2))),
                       (uint32_t)((0x100000000ull + (uint64_t)(W + 2) - 1) / (uint64_t)(W + 2))};

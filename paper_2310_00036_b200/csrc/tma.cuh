@@ -22,16 +22,21 @@ inline EncodeTiledFn encode_fn() {
   return fn;
 }
 
-// tensor [F][H][W][C] bf16 (C fastest); returns false if the driver refuses the map
-inline bool make_nhwc_map(CUtensorMap* m, const void* base, int F, int H, int W, int C, int box_w, int box_h, int box_f) {
+// tensor [F][H][W][C] bf16 (C fastest); returns false if the driver refuses the map.
+// box_c = 8: one 8-channel chunk per copy (plane layout, 16-byte pieces).  box_c = C in {16, 32, 64} with swizzle = true: whole
+// pixels (32/64/128-byte pieces: the TMA unit moves about one piece per clock whatever its size) written in the 32B/64B/128B
+// swizzle pattern, i.e. the canonical swizzled UMMA layout with one shared-memory row per pixel.
+inline bool make_nhwc_map(CUtensorMap* m, const void* base, int F, int H, int W, int C, int box_w, int box_h, int box_f, int box_c = 8, bool swizzle = false) {
   EncodeTiledFn fn = encode_fn();
   if (!fn) return false;
   cuuint64_t dims[4] = {(cuuint64_t)C, (cuuint64_t)W, (cuuint64_t)H, (cuuint64_t)F};
   cuuint64_t strides[3] = {(cuuint64_t)C * 2, (cuuint64_t)W * C * 2, (cuuint64_t)H * W * C * 2};
-  cuuint32_t box[4] = {8u, (cuuint32_t)box_w, (cuuint32_t)box_h, (cuuint32_t)box_f};
+  cuuint32_t box[4] = {(cuuint32_t)box_c, (cuuint32_t)box_w, (cuuint32_t)box_h, (cuuint32_t)box_f};
   cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+  CUtensorMapSwizzle sw = CU_TENSOR_MAP_SWIZZLE_NONE;
+  if (swizzle) sw = box_c == 16 ? CU_TENSOR_MAP_SWIZZLE_32B : (box_c == 32 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B);
   return fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+            sw, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 __device__ __forceinline__ void arrive_expect_tx(uint32_t bar, uint32_t bytes) {
