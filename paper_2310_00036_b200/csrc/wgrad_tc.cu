@@ -326,6 +326,167 @@ __global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nc
   grad[pm.w(o, c_off + row, tap / 3, tap % 3, g)] = tot;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Swizzled variant (TMA, Cin in {16, 32}): whole pixels are landed once, one shared-memory row of 2*CIN (X) or 2*COUT (DY)
+// bytes per position, in the 32B/64B/128B swizzle pattern.  The A descriptor is MN-major with LBO = one row: the M walk
+// steps to the NEXT POSITION, so rows dj*CIN + c of one MMA are the taps (di, 0..2) without any shifted copy of X
+// (the pattern is a function of the absolute address, so descriptors may start at any row).  Three accumulators
+// [UM x COUT] (one per di) stay in TMEM; the bias gradient is summed from the landed DY rows by the loader warps.
+//   warps 0-7  wait for a landed stage, apply the ReLU in place when the layer needs it, add DY into the bias sums
+//   warp 8     MMA issuer        warp 9  TMA producer (ring of `nstages` stages)
+struct WgradSwArgs {
+  float* partial; int F, H, W, G, R, nbands, npix_alloc, kext, relu_in, dy_rows, nstages;
+  uint32_t stage_bytes, y_off; int* error_flag;
+};
+constexpr int SW_MAX_STAGES = 3;
+
+template <int CIN, int COUT>
+__global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwArgs a, const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap ymap) {
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  constexpr int UM = CIN == 16 ? 64 : 128;
+  constexpr uint32_t PX = 2u * CIN, PY = 2u * COUT;
+  constexpr uint32_t SWX = CIN == 16 ? 6u : (CIN == 32 ? 4u : 2u), SWY = COUT == 16 ? 6u : (COUT == 32 ? 4u : 2u);
+  constexpr uint32_t TCOLS = 3 * COUT <= 128 ? 128u : 256u;
+  constexpr int YC8 = COUT / 8;
+  __shared__ __align__(8) uint64_t bars[3 * SW_MAX_STAGES + 1];      // raw[3], full[3], sempty[3], done
+  __shared__ uint32_t tmem_base_smem;
+  const int tid = threadIdx.x, warp = tid >> 5, NS = a.nstages;
+  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  const int Wp = a.W + 2, Rb = (a.R + 2) * Wp;
+  const uint32_t bar0 = smem_u32(&bars[0]);
+  auto RAW = [&](int s) { return bar0 + 8u * (uint32_t)s; };
+  auto FULL = [&](int s) { return bar0 + 8u * (uint32_t)(SW_MAX_STAGES + s); };
+  auto SEMPTY = [&](int s) { return bar0 + 8u * (uint32_t)(2 * SW_MAX_STAGES + s); };
+  const uint32_t DONE = bar0 + 8u * (3 * SW_MAX_STAGES);
+  if (tid == 0) {
+    for (int i = 0; i < 3 * SW_MAX_STAGES + 1; ++i)
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" :: "r"(bar0 + 8u * i), "r"((i >= 2 * SW_MAX_STAGES && i < 3 * SW_MAX_STAGES) ? 2 : 1) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    tma::prefetch_map(&xmap); tma::prefetch_map(&ymap);
+  }
+  if (warp == NLOAD / 32) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" :: "r"(smem_u32(&tmem_base_smem)), "r"(TCOLS) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+  }
+  // everything outside the landed boxes (slack positions, DY rows below a band) stays zero for the whole kernel
+  for (uint32_t i = tid; i < a.stage_bytes * (uint32_t)NS / 16; i += NLOAD + 64) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
+  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+  const uint32_t tmem_base = tmem_base_smem;
+  const int ngroups = (a.F + a.G - 1) / a.G, nitems = ngroups * a.nbands;
+  const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+  float* out = a.partial + (size_t)blockIdx.x * 9 * (CIN + 1) * COUT;
+
+  if (warp < NLOAD / 32) {
+    // ================= loaders: ReLU fix-up and bias sums =================
+    float db[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) db[k] = 0.f;
+    const int c8 = tid % YC8, p0 = tid / YC8, pstep = NLOAD / YC8, ny = a.G * a.dy_rows * Wp;
+    for (int it = 0; it < my_items; ++it) {
+      const int s = it % NS, use = it / NS;
+      if (!mbar_wait(RAW(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 7; }
+      uint8_t* xs = smem + (size_t)s * a.stage_bytes; const uint8_t* ys = xs + a.y_off;
+      if (a.relu_in) {
+        const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
+        const int n16 = a.G * Rb * (CIN / 8);
+        for (int i = tid; i < n16; i += NLOAD) {      // elementwise: the swizzle does not matter
+          uint4 v = reinterpret_cast<uint4*>(xs)[i];
+          __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
+          reinterpret_cast<uint4*>(xs)[i] = v;
+        }
+        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+        asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
+        if (tid == 0) mbar_arrive(FULL(s));
+      }
+      const uint32_t ybase = smem_u32(ys);
+      for (int p = p0; p < ny; p += pstep) {          // logical chunk c8 of row p sits at physical chunk c8 ^ (address bits 7..)
+        const uint32_t row = ybase + (uint32_t)p * PY, phys = (uint32_t)c8 ^ ((row >> 7) & (uint32_t)(YC8 - 1));
+        const uint4 v = *reinterpret_cast<const uint4*>(ys + (size_t)p * PY + phys * 16);
+        const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { const float2 f = __bfloat1622float2(h[k]); db[2 * k] += f.x; db[2 * k + 1] += f.y; }
+      }
+      asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
+      if (tid == 0) mbar_arrive(SEMPTY(s));
+    }
+    // ---- all MMAs complete: accumulators final, shared memory free ----
+    if (my_items > 0 && !mbar_wait(DONE, 0u)) { if (a.error_flag) *a.error_flag = 2; }
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    float* dbs = reinterpret_cast<float*>(smem);      // [NLOAD][8]
+#pragma unroll
+    for (int k = 0; k < 8; ++k) dbs[tid * 8 + k] = db[k];
+    asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
+    if (tid < COUT) {      // threads with chunk tid/8, in thread order: a fixed association
+      float t = 0.f;
+      for (int j = 0; j < pstep; ++j) t += dbs[(j * YC8 + tid / 8) * 8 + (tid % 8)];
+      out[(size_t)CIN * COUT + tid] = t;              // tap 0, row CIN = the bias gradient
+    }
+    if (warp < 4) {
+      const int lane = tid & 31;
+      const int row = (UM == 128) ? tid : ((lane < 16) ? warp * 16 + lane : 1 << 20);
+      const bool warp_needed = (UM == 128) ? (warp * 32 < 3 * CIN) : (warp * 16 < 3 * CIN);
+      if (warp_needed) {
+        for (int acc = 0; acc < 3; ++acc) {
+#pragma unroll
+          for (int c0 = 0; c0 < COUT; c0 += 16) {
+            float v[16];
+            tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(acc * COUT + c0), v);
+            if (row >= 3 * CIN) continue;
+            const int tap = acc * 3 + row / CIN, r = row % CIN;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + r) * COUT + c0 + i] = v[i];
+          }
+        }
+      }
+    }
+  } else if (warp == NLOAD / 32) {
+    // ================= MMA issuer =================
+    const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(COUT >> 3) << 17) | ((uint32_t)(UM >> 4) << 24);
+    const uint32_t a_hi = ((8u * PX) >> 4) | (1u << 14) | (SWX << 29), b_hi = ((8u * PY) >> 4) | (1u << 14) | (SWY << 29);
+    uint32_t accumulate = 0;
+    for (int it = 0; it < my_items; ++it) {
+      const int s = it % NS, use = it / NS;
+      if (!mbar_wait(a.relu_in ? FULL(s) : RAW(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
+      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+      const uint32_t x_base = smem_u32(smem) + (uint32_t)s * a.stage_bytes, y_base = x_base + a.y_off;
+      const uint32_t x_lo = ((x_base >> 4) & 0x3FFFu) | ((PX >> 4) << 16), y_lo = ((y_base >> 4) & 0x3FFFu) | (1u << 16);      // A: LBO = one position
+      for (int k0 = 0; k0 < a.kext; k0 += 16) {
+        const uint64_t bd = ((uint64_t)b_hi << 32) | (uint64_t)(y_lo + (uint32_t)k0 * (PY >> 4));
+#pragma unroll
+        for (int di = 0; di < 3; ++di) {
+          const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(x_lo + (uint32_t)(k0 + di * Wp) * (PX >> 4));
+          if (elect_one()) mma_f16(tmem_base + (uint32_t)(di * COUT), ad, bd, idesc, accumulate);
+        }
+        accumulate = 1;
+      }
+      if (elect_one()) mma_commit(SEMPTY(s));
+      __syncwarp();
+    }
+    if (elect_one()) mma_commit(DONE);
+    __syncwarp();
+  } else if (tid == NLOAD + 32) {
+    // ================= TMA producer =================
+    const uint32_t xbytes = (uint32_t)(a.G * Rb) * PX, ybytes = (uint32_t)(a.G * a.dy_rows * Wp) * PY;
+    for (int it = 0; it < my_items; ++it) {
+      const int item = blockIdx.x + it * gridDim.x, s = it % NS, use = it / NS;
+      if (use > 0 && !mbar_wait(SEMPTY(s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 7; }
+      const int grp = item / a.nbands, band = item - grp * a.nbands, f0 = grp * a.G, yb = band * a.R;
+      const uint32_t xs = smem_u32(smem) + (uint32_t)s * a.stage_bytes;
+      tma::arrive_expect_tx(RAW(s), xbytes + ybytes);
+      tma::load_4d(xs, &xmap, 0, -1, yb - 1, f0, RAW(s));
+      tma::load_4d(xs + a.y_off, &ymap, 0, 0, yb, f0, RAW(s));
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+  __syncthreads();
+  if (warp == NLOAD / 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tmem_base), "r"(TCOLS) : "memory");
+}
+
 }  // namespace tcw
 
 bool wgrad_tc_supported(const Geom& g) {
@@ -372,9 +533,72 @@ static int launch_w(const tcw::WgradTcArgs& a, const CUtensorMap& xmap, const CU
   return CB_OK;
 }
 
+// plan of the swizzled kernel: 3 stages of G whole frames (or one row band) in <= 208 KB; a function of the shape only
+struct SwPlan { int G, R, nbands, npix_alloc, kext, nstages; size_t stage_bytes, y_off, smem; bool ok; };
+static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
+  const int Wp = W + 2;
+  const size_t avail = (size_t)208 * 1024 / 3;
+  auto a1k = [](size_t b) { return (b + 1023) & ~(size_t)1023; };
+  auto stage = [&](int npos, int* kext, int* npix) {
+    *kext = (npos + 15) / 16 * 16; *npix = *kext + 2 * Wp + 8;
+    return a1k((size_t)*npix * cin * 2) + a1k((size_t)*npix * cout * 2);
+  };
+  SwPlan p{1, H, 1, 0, 0, 3, 0, 0, 0, true};
+  int kx, np;
+  if (stage((H + 2) * Wp, &kx, &np) <= avail) {
+    long best = -1;
+    for (int G = 1; G <= 8 && stage(G * (H + 2) * Wp, &kx, &np) <= avail; ++G) {
+      const long items = (F + G - 1) / G, per_cta = (items + 147) / 148, cost = per_cta * ((long)G * (H + 2) * Wp + 600);
+      if (best < 0 || cost < best) { best = cost; p.G = G; }
+    }
+  } else {
+    int rows = H;
+    while (rows > 1 && stage((rows + 2) * Wp, &kx, &np) > avail) --rows;
+    if (stage((rows + 2) * Wp, &kx, &np) > avail) { p.ok = false; return p; }
+    p.nbands = (H + rows - 1) / rows; p.R = (H + p.nbands - 1) / p.nbands;
+  }
+  p.stage_bytes = stage(p.G * (p.R + 2) * Wp, &p.kext, &p.npix_alloc);
+  p.y_off = a1k((size_t)p.npix_alloc * cin * 2);
+  p.smem = 1024 + (size_t)p.nstages * p.stage_bytes;
+  return p;
+}
+
+template <int CIN, int COUT>
+static int launch_sw(const tcw::WgradSwArgs& a, const CUtensorMap& xmap, const CUtensorMap& ymap, size_t smem, int grid, cudaStream_t st) {
+  static size_t configured = 0;
+  if (smem > configured) {
+    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_sw_kernel<CIN, COUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    configured = smem;
+  }
+  tcw::wgrad3x3_sw_kernel<CIN, COUT><<<grid, tcw::NLOAD + 64, smem, st>>>(a, xmap, ymap);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
 int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
                     int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
+  if (g.Cin == 16 || g.Cin == 32) {      // swizzled whole-pixel staging
+    const SwPlan q = sw_plan(F, g.H, g.W, g.Cin, g.Cout);
+    const int dy_rows = q.nbands > 1 ? q.R : q.R + 2;
+    CUtensorMap xmap, ymap; memset(&xmap, 0, sizeof xmap); memset(&ymap, 0, sizeof ymap);
+    if (q.ok && g.W + 2 <= 256 && q.R + 2 <= 256 && tma::make_nhwc_map(&xmap, x, F, g.H, g.W, g.Cin, g.W + 2, q.R + 2, q.G, g.Cin, true) &&
+        tma::make_nhwc_map(&ymap, dy, F, g.H, g.W, g.Cout, g.W + 2, dy_rows, q.G, g.Cout, true)) {
+      const int nitems = ((F + q.G - 1) / q.G) * q.nbands, grid = std::min(nitems, WGRAD_TC_MAX_CTAS);
+      tcw::WgradSwArgs a{partial, F, g.H, g.W, q.G, q.R, q.nbands, q.npix_alloc, q.kext, relu_in ? 1 : 0, dy_rows, q.nstages,
+                         (uint32_t)q.stage_bytes, (uint32_t)q.y_off, error_flag};
+      int rc;
+      if (g.Cin == 16 && g.Cout == 16) rc = launch_sw<16, 16>(a, xmap, ymap, q.smem, grid, st);
+      else if (g.Cin == 16) rc = launch_sw<16, 32>(a, xmap, ymap, q.smem, grid, st);
+      else if (g.Cout == 16) rc = launch_sw<32, 16>(a, xmap, ymap, q.smem, grid, st);
+      else if (g.Cout == 32) rc = launch_sw<32, 32>(a, xmap, ymap, q.smem, grid, st);
+      else rc = launch_sw<32, 64>(a, xmap, ymap, q.smem, grid, st);
+      if (rc) return rc;
+      tcw::wgrad_tc_reduce_kernel<<<(tcw::RL * 9 * (g.Cin + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, g.Cin, 0, grad);
+      CB_CUDA(cudaGetLastError());
+      return CB_OK;
+    }
+  }
   const int cin_k = g.Cin == 64 ? 32 : g.Cin;      // channels per kernel launch
   WPlan p = wgrad_plan(g.H, g.W, cin_k, g.Cout);
   if (p.smem > 224 * 1024) { set_error("wgrad_tc: plan does not fit shared memory"); return CB_EINVAL; }
