@@ -321,15 +321,17 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
       if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 4; }
       tc_fence_after();
       const uint32_t x_base = smem_u32(smem + (size_t)s * STAGE), y_base = x_base + P;
-      const uint32_t x_lo = ((x_base >> 4) & 0x3FFFu) | (8u << 16), y_lo = ((y_base >> 4) & 0x3FFFu) | (8u << 16);
-      for (int k0 = 0; k0 < a.kext; k0 += 16) {
-        const uint64_t bd = ((uint64_t)b_hi << 32) | (uint64_t)(y_lo + (uint32_t)k0);
-#pragma unroll
-        for (int di = 0; di < 3; ++di) {
-          const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(x_lo + (uint32_t)(k0 + di * Wp));
-          if (elect_one()) mma_f16(tmem_base + (uint32_t)(di * COUT), ad, bd, idesc, accumulate);
-        }
+      uint32_t xl0 = ((x_base >> 4) & 0x3FFFu) | (8u << 16), yl = ((y_base >> 4) & 0x3FFFu) | (8u << 16);      // running low words; LBO = 128 B
+      uint32_t xl1 = xl0 + (uint32_t)Wp, xl2 = xl1 + (uint32_t)Wp;
+      const int nk = a.kext >> 4;
+#pragma unroll 4
+      for (int k = 0; k < nk; ++k) {
+        const uint64_t bd = ((uint64_t)b_hi << 32) | yl;
+        if (elect_one()) mma_f16(tmem_base, ((uint64_t)a_hi << 32) | xl0, bd, idesc, accumulate);
+        if (elect_one()) mma_f16(tmem_base + (uint32_t)COUT, ((uint64_t)a_hi << 32) | xl1, bd, idesc, accumulate);
+        if (elect_one()) mma_f16(tmem_base + (uint32_t)(2 * COUT), ((uint64_t)a_hi << 32) | xl2, bd, idesc, accumulate);
         accumulate = 1;
+        xl0 += 16u; xl1 += 16u; xl2 += 16u; yl += 16u;      // 16 positions of 16 bytes
       }
       if (elect_one()) mma_commit(bar0 + 8u * (2 + s));
       __syncwarp();

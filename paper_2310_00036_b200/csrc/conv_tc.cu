@@ -435,17 +435,22 @@ __global__ void __launch_bounds__(PIPE_THREADS) conv3x3_tc_pipe_kernel(const Pip
         const int nt = min(TB, ntiles - t0), b = (int)(bc % PIPE_TBUF);
         if (bc >= PIPE_TBUF && !mbar_wait(TEMPTY(b), ((bc / PIPE_TBUF) - 1) & 1u)) { if (a.error_flag) *a.error_flag = 3; }
         tc_fence_after();
+#pragma unroll 1
         for (int sT = 0; sT < nt; ++sT) {
-          const uint32_t q0 = (uint32_t)(t0 + sT) * 128u, td = tmem_base + (uint32_t)(b * 128 + sT * COUT);
+          const uint32_t td = tmem_base + (uint32_t)(b * 128 + sT * COUT);
+          uint32_t row_lo = a_lo + (uint32_t)(t0 + sT) * 128u * (PITCH >> 4);      // start of the tile, tap row di = 0
 #pragma unroll
-          for (int tap = 0; tap < 9; ++tap) {
-            const uint32_t shift = (uint32_t)((tap / 3) * Wp + (tap % 3));
+          for (int di = 0; di < 3; ++di) {
 #pragma unroll
-            for (int ks = 0; ks < KSTEPS; ++ks) {
-              const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(a_lo + (q0 + shift) * (PITCH >> 4) + (uint32_t)(2 * ks));
-              const uint64_t bd = ((uint64_t)d_hi << 32) | (uint64_t)(b_lo + (uint32_t)((tap * NCH + 2 * ks) * COUT));
-              if (elect_one()) mma_f16(td, ad, bd, idesc, (tap | ks) ? 1u : 0u);
+            for (int dj = 0; dj < 3; ++dj) {
+#pragma unroll
+              for (int ks = 0; ks < KSTEPS; ++ks) {
+                const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(row_lo + (uint32_t)(dj * (PITCH >> 4) + 2 * ks));
+                const uint64_t bd = ((uint64_t)d_hi << 32) | (uint64_t)(b_lo + (uint32_t)(((di * 3 + dj) * NCH + 2 * ks) * COUT));
+                if (elect_one()) mma_f16(td, ad, bd, idesc, (di | dj | ks) ? 1u : 0u);
+              }
             }
+            row_lo += (uint32_t)Wp * (PITCH >> 4);
           }
         }
         if (elect_one()) {

@@ -454,15 +454,18 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
       if (!mbar_wait(a.relu_in ? FULL(s) : RAW(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
       asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
       const uint32_t x_base = smem_u32(smem) + (uint32_t)s * a.stage_bytes, y_base = x_base + a.y_off;
-      const uint32_t x_lo = ((x_base >> 4) & 0x3FFFu) | ((PX >> 4) << 16), y_lo = ((y_base >> 4) & 0x3FFFu) | (1u << 16);      // A: LBO = one position
-      for (int k0 = 0; k0 < a.kext; k0 += 16) {
-        const uint64_t bd = ((uint64_t)b_hi << 32) | (uint64_t)(y_lo + (uint32_t)k0 * (PY >> 4));
-#pragma unroll
-        for (int di = 0; di < 3; ++di) {
-          const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(x_lo + (uint32_t)(k0 + di * Wp) * (PX >> 4));
-          if (elect_one()) mma_f16(tmem_base + (uint32_t)(di * COUT), ad, bd, idesc, accumulate);
-        }
+      // running low words of the descriptors (the start address advances by 16 positions per step); LBO of A = one position
+      uint32_t xl0 = ((x_base >> 4) & 0x3FFFu) | ((PX >> 4) << 16), yl = ((y_base >> 4) & 0x3FFFu) | (1u << 16);
+      uint32_t xl1 = xl0 + (uint32_t)Wp * (PX >> 4), xl2 = xl1 + (uint32_t)Wp * (PX >> 4);
+      const int nk = a.kext >> 4;
+#pragma unroll 4
+      for (int k = 0; k < nk; ++k) {
+        const uint64_t bd = ((uint64_t)b_hi << 32) | yl;
+        if (elect_one()) mma_f16(tmem_base, ((uint64_t)a_hi << 32) | xl0, bd, idesc, accumulate);
+        if (elect_one()) mma_f16(tmem_base + (uint32_t)COUT, ((uint64_t)a_hi << 32) | xl1, bd, idesc, accumulate);
+        if (elect_one()) mma_f16(tmem_base + (uint32_t)(2 * COUT), ((uint64_t)a_hi << 32) | xl2, bd, idesc, accumulate);
         accumulate = 1;
+        xl0 += PX; xl1 += PX; xl2 += PX; yl += PY;      // 16 positions * (pitch / 16)
       }
       if (elect_one()) mma_commit(SEMPTY(s));
       __syncwarp();
@@ -551,6 +554,8 @@ static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
       const long items = (F + G - 1) / G, per_cta = (items + 147) / 148, cost = per_cta * ((long)G * (H + 2) * Wp + 600);
       if (best < 0 || cost < best) { best = cost; p.G = G; }
     }
+  } else if (stage((H + 2) * Wp, &kx, &np) <= (size_t)208 * 1024 / 2) {
+    p.nstages = 2;      // one whole frame per stage, two stages: fewer, longer items than three stages of half frames
   } else {
     int rows = H;
     while (rows > 1 && stage((rows + 2) * Wp, &kx, &np) > avail) --rows;
