@@ -536,17 +536,18 @@ static int launch_w(const tcw::WgradTcArgs& a, const CUtensorMap& xmap, const CU
   return CB_OK;
 }
 
-// plan of the swizzled kernel: 3 stages of G whole frames (or one row band) in <= 208 KB; a function of the shape only
+// plan of the swizzled kernel: 2 stages of G whole frames (or one row band) in <= 208 KB (measured: two large stages beat three or
+// four smaller ones, the per-item hand-off costs more than the extra depth buys); a function of the shape only
 struct SwPlan { int G, R, nbands, npix_alloc, kext, nstages; size_t stage_bytes, y_off, smem; bool ok; };
 static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
   const int Wp = W + 2;
-  const size_t avail = (size_t)208 * 1024 / 3;
+  const size_t avail = (size_t)208 * 1024 / 2;
   auto a1k = [](size_t b) { return (b + 1023) & ~(size_t)1023; };
   auto stage = [&](int npos, int* kext, int* npix) {
     *kext = (npos + 15) / 16 * 16; *npix = *kext + 2 * Wp + 8;
     return a1k((size_t)*npix * cin * 2) + a1k((size_t)*npix * cout * 2);
   };
-  SwPlan p{1, H, 1, 0, 0, 3, 0, 0, 0, true};
+  SwPlan p{1, H, 1, 0, 0, 2, 0, 0, 0, true};
   int kx, np;
   if (stage((H + 2) * Wp, &kx, &np) <= avail) {
     long best = -1;
@@ -554,8 +555,6 @@ static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
       const long items = (F + G - 1) / G, per_cta = (items + 147) / 148, cost = per_cta * ((long)G * (H + 2) * Wp + 600);
       if (best < 0 || cost < best) { best = cost; p.G = G; }
     }
-  } else if (stage((H + 2) * Wp, &kx, &np) <= (size_t)208 * 1024 / 2) {
-    p.nstages = 2;      // one whole frame per stage, two stages: fewer, longer items than three stages of half frames
   } else {
     int rows = H;
     while (rows > 1 && stage((rows + 2) * Wp, &kx, &np) > avail) --rows;
