@@ -110,7 +110,10 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
   constexpr int TILES_PER_BATCH = TMEM_COLS / COUT;
   __shared__ __align__(8) uint64_t bar_storage;
   __shared__ uint32_t tmem_base_smem;
+  __shared__ __align__(16) float bias_s[32];
   const int tid = threadIdx.x, warp = tid >> 5, wg = warp >> 2, lane_row = tid & 127, Wp = a.W + 2;      // two warpgroups
+  const uint32_t magic_Wp = (uint32_t)((0x100000000ull + (uint64_t)Wp - 1) / (uint64_t)Wp);      // q / Wp = umulhi(q, magic) for q * Wp < 2^32
+  if (tid < COUT) bias_s[tid] = a.bias[tid];
   uint8_t* w_smem = smem; uint8_t* xs = smem + W_BYTES;
   const uint32_t bar = smem_u32(&bar_storage);
   if (tid == 0) mbar_init(bar, 1);
@@ -154,11 +157,12 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
         if (elect_one()) mma_commit(bar);
         __syncwarp();
       }
-      if (!mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 3; }
+      if (warp == 0 && !mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 3; }      // one warp polls; the rest sleep in the barrier
       parity ^= 1;
+      __syncthreads();
       tc_fence_after();
       for (int s = wg; s < nt; s += 2) {      // each warpgroup drains every second accumulator tile
-        const int q = (t0 + s) * 128 + lane_row, yl = q / Wp, x = q - yl * Wp, y = yb + yl;
+        const int q = (t0 + s) * 128 + lane_row, yl = (int)__umulhi((uint32_t)q, magic_Wp), x = q - yl * Wp, y = yb + yl;
         const bool valid = yl < a.R && y < a.H && x < a.W;
         const size_t o = (((size_t)f * a.H + y) * a.W + x) * COUT;
 #pragma unroll
@@ -169,7 +173,10 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
           uint4 o0, o1;
           __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
 #pragma unroll
-          for (int i = 0; i < 16; ++i) v[i] = fmaf(v[i], 1.0f / 255.0f, a.bias[c0 + i]);
+          for (int i = 0; i < 16; i += 4) {
+            const float4 b4 = *reinterpret_cast<const float4*>(bias_s + c0 + i);
+            v[i] = fmaf(v[i], 1.0f / 255.0f, b4.x); v[i + 1] = fmaf(v[i + 1], 1.0f / 255.0f, b4.y); v[i + 2] = fmaf(v[i + 2], 1.0f / 255.0f, b4.z); v[i + 3] = fmaf(v[i + 3], 1.0f / 255.0f, b4.w);
+          }
 #pragma unroll
           for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
           if (fused) {      // keep the band of conv outputs (already rounded to bf16, as the unfused path stores them) in shared memory

@@ -283,12 +283,22 @@ __global__ void __launch_bounds__(NT) conv3x3_tc_kernel(const ConvTcArgs a, cons
 constexpr int PIPE_EPI_WARPS = 16, PIPE_THREADS = (PIPE_EPI_WARPS + 6) * 32, PIPE_MAX_STAGES = 3, PIPE_TBUF = 4;
 struct PipeArgs { ConvTcArgs c; int nstages; uint32_t stage_bytes, magic_R, magic_Wp; };      // magic_x = ceil(2^32 / x): q / x = umulhi(q, magic_x) for the q that occur
 
+// 32-byte global load (sm_100): one thread fetches its whole 16-channel slice of a pixel in one instruction
+__device__ __forceinline__ void ldg256(const void* p, uint4& a, uint4& b) {
+  asm volatile("ld.global.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
+               : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
+}
+
 template <int COUT, int MODE>
 __device__ __forceinline__ void load_aux(const ConvTcArgs& a, size_t o, bool valid, uint4 (&x0)[2], uint4 (&x1)[2]) {
   x0[0] = x0[1] = x1[0] = x1[1] = make_uint4(0, 0, 0, 0);
   if (!valid) return;
-  if (a.aux0) { x0[0] = *reinterpret_cast<const uint4*>(a.aux0 + o); x0[1] = *reinterpret_cast<const uint4*>(a.aux0 + o + 8); }
-  if (MODE == 1 && a.aux1) { x1[0] = *reinterpret_cast<const uint4*>(a.aux1 + o); x1[1] = *reinterpret_cast<const uint4*>(a.aux1 + o + 8); }
+  if (MODE == 0) {      // (measured: the 32-byte form helps the two-operand dgrad epilogue and hurts the forward one)
+    if (a.aux0) { x0[0] = *reinterpret_cast<const uint4*>(a.aux0 + o); x0[1] = *reinterpret_cast<const uint4*>(a.aux0 + o + 8); }
+  } else {
+    if (a.aux0) ldg256(a.aux0 + o, x0[0], x0[1]);
+    if (a.aux1) ldg256(a.aux1 + o, x1[0], x1[1]);
+  }
 }
 
 template <int COUT, int MODE>
@@ -319,7 +329,7 @@ __device__ __forceinline__ void finish_chunk(const ConvTcArgs& a, const float* b
   __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
 #pragma unroll
   for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
-  *reinterpret_cast<uint4*>(a.out + o) = o0;
+  *reinterpret_cast<uint4*>(a.out + o) = o0;      // two 16-byte stores: measured faster than one 32-byte store here
   *reinterpret_cast<uint4*>(a.out + o + 8) = o1;
 }
 
