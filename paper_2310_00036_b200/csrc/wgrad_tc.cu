@@ -330,13 +330,18 @@ __global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nc
 // Swizzled variant (TMA, Cin in {16, 32}): whole pixels are landed once, one shared-memory row of 2*CIN (X) or 2*COUT (DY)
 // bytes per position, in the 32B/64B/128B swizzle pattern.  The A descriptor is MN-major with LBO = one row: the M walk
 // steps to the NEXT POSITION, so rows dj*CIN + c of one MMA are the taps (di, 0..2) without any shifted copy of X
-// (the pattern is a function of the absolute address, so descriptors may start at any row).  Three accumulators
-// [UM x COUT] (one per di) stay in TMEM; the bias gradient is summed from the landed DY rows by the loader warps.
+// (the pattern is a function of the absolute address, so descriptors may start at any row).  The B descriptor walks N the
+// same way with LBO = one image row: column group e of the MMA reads DY one row further down, which pairs it with the tap
+// row di = 2 - e.  ONE MMA [UM x 3*COUT] per 16 positions therefore yields all nine taps; the accumulator stays in TMEM;
+// the bias gradient is summed from the landed DY rows by the loader warps.
 //   warps 0-7  wait for a landed stage, apply the ReLU in place when the layer needs it, add DY into the bias sums
 //   warp 8     MMA issuer        warp 9  TMA producer (ring of `nstages` stages)
 struct WgradSwArgs {
   float* partial; int F, H, W, G, R, nbands, npix_alloc, kext, relu_in, dy_rows, nstages;
-  uint32_t stage_bytes, y_off; int* error_flag;
+  uint32_t stage_bytes, y_off;
+  int dy_off;         // DY position p is stored at row p + dy_off (dy_off >= 2*(W+2), a multiple of the swizzle period)
+  int x_off;          // X position p is stored at row p + x_off (>= 16: the first K step may start up to 15 rows early)
+  int* error_flag;
 };
 constexpr int SW_MAX_STAGES = 3;
 
@@ -388,16 +393,17 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
     for (int it = 0; it < my_items; ++it) {
       const int s = it % NS, use = it / NS;
       if (!mbar_wait(RAW(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 7; }
-      uint8_t* xs = smem + (size_t)s * a.stage_bytes; const uint8_t* ys = xs + a.y_off;
+      uint8_t* xs = smem + (size_t)s * a.stage_bytes; const uint8_t* ys = xs + a.y_off + (size_t)a.dy_off * PY;
       if (a.relu_in) {
         const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
         const int n16 = a.G * Rb * (CIN / 8);
         for (int i = tid; i < n16; i += NLOAD) {      // elementwise: the swizzle does not matter
-          uint4 v = reinterpret_cast<uint4*>(xs)[i];
+          uint4* px = reinterpret_cast<uint4*>(xs + (size_t)a.x_off * PX) + i;
+          uint4 v = *px;
           __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
 #pragma unroll
           for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
-          reinterpret_cast<uint4*>(xs)[i] = v;
+          *px = v;
         }
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
@@ -437,7 +443,7 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
             float v[16];
             tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(acc * COUT + c0), v);
             if (row >= 3 * CIN) continue;
-            const int tap = acc * 3 + row / CIN, r = row % CIN;
+            const int tap = (2 - acc) * 3 + row / CIN, r = row % CIN;      // column group e = acc holds the tap row di = 2 - e
 #pragma unroll
             for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + r) * COUT + c0 + i] = v[i];
           }
@@ -446,26 +452,24 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
     }
   } else if (warp == NLOAD / 32) {
     // ================= MMA issuer =================
-    const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(COUT >> 3) << 17) | ((uint32_t)(UM >> 4) << 24);
+    const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)((3 * COUT) >> 3) << 17) | ((uint32_t)(UM >> 4) << 24);
     const uint32_t a_hi = ((8u * PX) >> 4) | (1u << 14) | (SWX << 29), b_hi = ((8u * PY) >> 4) | (1u << 14) | (SWY << 29);
+    // K runs over stored DY rows r: column group e reads row r + e*Wp = DY position r + e*Wp - dy_off, A reads X position
+    // r - (dy_off - 2*Wp) + dj; with p = r + e*Wp - dy_off this is X[p + (2-e)*Wp + dj] * DY[p]: tap (2-e, dj)
+    const int r_begin = ((a.dy_off - 2 * Wp) / 16) * 16, r_end = a.kext + a.dy_off;
     uint32_t accumulate = 0;
     for (int it = 0; it < my_items; ++it) {
       const int s = it % NS, use = it / NS;
       if (!mbar_wait(a.relu_in ? FULL(s) : RAW(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
       asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
       const uint32_t x_base = smem_u32(smem) + (uint32_t)s * a.stage_bytes, y_base = x_base + a.y_off;
-      // running low words of the descriptors (the start address advances by 16 positions per step); LBO of A = one position
-      uint32_t xl0 = ((x_base >> 4) & 0x3FFFu) | ((PX >> 4) << 16), yl = ((y_base >> 4) & 0x3FFFu) | (1u << 16);
-      uint32_t xl1 = xl0 + (uint32_t)Wp * (PX >> 4), xl2 = xl1 + (uint32_t)Wp * (PX >> 4);
-      const int nk = a.kext >> 4;
+      uint32_t xl = (((x_base >> 4) & 0x3FFFu) | ((PX >> 4) << 16)) + (uint32_t)(a.x_off + r_begin - (a.dy_off - 2 * Wp)) * (PX >> 4);      // LBO = one position
+      uint32_t yl = (((y_base >> 4) & 0x3FFFu) | ((((uint32_t)Wp * PY) >> 4) << 16)) + (uint32_t)r_begin * (PY >> 4);           // LBO = one image row
 #pragma unroll 4
-      for (int k = 0; k < nk; ++k) {
-        const uint64_t bd = ((uint64_t)b_hi << 32) | yl;
-        if (elect_one()) mma_f16(tmem_base, ((uint64_t)a_hi << 32) | xl0, bd, idesc, accumulate);
-        if (elect_one()) mma_f16(tmem_base + (uint32_t)COUT, ((uint64_t)a_hi << 32) | xl1, bd, idesc, accumulate);
-        if (elect_one()) mma_f16(tmem_base + (uint32_t)(2 * COUT), ((uint64_t)a_hi << 32) | xl2, bd, idesc, accumulate);
+      for (int r = r_begin; r < r_end; r += 16) {
+        if (elect_one()) mma_f16(tmem_base, ((uint64_t)a_hi << 32) | xl, ((uint64_t)b_hi << 32) | yl, idesc, accumulate);
         accumulate = 1;
-        xl0 += PX; xl1 += PX; xl2 += PX; yl += PY;      // 16 positions * (pitch / 16)
+        xl += PX; yl += PY;      // 16 positions * (pitch / 16)
       }
       if (elect_one()) mma_commit(SEMPTY(s));
       __syncwarp();
@@ -481,8 +485,8 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
       const int grp = item / a.nbands, band = item - grp * a.nbands, f0 = grp * a.G, yb = band * a.R;
       const uint32_t xs = smem_u32(smem) + (uint32_t)s * a.stage_bytes;
       tma::arrive_expect_tx(RAW(s), xbytes + ybytes);
-      tma::load_4d(xs, &xmap, 0, -1, yb - 1, f0, RAW(s));
-      tma::load_4d(xs + a.y_off, &ymap, 0, 0, yb, f0, RAW(s));
+      tma::load_4d(xs + (uint32_t)a.x_off * PX, &xmap, 0, -1, yb - 1, f0, RAW(s));
+      tma::load_4d(xs + a.y_off + (uint32_t)a.dy_off * PY, &ymap, 0, 0, yb, f0, RAW(s));
     }
   }
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
@@ -538,14 +542,16 @@ static int launch_w(const tcw::WgradTcArgs& a, const CUtensorMap& xmap, const CU
 
 // plan of the swizzled kernel: 2 stages of G whole frames (or one row band) in <= 208 KB (measured: two large stages beat three or
 // four smaller ones, the per-item hand-off costs more than the extra depth buys); a function of the shape only
-struct SwPlan { int G, R, nbands, npix_alloc, kext, nstages; size_t stage_bytes, y_off, smem; bool ok; };
+struct SwPlan { int G, R, nbands, npix_alloc, kext, nstages; size_t stage_bytes, y_off, smem; bool ok; int dy_off, x_off; };
 static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
   const int Wp = W + 2;
   const size_t avail = (size_t)208 * 1024 / 2;
   auto a1k = [](size_t b) { return (b + 1023) & ~(size_t)1023; };
+  const int px = 2 * cin, py = 2 * cout;
+  const int x_off = std::max(16, 1024 / px), per = 1024 / py, dy_off = (2 * Wp + per - 1) / per * per;      // both keep the landed boxes 1024-byte aligned
   auto stage = [&](int npos, int* kext, int* npix) {
     *kext = (npos + 15) / 16 * 16; *npix = *kext + 2 * Wp + 8;
-    return a1k((size_t)*npix * cin * 2) + a1k((size_t)*npix * cout * 2);
+    return a1k((size_t)(x_off + *npix) * px) + a1k((size_t)(dy_off + *npix) * py);
   };
   SwPlan p{1, H, 1, 0, 0, 2, 0, 0, 0, true};
   int kx, np;
@@ -562,7 +568,8 @@ static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
     p.nbands = (H + rows - 1) / rows; p.R = (H + p.nbands - 1) / p.nbands;
   }
   p.stage_bytes = stage(p.G * (p.R + 2) * Wp, &p.kext, &p.npix_alloc);
-  p.y_off = a1k((size_t)p.npix_alloc * cin * 2);
+  p.y_off = a1k((size_t)(x_off + p.npix_alloc) * px);
+  p.dy_off = dy_off; p.x_off = x_off;
   p.smem = 1024 + (size_t)p.nstages * p.stage_bytes;
   return p;
 }
@@ -590,7 +597,7 @@ int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, con
         tma::make_nhwc_map(&ymap, dy, F, g.H, g.W, g.Cout, g.W + 2, dy_rows, q.G, g.Cout, true)) {
       const int nitems = ((F + q.G - 1) / q.G) * q.nbands, grid = std::min(nitems, WGRAD_TC_MAX_CTAS);
       tcw::WgradSwArgs a{partial, F, g.H, g.W, q.G, q.R, q.nbands, q.npix_alloc, q.kext, relu_in ? 1 : 0, dy_rows, q.nstages,
-                         (uint32_t)q.stage_bytes, (uint32_t)q.y_off, error_flag};
+                         (uint32_t)q.stage_bytes, (uint32_t)q.y_off, q.dy_off, q.x_off, error_flag};
       int rc;
       if (g.Cin == 16 && g.Cout == 16) rc = launch_sw<16, 16>(a, xmap, ymap, q.smem, grid, st);
       else if (g.Cin == 16) rc = launch_sw<16, 32>(a, xmap, ymap, q.smem, grid, st);
