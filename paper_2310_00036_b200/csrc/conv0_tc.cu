@@ -25,6 +25,7 @@ struct Args {
   const bf16* dy; float* partial;                 // wgrad: dy [F,H,W,COUT], partial [grid][3][24][COUT]
   const uint8_t* pool_arg; const bf16* dpool;     // wgrad, fused max-pool adjoint: dy is gathered from dpool [F,Ho,Wo,COUT] through pool_arg
   int F, H, W, CIN, R, nbands, npix_alloc, kext;
+  int w_xoff, w_yoff, w_ybytes;   // wgrad: X position p at plane row p + w_xoff; DY position p at row p + w_yoff of the swizzled DY region, w_ybytes per stage
   bf16* pool_out; uint8_t* pool_arg_out; int Rp;  // forward, fused 3x3 s2 SAME max-pool: pooled map + arg-max positions; Rp pooled rows per band
   int* error_flag;
 };
@@ -83,21 +84,27 @@ __device__ __forceinline__ bool pool_item(const PoolGeom& q, int p, int i, int y
   oy = first + 2 * iy; ox = pb + 2 * ix;
   return true;
 }
-__device__ __forceinline__ void pool_scatter(const Args& a, const PoolGeom& q, uint8_t* ys, uint32_t P, int yb, int oy, int ox, int ch,
+// DY region of the weight-gradient kernel: one row of PY = 2*COUT bytes per position in the 32B/64B swizzle pattern (16-byte
+// chunk c of a row sits at chunk c ^ (address bits 7..)), the layout the MN-major B descriptor with LBO = one image row reads
+template <int COUT>
+__device__ __forceinline__ uint8_t* dy_chunk(uint8_t* ys, uint32_t ys_addr, int pos, int ch) {
+  constexpr uint32_t PY = 2u * COUT;
+  const uint32_t row = ys_addr + (uint32_t)pos * PY;
+  return ys + (size_t)pos * PY + (((uint32_t)ch ^ ((row >> 7) & (COUT / 8 - 1))) << 4);
+}
+template <int COUT>
+__device__ __forceinline__ void pool_scatter(const Args& a, const PoolGeom& q, uint8_t* ys, uint32_t ys_addr, int yb, int oy, int ox, int ch,
                                              uint2 pk, uint4 dv) {
   const int Wp = a.W + 2, rows = min(a.R, a.H - yb);
   const int y0 = oy * 2 - q.ph - yb, x0 = ox * 2 - q.pw;
-  uint8_t* base = ys + (size_t)ch * P;
   const uint16_t* h = reinterpret_cast<const uint16_t*>(&dv);
 #pragma unroll
   for (int k = 0; k < 8; ++k) {
     const uint32_t arg = ((k < 4 ? pk.x : pk.y) >> (8 * (k & 3))) & 255u;
     const int wy = (int)((arg * 11u) >> 5), wx = (int)arg - 3 * wy;
     const int yl = y0 + wy;
-    if ((unsigned)yl < (unsigned)rows) {
-      uint16_t* p = reinterpret_cast<uint16_t*>(base + (size_t)(yl * Wp + x0 + wx) * 16) + k;
-      pool::add_bf16(p, h[k]);
-    }
+    if ((unsigned)yl < (unsigned)rows)
+      pool::add_bf16(reinterpret_cast<uint16_t*>(dy_chunk<COUT>(ys, ys_addr, yl * Wp + x0 + wx, ch)) + k, h[k]);
   }
 }
 
@@ -229,17 +236,20 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 
 constexpr int WNLOAD = 512;     // warps 0-15 stage (the gather is latency-bound: more loads in flight); warps 0-1 later drain TMEM; warp 16 issues the MMAs
 
-// Two stages of (X plane, DY planes): the loaders fill one while the tensor core reads the other.  UMMA M = 64:
-// accumulator row r = 8*dj + c sits in TMEM lane 32*(r/16) + r%16.
+// Two stages of (X plane, DY region): the loaders fill one while the tensor core reads the other.  ONE MMA [64 x 3*COUT] per
+// 16 positions: the A descriptor walks M over neighbouring positions (rows 8*dj + c), the B descriptor walks N over image rows
+// of the swizzled DY region (column group e pairs with the tap row di = 2 - e; see wgrad_tc.cu).  Accumulator row r sits in
+// TMEM lane 32*(r/16) + r%16.
 template <int COUT>
 __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) {
-  extern __shared__ __align__(128) uint8_t smem[];
+  extern __shared__ __align__(128) uint8_t smem_raw[];
   constexpr int YCH = COUT / 8;
-  constexpr uint32_t TCOLS = 128;
+  constexpr uint32_t TCOLS = 128, PY = 2u * COUT, SWY = COUT == 16 ? 6u : 4u;
   __shared__ __align__(8) uint64_t bars[5];       // full[2], empty[2], done
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5, Wp = a.W + 2;
-  const uint32_t P = (uint32_t)a.npix_alloc * 16u, STAGE = (1u + YCH) * P;
+  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  const uint32_t XB = (((uint32_t)(a.w_xoff + a.npix_alloc) * 16u) + 1023u) & ~1023u, STAGE = XB + (uint32_t)a.w_ybytes;
   const uint32_t bar0 = smem_u32(&bars[0]);
   if (tid == 0) {
     for (int i = 0; i < 5; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
@@ -248,8 +258,8 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
   if (warp == WNLOAD / 32) tmem_alloc(smem_u32(&tmem_base_smem), TCOLS);
   for (int st = 0; st < 2; ++st) {
     uint8_t* xs = smem + (size_t)st * STAGE;
-    for (int i = tid; i < a.npix_alloc; i += WNLOAD + 32) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
-    for (uint32_t i = tid; i < P * YCH / 16; i += WNLOAD + 32) reinterpret_cast<uint4*>(xs + P)[i] = make_uint4(0, 0, 0, 0);
+    for (uint32_t i = tid; i < XB / 16; i += WNLOAD + 32) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
+    for (uint32_t i = tid; i < (uint32_t)a.w_ybytes / 16; i += WNLOAD + 32) reinterpret_cast<uint4*>(xs + XB)[i] = make_uint4(0, 0, 0, 0);
   }
   fence_async_smem();
   tc_fence_before(); __syncthreads(); tc_fence_after();
@@ -274,7 +284,8 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
         }
       }
       if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 4; }
-      uint8_t* xs = smem + (size_t)s * STAGE; uint8_t* ys = xs + P;
+      uint8_t* xs = smem + (size_t)s * STAGE + (size_t)a.w_xoff * 16; uint8_t* ys = smem + (size_t)s * STAGE + XB + (size_t)a.w_yoff * PY;
+      const uint32_t ys_addr = smem_u32(ys);
       const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
       stage_band(a, xs, fr, yb, tid, WNLOAD);
       if (a.pool_arg == nullptr) {
@@ -282,19 +293,19 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
           int ch = i % YCH, pos = i / YCH, yl = pos / Wp, x = pos - yl * Wp, y = yb + yl;
           uint4 v = make_uint4(0, 0, 0, 0);
           if (yl < a.R && y < a.H && x < a.W) v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)f * a.H + y) * a.W + x) * COUT + ch * 8);
-          *reinterpret_cast<uint4*>(ys + (size_t)ch * P + (size_t)pos * 16) = v;
+          *reinterpret_cast<uint4*>(dy_chunk<COUT>(ys, ys_addr, pos, ch)) = v;
         }
       } else {
         for (int i = tid; i < a.kext * YCH; i += WNLOAD)
-          *reinterpret_cast<uint4*>(ys + (size_t)(i % YCH) * P + (size_t)(i / YCH) * 16) = make_uint4(0, 0, 0, 0);
+          reinterpret_cast<uint4*>(ys)[i] = make_uint4(0, 0, 0, 0);
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
           asm volatile("bar.sync 1, %0;\n" :: "n"(WNLOAD) : "memory");
-          if (pf_ok[p]) pool_scatter(a, q, ys, P, yb, pf_oy[p], pf_ox[p], pf_ch[p], pf_pk[p], pf_dv[p]);
+          if (pf_ok[p]) pool_scatter<COUT>(a, q, ys, ys_addr, yb, pf_oy[p], pf_ox[p], pf_ch[p], pf_pk[p], pf_dv[p]);
           for (int i = tid + WNLOAD; ; i += WNLOAD) {
             int oy, ox, ch; if (!pool_item(q, p, i, YCH, oy, ox, ch)) break;
             const size_t o = (((size_t)f * q.Ho + oy) * q.Wo + ox) * COUT + ch * 8;
-            pool_scatter(a, q, ys, P, yb, oy, ox, ch, *reinterpret_cast<const uint2*>(a.pool_arg + o), *reinterpret_cast<const uint4*>(a.dpool + o));
+            pool_scatter<COUT>(a, q, ys, ys_addr, yb, oy, ox, ch, *reinterpret_cast<const uint2*>(a.pool_arg + o), *reinterpret_cast<const uint4*>(a.dpool + o));
           }
         }
       }
@@ -314,31 +325,28 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
           tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(di * COUT + c0), v);
           if (row < 24) {
 #pragma unroll
-            for (int i = 0; i < 16; ++i) out[((size_t)di * 24 + row) * COUT + c0 + i] = v[i];
+            for (int i = 0; i < 16; ++i) out[((size_t)(2 - di) * 24 + row) * COUT + c0 + i] = v[i];      // column group e = di holds the tap row 2 - e
           }
         }
       }
     }
   } else {      // warp WNLOAD / 32: the whole warp runs the loop, one elected lane issues
-    const uint32_t idesc = make_idesc(64, COUT, 1, 1);
-    const uint32_t a_hi = 1u | (1u << 14), b_hi = ((P >> 4) & 0x3FFFu) | (1u << 14);     // A: SBO = 16 B (M walk); B: SBO = plane
+    const uint32_t idesc = make_idesc(64, 3 * COUT, 1, 1);
+    const uint32_t a_hi = 1u | (1u << 14), b_hi = ((8u * PY) >> 4) | (1u << 14) | (SWY << 29);     // A: SBO = 16 B (M walk); B: SBO = 8 rows, swizzled
+    const int r_begin = ((a.w_yoff - 2 * Wp) / 16) * 16, r_end = a.kext + a.w_yoff;               // stored DY rows the contraction runs over
     uint32_t accumulate = 0;
     for (int it = 0; it < my_items; ++it) {
       const int s = it & 1, use = it >> 1;
       if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 4; }
       tc_fence_after();
-      const uint32_t x_base = smem_u32(smem + (size_t)s * STAGE), y_base = x_base + P;
-      uint32_t xl0 = ((x_base >> 4) & 0x3FFFu) | (8u << 16), yl = ((y_base >> 4) & 0x3FFFu) | (8u << 16);      // running low words; LBO = 128 B
-      uint32_t xl1 = xl0 + (uint32_t)Wp, xl2 = xl1 + (uint32_t)Wp;
-      const int nk = a.kext >> 4;
+      const uint32_t x_base = smem_u32(smem + (size_t)s * STAGE), y_base = x_base + XB;
+      uint32_t xl = (((x_base >> 4) & 0x3FFFu) | (8u << 16)) + (uint32_t)(a.w_xoff + r_begin - (a.w_yoff - 2 * Wp));      // LBO = 128 B; 16 B per position
+      uint32_t yl = (((y_base >> 4) & 0x3FFFu) | ((((uint32_t)Wp * PY) >> 4) << 16)) + (uint32_t)r_begin * (PY >> 4);  // LBO = one image row
 #pragma unroll 4
-      for (int k = 0; k < nk; ++k) {
-        const uint64_t bd = ((uint64_t)b_hi << 32) | yl;
-        if (elect_one()) mma_f16(tmem_base, ((uint64_t)a_hi << 32) | xl0, bd, idesc, accumulate);
-        if (elect_one()) mma_f16(tmem_base + (uint32_t)COUT, ((uint64_t)a_hi << 32) | xl1, bd, idesc, accumulate);
-        if (elect_one()) mma_f16(tmem_base + (uint32_t)(2 * COUT), ((uint64_t)a_hi << 32) | xl2, bd, idesc, accumulate);
+      for (int r = r_begin; r < r_end; r += 16) {
+        if (elect_one()) mma_f16(tmem_base, ((uint64_t)a_hi << 32) | xl, ((uint64_t)b_hi << 32) | yl, idesc, accumulate);
         accumulate = 1;
-        xl0 += 16u; xl1 += 16u; xl2 += 16u; yl += 16u;      // 16 positions of 16 bytes
+        xl += 16u; yl += PY;
       }
       if (elect_one()) mma_commit(bar0 + 8u * (2 + s));
       __syncwarp();
@@ -411,7 +419,7 @@ int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* fr
   }
   const int npix = ((R * Wp + 127) / 128) * 128 + 2 * Wp + 8;
   const size_t smem = (size_t)6 * 2 * g.Cout * 16 + (size_t)npix * 16 + ctile;
-  tc0::Args a{obs, frame_idx, wimg, bias, out, nullptr, nullptr, nullptr, nullptr, F, g.H, g.W, g.Cin, R, nb, npix, 0, pool_out, pool_arg, Rp, error_flag};
+  tc0::Args a{obs, frame_idx, wimg, bias, out, nullptr, nullptr, nullptr, nullptr, F, g.H, g.W, g.Cin, R, nb, npix, 0, 0, 0, 0, pool_out, pool_arg, Rp, error_flag};
   const int grid = std::min(F * nb, 296);
   static size_t c16 = 0, c32 = 0; int rc;
   if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_fwd_kernel<16>, smem, &c16))) return rc; tc0::conv0_fwd_kernel<16><<<grid, 256, smem, st>>>(a); }
@@ -423,15 +431,21 @@ int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* fr
 int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* dy, const uint8_t* pool_arg,
                        const bf16* dpool, float* partial, float* grad, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
-  const int Wp = g.W + 2, ych = g.Cout / 8;
-  const int maxpos = (int)(100 * 1024 / 16 / (1 + ych));      // two stages of (1 + ych) planes in <= 200 KB
-  int R = std::min(g.H, (maxpos - 2 * Wp - 48) / Wp); if (R < 1) R = 1;
+  const int Wp = g.W + 2, py = 2 * g.Cout;
+  const int xoff = 16, per = 1024 / py, yoff = (2 * Wp + per - 1) / per * per;      // the swizzled DY rows start on a 1024-byte boundary
+  auto a1k = [](size_t b) { return (b + 1023) & ~(size_t)1023; };
+  auto plan = [&](int R, int* kext, int* npix, size_t* ybytes) {      // bytes of one stage (X plane + DY region) for bands of R rows
+    *kext = (R * Wp + 15) / 16 * 16; *npix = (*kext + 2 * Wp + 40 + 7) / 8 * 8;
+    *ybytes = a1k((size_t)(yoff + *npix) * py);
+    return a1k((size_t)(xoff + *npix) * 16) + *ybytes;
+  };
+  int kext, npix; size_t ybytes;
+  int R = g.H; while (R > 1 && 2 * plan(R, &kext, &npix, &ybytes) + 1024 > (size_t)200 * 1024) --R;
   const int nb = (g.H + R - 1) / R; R = (g.H + nb - 1) / nb;
-  const int kext = (R * Wp + 15) / 16 * 16;
-  const int npix = (kext + 2 * Wp + 40 + 7) / 8 * 8;
-  const size_t smem = (size_t)2 * (1 + ych) * npix * 16;
+  const size_t smem = 2 * plan(R, &kext, &npix, &ybytes) + 1024;
   const int grid = std::min(F * nb, CONV0_MAX_CTAS);
-  tc0::Args a{obs, frame_idx, nullptr, nullptr, nullptr, dy, partial, pool_arg, dpool, F, g.H, g.W, g.Cin, R, nb, npix, kext, nullptr, nullptr, 0, error_flag};
+  tc0::Args a{obs, frame_idx, nullptr, nullptr, nullptr, dy, partial, pool_arg, dpool, F, g.H, g.W, g.Cin, R, nb, npix, kext, xoff, yoff, (int)ybytes,
+              nullptr, nullptr, 0, error_flag};
   static size_t c16 = 0, c32 = 0; int rc;
   if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_wgrad_kernel<16>, smem, &c16))) return rc; tc0::conv0_wgrad_kernel<16><<<grid, tc0::WNLOAD + 32, smem, st>>>(a); }
   else { if ((rc = set_smem(tc0::conv0_wgrad_kernel<32>, smem, &c32))) return rc; tc0::conv0_wgrad_kernel<32><<<grid, tc0::WNLOAD + 32, smem, st>>>(a); }
