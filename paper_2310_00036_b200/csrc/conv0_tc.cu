@@ -267,8 +267,12 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
   const int nitems = a.F * a.nbands;
   const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
   if (warp < WNLOAD / 32) {
-    for (int it = 0; it < my_items; ++it) {
-      const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
+    // two loader teams of eight warps; team t stages the items it = t, t+2, ... into stage t, so the global-load latencies and the
+    // barrier chains of two consecutive items overlap
+    constexpr int TN = WNLOAD / 2;
+    const int team = tid / TN, ttid = tid - team * TN;
+    for (int it = team; it < my_items; it += 2) {
+      const int item = blockIdx.x + it * gridDim.x, s = team, use = it >> 1;
       const int f = item / a.nbands, yb = (item - f * a.nbands) * a.R;
       // the pooled gradients of this thread's first item of each phase are fetched before anything waits
       PoolGeom q; bool pf_ok[4] = {false, false, false, false}; int pf_oy[4], pf_ox[4], pf_ch[4]; uint2 pf_pk[4]; uint4 pf_dv[4];
@@ -276,7 +280,7 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
         q = pool_geom(a, yb);
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
-          pf_ok[p] = pool_item(q, p, tid, YCH, pf_oy[p], pf_ox[p], pf_ch[p]);
+          pf_ok[p] = pool_item(q, p, ttid, YCH, pf_oy[p], pf_ox[p], pf_ch[p]);
           if (pf_ok[p]) {
             const size_t o = (((size_t)f * q.Ho + pf_oy[p]) * q.Wo + pf_ox[p]) * COUT + pf_ch[p] * 8;
             pf_pk[p] = *reinterpret_cast<const uint2*>(a.pool_arg + o); pf_dv[p] = *reinterpret_cast<const uint4*>(a.dpool + o);
@@ -287,22 +291,22 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
       uint8_t* xs = smem + (size_t)s * STAGE + (size_t)a.w_xoff * 16; uint8_t* ys = smem + (size_t)s * STAGE + XB + (size_t)a.w_yoff * PY;
       const uint32_t ys_addr = smem_u32(ys);
       const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
-      stage_band(a, xs, fr, yb, tid, WNLOAD);
+      stage_band(a, xs, fr, yb, ttid, TN);
       if (a.pool_arg == nullptr) {
-        for (int i = tid; i < a.kext * YCH; i += WNLOAD) {
+        for (int i = ttid; i < a.kext * YCH; i += TN) {
           int ch = i % YCH, pos = i / YCH, yl = pos / Wp, x = pos - yl * Wp, y = yb + yl;
           uint4 v = make_uint4(0, 0, 0, 0);
           if (yl < a.R && y < a.H && x < a.W) v = *reinterpret_cast<const uint4*>(a.dy + (((size_t)f * a.H + y) * a.W + x) * COUT + ch * 8);
           *reinterpret_cast<uint4*>(dy_chunk<COUT>(ys, ys_addr, pos, ch)) = v;
         }
       } else {
-        for (int i = tid; i < a.kext * YCH; i += WNLOAD)
+        for (int i = ttid; i < a.kext * YCH; i += TN)
           reinterpret_cast<uint4*>(ys)[i] = make_uint4(0, 0, 0, 0);
 #pragma unroll
         for (int p = 0; p < 4; ++p) {
-          asm volatile("bar.sync 1, %0;\n" :: "n"(WNLOAD) : "memory");
+          asm volatile("bar.sync %0, %1;\n" :: "r"(1 + team), "n"(TN) : "memory");
           if (pf_ok[p]) pool_scatter<COUT>(a, q, ys, ys_addr, yb, pf_oy[p], pf_ox[p], pf_ch[p], pf_pk[p], pf_dv[p]);
-          for (int i = tid + WNLOAD; ; i += WNLOAD) {
+          for (int i = ttid + TN; ; i += TN) {
             int oy, ox, ch; if (!pool_item(q, p, i, YCH, oy, ox, ch)) break;
             const size_t o = (((size_t)f * q.Ho + oy) * q.Wo + ox) * COUT + ch * 8;
             pool_scatter<COUT>(a, q, ys, ys_addr, yb, oy, ox, ch, *reinterpret_cast<const uint2*>(a.pool_arg + o), *reinterpret_cast<const uint4*>(a.dpool + o));
@@ -310,8 +314,8 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
         }
       }
       fence_async_smem();
-      asm volatile("bar.sync 1, %0;\n" :: "n"(WNLOAD) : "memory");
-      if (tid == 0) mbar_arrive(bar0 + 8u * s);
+      asm volatile("bar.sync %0, %1;\n" :: "r"(1 + team), "n"(TN) : "memory");
+      if (ttid == 0) mbar_arrive(bar0 + 8u * s);
     }
     if (warp < 2) {
       if (my_items > 0 && !mbar_wait(bar0 + 8u * 4, 0u)) { if (a.error_flag) *a.error_flag = 4; }
