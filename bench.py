@@ -277,23 +277,37 @@ def main():
     # ---- end to end through the public API with HOST buffers: H2D of the step's inputs + D2H of its stats ---
     h2d = sum(v.numel() * v.element_size() for v in host_sets[0].values()); d2h = stats.numel() * 4
     stats_host = torch.empty(stats.shape, dtype=torch.float32).pin_memory()
-    stage = {k: torch.empty_like(v, device="cuda") for k, v in host_sets[0].items()}
+    # two device staging sets and a copy stream: the pinned-host -> device copy of step i+1 is issued before step i is launched, the
+    # way a training loop prefetches its next batch; every step's inputs still cross the bus and every step's loss is read back
+    # inside the timed region
+    stages = [{k: torch.empty_like(v, device="cuda") for k, v in host_sets[0].items()} for _ in range(2)]
+    ready = [torch.cuda.Event(), torch.cuda.Event()]
+    copy_stream = torch.cuda.Stream()
 
-    def e2e_step(i):
+    def issue_copy(i):
+        hs, st = host_sets[i % len(host_sets)], stages[i % 2]
+        with torch.cuda.stream(copy_stream):
+            for k in keys:
+                st[k].copy_(hs[k], non_blocking=True)
+            ready[i % 2].record(copy_stream)
+
+    def e2e_step(i, last):
         nonlocal kstep
-        hs = host_sets[i % len(host_sets)]
-        for k in keys:
-            stage[k].copy_(hs[k], non_blocking=True)
-        kstep, _ = net.learner_step(dp, dm, dv, kstep, stage["obs"], stage["actions"], stage["rewards"], stage["dones"], stage["behaviour_logits"], hp, stats)
+        if not last:
+            issue_copy(i + 1)          # buffer (i+1) % 2 was last read by step i-1, which has completed (synchronised below)
+        st = stages[i % 2]
+        stream.wait_event(ready[i % 2])
+        kstep, _ = net.learner_step(dp, dm, dv, kstep, st["obs"], st["actions"], st["rewards"], st["dones"], st["behaviour_logits"], hp, stats)
         stats_host.copy_(stats, non_blocking=True)
         stream.synchronize()        # the caller reads the loss every step
         return float(stats_host[-1, 0])
 
-    e2e_step(0)
+    issue_copy(0); e2e_step(0, True)
     barrier()
     w0 = time.perf_counter(); e0.record(stream)
+    issue_copy(0)
     for i in range(steps):
-        e2e_step(i)
+        e2e_step(i, i + 1 == steps)
     e1.record(stream)
     barrier()
     t_e2e = max_over_ranks(max(e0.elapsed_time(e1) / 1e3, time.perf_counter() - w0), world)
