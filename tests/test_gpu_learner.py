@@ -330,3 +330,94 @@ def test_learner_impala_wide_small():
     the 64-output weight gradients and the Cin = 64 gradients computed as two 32-channel launches."""
     net, got, ref, ctx = _run_learner(synth.IMPALA_WIDE, "impala", "bf16", 2, 2, 1005, blobs=True, warm=True)
     _check_learner(synth.IMPALA_WIDE, got, ref, ctx, "bf16", False)
+
+
+def _step_views(arch, prec, T, B, bt, params, **kw):
+    hp, _ = _hp_pair("impala", prec, T, B, **kw)
+    net = binding.Net(arch); P = params.size
+    dp, dm, dv = dev(params), dev(np.zeros(P, np.float32)), dev(np.zeros(P, np.float32))
+    args = [dev(np.ascontiguousarray(bt[k])) for k in ("obs", "actions", "rewards", "dones", "behaviour_logits")]
+    _, stats = net.learner_step(dp, dm, dv, 0, *args, hp)
+    torch.cuda.synchronize()
+    assert np.isfinite(host(stats)).all()
+    return host(net.learner_view(0)).reshape(-1, arch.n_actions + 1), host(net.learner_view(3))
+
+
+def test_learner_config2_full_size():
+    """BASELINE.json configs[2] at full size, in the launch configuration bench.py times (2688 frames: every CTA of the persistent
+    tensor-core kernels walks ~18 items, so stage rings wrap and barrier phases flip many times -- paths the small cases above,
+    where a CTA sees at most one item, never reach).  The oracle needs ~6 min for this batch, so:
+    (1) forward: the heads of sampled frames against the oracle (first / last items of several CTAs);
+    (2) a property that holds at any size: with sum reduction the loss is a sum over envs, so the gradient of the full batch is
+        the sum of the gradients of env sub-batches.  Halves (1344 frames, still no split-K in fc): heads bitwise equal (a frame's
+        forward does not depend on its neighbours), gradients equal up to fp32 summation order (2e-4 per tensor: the first layer sums
+        1.9e7 cancelling terms per weight; measured 5e-5).  32 chunks of 4 envs (84 frames:
+        ONE item per CTA, the regime the oracle-checked small cases cover; fc switches to split-K there, which re-rounds the
+        hidden layer in bf16): heads within 2e-3, summed gradient within 1e-2 per tensor -- a dropped, duplicated or stale item
+        among a CTA's ~18 would show as >= 5e-2;
+    (3) bf16 tensor-core mode against the library's fp32 reference mode (generic SIMT kernels) on the same inputs: heads of all
+        frames within the bf16 bound (A15b); gradients per tensor within 0.5 relative L2 -- loose on purpose: the end-to-end
+        difference between the two precisions is dominated by value noise (the same comparison on 40 frames gives 0.1-0.25
+        in stage 0 and 1e-2 at the heads), it only guards against gross errors."""
+    arch = synth.IMPALA; T, B = 20, 128; A = arch.n_actions
+    bt = _batch(arch, T, B, 2002, blobs=True)
+    params = synth.gen_params(arch, 2007, bias_scale=0.05, head_scale=0.1)
+    layout = binding.Net(arch).param_layout()
+    frames = bt["obs"].reshape((T + 1) * B, arch.in_c, arch.in_h, arch.in_w)
+    # (1)
+    head, grad = _step_views(arch, "bf16", T, B, bt, params)
+    sel = np.array([0, 1, 147, 148, 1343, 2000, 2686, 2687])
+    rl, rv = oracle.forward(orc_arch(arch), params, frames[sel])
+    close_bf16(head[sel, :A], rl, "logits at full size"); close_bf16(head[sel, A], rv, "value at full size")
+    # (2)
+    head_s, grad_s = _step_views(arch, "bf16", T, B, bt, params, loss_reduction=1)
+    assert np.array_equal(head_s, head)
+
+    def sub(lo, n):
+        return {k: (v[:, lo:lo + n] if k != "obs" else v[:, lo:lo + n]) for k, v in bt.items()}
+
+    def frame_rows(lo, n):
+        return (np.arange(T + 1)[:, None] * B + lo + np.arange(n)[None, :]).reshape(-1)
+
+    for n, htol, gtol in ((64, 0.0, 2e-4), (4, 2e-3, 1e-2)):
+        acc = np.zeros(grad_s.shape, np.float64)
+        for lo in range(0, B, n):
+            h, g = _step_views(arch, "bf16", T, n, sub(lo, n), params, loss_reduction=1)
+            ref = head_s[frame_rows(lo, n)]
+            if htol == 0.0:
+                assert np.array_equal(h, ref), f"heads of envs {lo}..{lo + n - 1} differ between the full batch and the half batch"
+            else:
+                assert rel_l2(h, ref) <= htol, f"heads of envs {lo}..{lo + n - 1}: rel L2 {rel_l2(h, ref):.2e}"
+            acc += g
+        for name, off, shape in layout:
+            m = int(np.prod(shape)); e = rel_l2(acc[off:off + m], grad_s[off:off + m])
+            assert e <= gtol, f"gradient of {name}: full batch vs sum over {B // n} sub-batches of {n} envs: rel L2 {e:.2e} > {gtol}"
+    # (3)
+    head32, grad32 = _step_views(arch, "fp32", T, B, bt, params)
+    close(head32[sel, :A], rl, 1e-4, what="fp32 logits at full size")
+    close_bf16(head, head32, "heads, all frames, bf16 vs fp32 mode")
+    for name, off, shape in layout:
+        m = int(np.prod(shape)); e = rel_l2(grad[off:off + m], grad32[off:off + m])
+        assert e <= 0.5, f"gradient of {name}: relative L2 {e:.3e} between bf16 tensor-core mode and fp32 reference mode"
+
+
+def test_learner_wide_multi_item_batch_split():
+    """The wide network (BASELINE.json configs[4] architecture: 64-channel layers, row-banded staging at 42x42, the plane-layout
+    weight-gradient kernel for Cin = 64) with 672 frames, several items per CTA: the sum-reduction gradient of the batch equals the
+    sum over env sub-batches of 16 and of 4 envs (84 frames: at most one item per CTA), heads bitwise equal (fc uses the same
+    split-K policy at all three sizes)."""
+    arch = synth.ArchSpec("impala", (32, 64, 64), 512, 18, 4, 84, 84); T, B = 20, 32
+    bt = _batch(arch, T, B, 3003, blobs=True)
+    params = synth.gen_params(arch, 3007, bias_scale=0.05, head_scale=0.1)
+    layout = binding.Net(arch).param_layout()
+    head, grad = _step_views(arch, "bf16", T, B, bt, params, loss_reduction=1)
+    for n in (16, 4):
+        acc = np.zeros(grad.shape, np.float64)
+        for lo in range(0, B, n):
+            h, g = _step_views(arch, "bf16", T, n, {k: v[:, lo:lo + n] for k, v in bt.items()}, params, loss_reduction=1)
+            rows = (np.arange(T + 1)[:, None] * B + lo + np.arange(n)[None, :]).reshape(-1)
+            assert np.array_equal(h, head[rows]), f"heads of envs {lo}..{lo + n - 1} differ between batch sizes {B} and {n}"
+            acc += g
+        for name, off, shape in layout:
+            m = int(np.prod(shape)); e = rel_l2(acc[off:off + m], grad[off:off + m])
+            assert e <= 2e-4, f"gradient of {name}: batch of {B} vs sum over sub-batches of {n} envs: rel L2 {e:.2e}"
