@@ -92,7 +92,10 @@ int cb_net_init(const cb_net* net, uint64_t seed, float* params_host);
 /* ---- actor side (Alg. 1 l.8) ------------------------------------------------ */
 /* logits, value = net(obs);  actions[b] = argmax_i(logits[b,i] + Gumbel_i), the Gumbel noise
  * from Philox4x32-10 with key = seed and counter = (env_offset + b, step_lo, step_hi, i/4), word
- * i%4 (A9).  params: dev [P] fp32.  obs: dev uint8 [B,in_c,in_h,in_w].  precision: CB_PREC_*.
+ * i%4 (A9).  params: dev [P] fp32, or NULL to reuse the operand-layout weights packed by the previous
+ * call on this net in the same precision mode (an actor takes new parameters from its queue once
+ * per rollout, not per step: Figure 1 / PAPER.md:148-150; CB_EINVAL if there was no such call).  obs: dev uint8
+ * [B,in_c,in_h,in_w].  precision: CB_PREC_*.
  * Outputs (dev): logits fp32 [B,A], value fp32 [B], actions int32 [B]; any may be NULL. */
 int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int B, uint64_t seed,
                       uint64_t step, uint32_t env_offset, int precision, float* logits, float* value,

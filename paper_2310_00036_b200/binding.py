@@ -149,10 +149,12 @@ class Net:
         return p
 
     def policy_forward(self, params, obs, seed=0, step=0, env_offset=0, precision="bf16", want_actions=True):
-        """cb_policy_forward on the current torch stream.  params: cuda fp32 [P]; obs: cuda uint8 [B,C,H,W].
-        Returns (logits [B,A], value [B], actions int32 [B])."""
+        """cb_policy_forward on the current torch stream.  params: cuda fp32 [P], or None to reuse the weights packed by the
+        previous call in this precision mode; obs: cuda uint8 [B,C,H,W].  Returns (logits [B,A], value [B], actions int32 [B])."""
         torch = _torch()
-        _dev(params, torch.float32, "params"); _dev(obs, torch.uint8, "obs")
+        if params is not None:
+            _dev(params, torch.float32, "params")
+        _dev(obs, torch.uint8, "obs")
         B = obs.shape[0]
         logits = torch.empty((B, self.A), dtype=torch.float32, device=obs.device)
         value = torch.empty((B,), dtype=torch.float32, device=obs.device)

@@ -294,13 +294,14 @@ static bool misaligned(const void* p, size_t a) { return ((uintptr_t)p & (a - 1)
 
 int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int B, uint64_t seed, uint64_t step, uint32_t env_offset,
                       int precision, float* logits, float* value, int32_t* actions, void* stream) {
-  if (!net || !params || !obs || B < 0) { set_error("null or negative argument"); return CB_EINVAL; }
+  if (!net || !obs || B < 0) { set_error("null or negative argument"); return CB_EINVAL; }
   if (check_prec(precision)) return CB_EINVAL;
-  if (misaligned(params, 16)) { set_error("params must be 16-byte aligned"); return CB_EINVAL; }
+  if (params && misaligned(params, 16)) { set_error("params must be 16-byte aligned"); return CB_EINVAL; }
   if (B == 0) return CB_OK;
   cudaStream_t st = (cudaStream_t)stream; int rc;
   if ((rc = ensure_workspace(net, precision, B))) return rc;
-  if ((rc = pack_weights(net, precision, params, st))) return rc;
+  if (params) { if ((rc = pack_weights(net, precision, params, st))) return rc; }
+  else if (!net->ws[precision].packed) { set_error("params == NULL but no weights have been packed in this precision mode yet"); return CB_EINVAL; }
   if ((rc = forward(net, precision, obs, nullptr, B, st, true))) return rc;      // everything up to the hidden layer
   Workspace& ws = net->ws[precision];
   const Layer& HL = net->layers.back();

@@ -75,6 +75,7 @@ struct Workspace {     // one per precision mode
   std::vector<void*> act;            // per tensor, [frames * per_frame]
   void* grad[G_COUNT] = {nullptr, nullptr, nullptr, nullptr, nullptr};
   void* wf = nullptr; void* wd = nullptr; float* bias = nullptr;   // packed weights (mode type), fp32 bias
+  bool packed = false;                                             // the packs hold the params of the last pack_weights call
   bf16* w0img = nullptr;                                           // first-layer forward B image (conv0_tc.cu)
   bf16* wtc_f = nullptr; bf16* wtc_d = nullptr;                     // tcgen05 B-operand packs (forward / dgrad), bf16 mode only
   PackDesc* packtab = nullptr;                                     // device copy of the layer table for packing

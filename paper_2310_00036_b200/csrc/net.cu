@@ -74,7 +74,7 @@ __global__ void pack_all_kernel(const float* __restrict__ params, const PackDesc
 template <typename AT>
 static int pack_all(cb_net* net, Workspace& ws, const float* params, cudaStream_t st) {
   ProfScope ps(K_PACK, st, 1, 0.0, (double)net->P * (4 + 2 * sizeof(AT)));
-  dim3 grid(64, (unsigned)net->layers.size());
+  dim3 grid(296, (unsigned)net->layers.size());      // the fc layer holds 90 % of the elements: enough CTAs to cover its strided reads
   pack_all_kernel<AT><<<grid, 256, 0, st>>>(params, ws.packtab, (AT*)ws.wf, (AT*)ws.wd, ws.bias, ws.wtc_f, ws.wtc_d, ws.w0img);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -82,6 +82,7 @@ static int pack_all(cb_net* net, Workspace& ws, const float* params, cudaStream_
 
 int pack_weights(cb_net* net, int prec, const float* params, cudaStream_t st) {
   Workspace& ws = net->ws[prec];
+  ws.packed = true;
   return prec == CB_PREC_FP32_REF ? pack_all<float>(net, ws, params, st) : pack_all<bf16>(net, ws, params, st);
 }
 

@@ -79,6 +79,10 @@ def test_policy_forward_config1_shape():
     assert torch.equal(l2, logits) and torch.equal(v2, value) and torch.equal(a2, actions)   # A16
     _, _, a3 = net.policy_forward(dp, dobs, seed=1001, step=1, precision="bf16")
     assert not torch.equal(a3, actions)
+    l4, v4, a4 = net.policy_forward(None, dobs, seed=1001, step=0, precision="bf16")      # params = NULL: reuse the packed weights
+    assert torch.equal(l4, logits) and torch.equal(v4, value) and torch.equal(a4, actions)
+    with pytest.raises(Exception):
+        binding.Net(arch).policy_forward(None, dobs, precision="bf16")                   # nothing packed yet on a fresh net
 
 
 def _run_learner(arch, algo, prec, T, B, seed, blobs=False, warm=False, head_scale=0.1, **kw):
