@@ -74,28 +74,47 @@ def gen_inputs(cfg_index, cfg, n_sets, rank):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms.  The process is started BEFORE the warm-up steps (nvidia-smi
+    needs a few hundred ms to come up, longer than a short timed region); a reader thread stamps every sample with its arrival
+    time and stop() keeps the samples that fall between begin() and end(), i.e. during the timed region."""
     Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
 
     def __init__(self, gpu_index):
-        self.p = None
+        self.p = None; self.lines = []; self.t0 = self.t1 = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"],
-                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True, bufsize=1)
         except OSError:
-            pass
+            return
+        import threading
+
+        def reader():
+            for line in self.p.stdout:
+                self.lines.append((time.perf_counter(), line))
+        self.th = threading.Thread(target=reader, daemon=True); self.th.start()
+
+    def begin(self):
+        self.t0 = time.perf_counter()
+
+    def end(self):
+        self.t1 = time.perf_counter()
 
     def stop(self):
         if self.p is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)      # let the sample in flight arrive
         self.p.terminate()
         try:
-            out, _ = self.p.communicate(timeout=5)
+            self.p.wait(timeout=5)
         except subprocess.TimeoutExpired:
-            self.p.kill(); out, _ = self.p.communicate()
+            self.p.kill()
+        self.th.join(timeout=2)
+        t0 = self.t0 if self.t0 is not None else 0.0; t1 = (self.t1 if self.t1 is not None else time.perf_counter()) + 0.06
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for line in out.strip().splitlines():
+        for ts, line in self.lines:
+            if not (t0 <= ts <= t1):
+                continue
             f = [x.strip() for x in line.split(",")]
             if len(f) < 6:
                 continue
@@ -246,6 +265,7 @@ def main():
         torch.cuda.synchronize()
 
     # ---- warm-up; the first pass profiles every kernel class to find the dominant one ----------------------
+    clocks = ClockSampler(local)      # started here: nvidia-smi takes longer to come up than a short timed region lasts
     step(0, dev_sets); torch.cuda.synchronize()
     binding.profile_begin(-1)
     step(1, dev_sets)
@@ -255,15 +275,16 @@ def main():
         step(i, dev_sets)
     # ---- timed region: K steps, inputs resident in HBM; events on the launching stream ----------------------
     barrier()
-    clocks = ClockSampler(local)
     l0 = binding.launch_count()
     binding.profile_begin(dominant["cls"])        # two events around each launch of the dominant class only
     e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    clocks.begin()
     e0.record(stream)
     for i in range(steps):
         step(i, dev_sets)
     e1.record(stream)
     barrier()
+    clocks.end()
     t_local = e0.elapsed_time(e1) / 1e3
     dom = binding.profile_end()[0]
     launches = binding.launch_count() - l0
