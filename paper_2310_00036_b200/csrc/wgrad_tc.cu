@@ -349,9 +349,10 @@ template <int CIN, int COUT>
 __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwArgs a, const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap ymap) {
   extern __shared__ __align__(128) uint8_t smem_raw[];
   constexpr int UM = CIN == 16 ? 64 : 128;
+  constexpr bool TWO = CIN == 64;      // 3*CIN = 192 rows: one MMA with M = 128 (dj = 0, 1) and one with M = 64 (dj = 2, A two positions further)
   constexpr uint32_t PX = 2u * CIN, PY = 2u * COUT;
   constexpr uint32_t SWX = CIN == 16 ? 6u : (CIN == 32 ? 4u : 2u), SWY = COUT == 16 ? 6u : (COUT == 32 ? 4u : 2u);
-  constexpr uint32_t TCOLS = 3 * COUT <= 128 ? 128u : 256u;
+  constexpr uint32_t NACCC = (TWO ? 6u : 3u) * COUT, TCOLS = NACCC <= 128 ? 128u : (NACCC <= 256 ? 256u : 512u);
   constexpr int YC8 = COUT / 8;
   __shared__ __align__(8) uint64_t bars[3 * SW_MAX_STAGES + 1];      // raw[3], full[3], sempty[3], done
   __shared__ uint32_t tmem_base_smem;
@@ -434,16 +435,21 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
     }
     if (warp < 4) {
       const int lane = tid & 31;
-      const int row = (UM == 128) ? tid : ((lane < 16) ? warp * 16 + lane : 1 << 20);
-      const bool warp_needed = (UM == 128) ? (warp * 32 < 3 * CIN) : (warp * 16 < 3 * CIN);
-      if (warp_needed) {
+      // accumulator rows: M = 128 -> row = TMEM lane; M = 64 -> row r sits in lane 32*(r/16) + r%16
+      const int row128 = tid, row64 = (lane < 16) ? warp * 16 + lane : 1 << 20;
+      for (int part = 0; part < (TWO ? 2 : 1); ++part) {
+        const int um = (TWO && part == 1) ? 64 : UM;
+        const int row = um == 128 ? row128 : row64;
+        const int nrows = TWO ? (part == 0 ? 128 : 64) : 3 * CIN, dj0 = part * 2;
+        const bool warp_needed = um == 128 ? (warp * 32 < nrows) : (warp * 16 < nrows);
+        if (!warp_needed) continue;
         for (int acc = 0; acc < 3; ++acc) {
 #pragma unroll
           for (int c0 = 0; c0 < COUT; c0 += 16) {
             float v[16];
-            tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(acc * COUT + c0), v);
-            if (row >= 3 * CIN) continue;
-            const int tap = (2 - acc) * 3 + row / CIN, r = row % CIN;      // column group e = acc holds the tap row di = 2 - e
+            tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(part * 3 * COUT + acc * COUT + c0), v);
+            if (row >= nrows) continue;
+            const int tap = (2 - acc) * 3 + dj0 + row / CIN, r = row % CIN;      // column group e = acc holds the tap row di = 2 - e
 #pragma unroll
             for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + r) * COUT + c0 + i] = v[i];
           }
@@ -453,6 +459,7 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
   } else if (warp == NLOAD / 32) {
     // ================= MMA issuer =================
     const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)((3 * COUT) >> 3) << 17) | ((uint32_t)(UM >> 4) << 24);
+    const uint32_t idesc64 = (idesc & ~(0x1Fu << 24)) | ((uint32_t)(64 >> 4) << 24);
     const uint32_t a_hi = ((8u * PX) >> 4) | (1u << 14) | (SWX << 29), b_hi = ((8u * PY) >> 4) | (1u << 14) | (SWY << 29);
     // K runs over stored DY rows r: column group e reads row r + e*Wp = DY position r + e*Wp - dy_off, A reads X position
     // r - (dy_off - 2*Wp) + dj; with p = r + e*Wp - dy_off this is X[p + (2-e)*Wp + dj] * DY[p]: tap (2-e, dj)
@@ -468,6 +475,7 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
 #pragma unroll 4
       for (int r = r_begin; r < r_end; r += 16) {
         if (elect_one()) mma_f16(tmem_base, ((uint64_t)a_hi << 32) | xl, ((uint64_t)b_hi << 32) | yl, idesc, accumulate);
+        if (TWO) { if (elect_one()) mma_f16(tmem_base + 3u * COUT, ((uint64_t)a_hi << 32) | (xl + 2u * (PX >> 4)), ((uint64_t)b_hi << 32) | yl, idesc64, accumulate); }
         accumulate = 1;
         xl += PX; yl += PY;      // 16 positions * (pitch / 16)
       }
@@ -589,7 +597,7 @@ static int launch_sw(const tcw::WgradSwArgs& a, const CUtensorMap& xmap, const C
 int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
                     int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
-  if (g.Cin == 16 || g.Cin == 32) {      // swizzled whole-pixel staging
+  if (g.Cin == 16 || g.Cin == 32 || g.Cin == 64) {      // swizzled whole-pixel staging
     const SwPlan q = sw_plan(F, g.H, g.W, g.Cin, g.Cout);
     const int dy_rows = q.nbands > 1 ? q.R : q.R + 2;
     CUtensorMap xmap, ymap; memset(&xmap, 0, sizeof xmap); memset(&ymap, 0, sizeof ymap);
@@ -601,9 +609,12 @@ int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, con
       int rc;
       if (g.Cin == 16 && g.Cout == 16) rc = launch_sw<16, 16>(a, xmap, ymap, q.smem, grid, st);
       else if (g.Cin == 16) rc = launch_sw<16, 32>(a, xmap, ymap, q.smem, grid, st);
-      else if (g.Cout == 16) rc = launch_sw<32, 16>(a, xmap, ymap, q.smem, grid, st);
-      else if (g.Cout == 32) rc = launch_sw<32, 32>(a, xmap, ymap, q.smem, grid, st);
-      else rc = launch_sw<32, 64>(a, xmap, ymap, q.smem, grid, st);
+      else if (g.Cin == 32 && g.Cout == 16) rc = launch_sw<32, 16>(a, xmap, ymap, q.smem, grid, st);
+      else if (g.Cin == 32 && g.Cout == 32) rc = launch_sw<32, 32>(a, xmap, ymap, q.smem, grid, st);
+      else if (g.Cin == 32) rc = launch_sw<32, 64>(a, xmap, ymap, q.smem, grid, st);
+      else if (g.Cout == 16) rc = launch_sw<64, 16>(a, xmap, ymap, q.smem, grid, st);
+      else if (g.Cout == 32) rc = launch_sw<64, 32>(a, xmap, ymap, q.smem, grid, st);
+      else rc = launch_sw<64, 64>(a, xmap, ymap, q.smem, grid, st);
       if (rc) return rc;
       tcw::wgrad_tc_reduce_kernel<<<(tcw::RL * 9 * (g.Cin + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, g.Cin, 0, grad);
       CB_CUDA(cudaGetLastError());
