@@ -50,7 +50,8 @@ __device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr
   for (int i = tid; i < rows * W4; i += nthr, ++j) {
     int lr = i / W4, x0 = (i - lr * W4) * 4, y = yb - 1 + lr;
     uint32_t px[4] = {0, 0, 0, 0};     // per channel: 4 pixels
-    if (j < npre) { px[0] = pre[j][0]; px[1] = pre[j][1]; px[2] = pre[j][2]; px[3] = pre[j][3]; }
+    if (j == 0 && npre > 0) { px[0] = pre[0][0]; px[1] = pre[0][1]; px[2] = pre[0][2]; px[3] = pre[0][3]; }            // static indices: registers
+    else if (j == 1 && npre > 1) { px[0] = pre[1][0]; px[1] = pre[1][1]; px[2] = pre[1][2]; px[3] = pre[1][3]; }
     else if ((unsigned)y < (unsigned)a.H)
       for (int c = 0; c < a.CIN; ++c) px[c] = *reinterpret_cast<const uint32_t*>(a.obs + ((fr * a.CIN + c) * a.H + y) * a.W + x0);
 #pragma unroll
