@@ -30,17 +30,6 @@ struct Args {
   int* error_flag;
 };
 
-// loads the compiler may not sink to their first use: issued where written (ahead of a barrier wait), consumed after it
-__device__ __forceinline__ uint32_t ldg_early_u32(const void* p) {
-  uint32_t v; asm volatile("ld.global.nc.u32 %0, [%1];\n" : "=r"(v) : "l"(p)); return v;
-}
-__device__ __forceinline__ uint2 ldg_early_v2(const void* p) {
-  uint2 v; asm volatile("ld.global.nc.v2.u32 {%0,%1}, [%2];\n" : "=r"(v.x), "=r"(v.y) : "l"(p)); return v;
-}
-__device__ __forceinline__ uint4 ldg_early_v4(const void* p) {
-  uint4 v; asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];\n" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p)); return v;
-}
-
 // stage rows yb-1 .. yb+R of frame `fr` into the plane (all positions rewritten); the first `npre` quads of this thread may have
 // been fetched by the caller (`pre`)
 __device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr, int yb, int tid, int nthr = 128, const uint32_t (*pre)[4] = nullptr, int npre = 0) {
@@ -298,7 +287,7 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
           pf_ok[p] = pool_item(q, p, ttid, YCH, pf_oy[p], pf_ox[p], pf_ch[p]);
           if (pf_ok[p]) {
             const size_t o = (((size_t)f * q.Ho + pf_oy[p]) * q.Wo + pf_ox[p]) * COUT + pf_ch[p] * 8;
-            pf_pk[p] = ldg_early_v2(a.pool_arg + o); pf_dv[p] = ldg_early_v4(a.dpool + o);
+            pf_pk[p] = pool::ldg_early_v2(a.pool_arg + o); pf_dv[p] = pool::ldg_early_v4(a.dpool + o);
           }
         }
       }
@@ -309,7 +298,7 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
         const int i = ttid + j * TN, W4 = a.W / 4, lr = i / W4, x0 = (i - lr * W4) * 4, y = yb - 1 + lr;
         pre[j][0] = pre[j][1] = pre[j][2] = pre[j][3] = 0;
         if (i < (a.R + 2) * W4 && (unsigned)y < (unsigned)a.H)
-          for (int c = 0; c < a.CIN; ++c) pre[j][c] = ldg_early_u32(a.obs + ((fr * a.CIN + c) * a.H + y) * a.W + x0);
+          for (int c = 0; c < a.CIN; ++c) pre[j][c] = pool::ldg_early_u32(a.obs + ((fr * a.CIN + c) * a.H + y) * a.W + x0);
       }
       if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 4; }
       uint8_t* xs = smem + (size_t)s * STAGE + (size_t)a.w_xoff * 16; uint8_t* ys = smem + (size_t)s * STAGE + XB + (size_t)a.w_yoff * PY;

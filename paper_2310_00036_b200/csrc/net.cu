@@ -199,7 +199,7 @@ __global__ void __launch_bounds__(256) pool_bwd_scatter_kernel(const uint8_t* __
       if (ok[p]) {
         pc[p] = tid % C8; const int r = tid / C8; px[p] = pb + 2 * (r % nox); py[p] = first + 2 * (r / nox);
         const size_t o = (((size_t)f * Ho + py[p]) * Wo + px[p]) * C + pc[p] * 8;
-        pk[p] = *reinterpret_cast<const uint2*>(arg + o); dv[p] = *reinterpret_cast<const uint4*>(dy + o);
+        pk[p] = pool::ldg_early_v2(arg + o); dv[p] = pool::ldg_early_v4(dy + o);      // issued here, ahead of the zero fill and the barriers
       }
     }
     for (int i = tid; i < n16; i += 256) reinterpret_cast<uint4*>(tile)[i] = make_uint4(0, 0, 0, 0);

@@ -38,6 +38,17 @@ __device__ __forceinline__ void window_max(const uint4 (&v)[9], uint32_t valid, 
   arg.x = __byte_perm(a[0], a[1], 0x6420); arg.y = __byte_perm(a[2], a[3], 0x6420);
 }
 
+// loads the compiler may not sink to their first use: issued where written (ahead of a barrier wait), consumed after it
+__device__ __forceinline__ uint32_t ldg_early_u32(const void* p) {
+  uint32_t v; asm volatile("ld.global.nc.u32 %0, [%1];\n" : "=r"(v) : "l"(p)); return v;
+}
+__device__ __forceinline__ uint2 ldg_early_v2(const void* p) {
+  uint2 v; asm volatile("ld.global.nc.v2.u32 {%0,%1}, [%2];\n" : "=r"(v.x), "=r"(v.y) : "l"(p)); return v;
+}
+__device__ __forceinline__ uint4 ldg_early_v4(const void* p) {
+  uint4 v; asm volatile("ld.global.nc.v4.u32 {%0,%1,%2,%3}, [%4];\n" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p)); return v;
+}
+
 // dst (one bf16) += g, rounded to bf16; plain read-modify-write (the caller orders conflicting writers)
 __device__ __forceinline__ void add_bf16(uint16_t* dst, uint16_t g) {
   const float o = __uint_as_float((uint32_t)(*dst) << 16), t = __uint_as_float((uint32_t)g << 16);
