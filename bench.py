@@ -340,8 +340,8 @@ def main():
         Bi = 128
         obs_i = [dev_sets[i % len(dev_sets)]["obs"].reshape(-1, arch.in_c, arch.in_h, arch.in_w)[j * Bi:(j + 1) * Bi].contiguous()
                  for i in range(N_ROTATE) for j in range(4)]
-        for i in range(5):
-            net.policy_forward(dp, obs_i[i % len(obs_i)], seed=1, step=i, precision=prec)
+        for i in range(3 * len(obs_i)):      # steady state of a rollout loop: every observation buffer has been seen (third call on: graph replay)
+            net.policy_forward(dp if i == 0 else None, obs_i[i % len(obs_i)], seed=1, step=i, precision=prec)
         torch.cuda.synchronize()
         li = binding.launch_count(); ncall = 100
         e0.record(stream)

@@ -139,11 +139,16 @@ static int build_program(cb_net* net) {
   return CB_OK;
 }
 
+static void drop_fwd_graphs(cb_net* net) {
+  for (auto& fg : net->fwd_graphs) if (fg.exec) cudaGraphExecDestroy(fg.exec);
+  net->fwd_graphs.clear();
+}
 static void free_workspace(Workspace& ws) {
   for (void* p : ws.act) cudaFree(p);
   ws.act.clear();
   for (int i = 0; i < G_COUNT; ++i) { cudaFree(ws.grad[i]); ws.grad[i] = nullptr; }
   cudaFree(ws.partial); ws.partial = nullptr; ws.frames = 0;
+  cudaFree(ws.partial_tc); ws.partial_tc = nullptr; ws.partial_tc_elems = 0;
 }
 static void free_scratch(Workspace& ws) {
   void* ps[] = {ws.logpi, ws.logmu, ws.ent, ws.t0, ws.t1, ws.rho, ws.values, ws.terms, ws.red, ws.advstat, ws.perm, ws.permj, ws.act_m, ws.rew_m, ws.dones_m, ws.logmu_m};
@@ -175,6 +180,7 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
   if (ws.frames >= frames) return CB_OK;
   frames = std::max(frames, net->max_frames);
   CB_CUDA(cudaDeviceSynchronize());
+  drop_fwd_graphs(net);      // they hold the old activation pointers
   free_workspace(ws);
   ws.act.assign(net->tensors.size(), nullptr);
   for (size_t i = 0; i < net->tensors.size(); ++i)
@@ -188,6 +194,11 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
     if (dense_tc_supported(L.g)) pe = std::max(pe, (size_t)8 * std::min(frames, 1024) * L.g.Cout);
   }
   CB_ALLOC(ws.partial, pe * 4); ws.partial_elems = pe;
+  if (prec == CB_PREC_BF16_TC) {
+    size_t pt = 0;
+    for (const Layer& L : net->layers) if (wgrad_tc_supported(L.g)) pt += wgrad_tc_partial_elems(L.g);
+    if (pt) { CB_ALLOC(ws.partial_tc, pt * 4); ws.partial_tc_elems = pt; }
+  }
   ws.frames = frames;
   return CB_OK;
 }
@@ -245,6 +256,9 @@ int cb_net_create(const cb_arch* arch, int max_frames, cb_net** out) {
 
 void cb_net_destroy(cb_net* net) {
   if (!net) return;
+  cudaDeviceSynchronize();
+  drop_fwd_graphs(net);
+  if (net->capture_stream) cudaStreamDestroy(net->capture_stream);
   for (int p = 0; p < 2; ++p) {
     Workspace& ws = net->ws[p];
     if (!ws.wf) continue;
@@ -292,6 +306,44 @@ int cb_net_init(const cb_net* net, uint64_t seed, float* params_host) {
 static int check_prec(int prec) { if (prec != CB_PREC_FP32_REF && prec != CB_PREC_BF16_TC) { set_error("bad precision mode"); return CB_EINVAL; } return CB_OK; }
 static bool misaligned(const void* p, size_t a) { return ((uintptr_t)p & (a - 1)) != 0; }
 
+// The actor calls the trunk thousands of times with the same shapes and a handful of observation buffers, and at B = 128 its
+// ~18 kernels are shorter than their host-side launch cost (tensor-map encoding included).  The first call with a given
+// (precision, B, obs pointer) runs eagerly, the second is captured into a CUDA graph on a private stream, later ones replay it
+// on the caller's stream.  Weights and activations live in library-owned buffers whose addresses only change in
+// ensure_workspace, which drops the graphs.  Event-timed profiling (cb_profile_begin) uses the eager path.
+static int trunk_forward(cb_net* net, int precision, const uint8_t* obs, int B, cudaStream_t st) {
+  if (prof_active()) return forward(net, precision, obs, nullptr, B, st, true);
+  cb_net::FwdGraph* fg = nullptr;
+  for (auto& e : net->fwd_graphs) if (e.prec == precision && e.B == B && e.obs == obs) { fg = &e; break; }
+  if (!fg) {
+    if (net->fwd_graphs.size() >= 64) drop_fwd_graphs(net);
+    net->fwd_graphs.push_back({precision, B, obs, nullptr, 0, false});
+    return forward(net, precision, obs, nullptr, B, st, true);
+  }
+  if (fg->bad) return forward(net, precision, obs, nullptr, B, st, true);
+  if (!fg->exec) {
+    if (!net->capture_stream) CB_CUDA(cudaStreamCreateWithFlags(&net->capture_stream, cudaStreamNonBlocking));
+    const uint64_t l0 = cb_launch_count();
+    cudaGraph_t graph = nullptr;
+    CB_CUDA(cudaStreamBeginCapture(net->capture_stream, cudaStreamCaptureModeRelaxed));
+    const int rc = forward(net, precision, obs, nullptr, B, net->capture_stream, true);
+    const cudaError_t ce = cudaStreamEndCapture(net->capture_stream, &graph);
+    fg->launches = cb_launch_count() - l0;
+    if (rc == CB_OK && ce == cudaSuccess && graph && cudaGraphInstantiate(&fg->exec, graph, 0) == cudaSuccess) {
+      cudaGraphDestroy(graph);
+      CB_CUDA(cudaGraphLaunch(fg->exec, st));
+      return CB_OK;
+    }
+    if (graph) cudaGraphDestroy(graph);
+    (void)cudaGetLastError();
+    fg->exec = nullptr; fg->bad = true;      // not capturable here: stay eager (the counted launches of the failed capture are re-counted below)
+    return forward(net, precision, obs, nullptr, B, st, true);
+  }
+  CB_CUDA(cudaGraphLaunch(fg->exec, st));
+  prof_add_launches(fg->launches);
+  return CB_OK;
+}
+
 int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int B, uint64_t seed, uint64_t step, uint32_t env_offset,
                       int precision, float* logits, float* value, int32_t* actions, void* stream) {
   if (!net || !obs || B < 0) { set_error("null or negative argument"); return CB_EINVAL; }
@@ -302,7 +354,7 @@ int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int 
   if ((rc = ensure_workspace(net, precision, B))) return rc;
   if (params) { if ((rc = pack_weights(net, precision, params, st))) return rc; }
   else if (!net->ws[precision].packed) { set_error("params == NULL but no weights have been packed in this precision mode yet"); return CB_EINVAL; }
-  if ((rc = forward(net, precision, obs, nullptr, B, st, true))) return rc;      // everything up to the hidden layer
+  if ((rc = trunk_forward(net, precision, obs, B, st))) return rc;      // everything up to the hidden layer
   Workspace& ws = net->ws[precision];
   const Layer& HL = net->layers.back();
   const int A = net->arch.n_actions;

@@ -81,6 +81,7 @@ struct Workspace {     // one per precision mode
   PackDesc* packtab = nullptr;                                     // device copy of the layer table for packing
   int* errflag = nullptr;                                          // set by a kernel whose tcgen05 pipeline timed out
   float* partial = nullptr; size_t partial_elems = 0;             // wgrad split-K partials
+  float* partial_tc = nullptr; size_t partial_tc_elems = 0;       // one slot per tensor-core 3x3 layer: their reductions run as ONE launch after the backward pass
   float* gradbuf = nullptr;          // [P]
   // learner scratch (fp32 unless noted)
   float *logpi = nullptr, *logmu = nullptr, *ent = nullptr, *t0 = nullptr, *t1 = nullptr, *rho = nullptr, *values = nullptr;
@@ -111,6 +112,10 @@ struct cb_net {
   std::vector<PT> ptensors;
   cb::Workspace ws[2];
   int last_prec = -1; int last_F = 0, last_N = 0; bool last_ppo = false;
+  // actor side: the trunk of cb_policy_forward replayed as a CUDA graph per (precision, B, obs pointer); see api.cu
+  struct FwdGraph { int prec, B; const uint8_t* obs; cudaGraphExec_t exec; uint64_t launches; bool bad; };
+  std::vector<FwdGraph> fwd_graphs;
+  cudaStream_t capture_stream = nullptr;
 };
 
 namespace cb {
@@ -122,6 +127,8 @@ int cuda_fail(cudaError_t e, const char* what);
 // prof.cu -- launch counter and per-class event timing
 enum KClass { K_PACK = 0, K_CONV_FWD, K_POOL_FWD, K_CONV_DGRAD, K_CONV_WGRAD, K_WGRAD_REDUCE, K_POOL_BWD, K_HEAD_MISC, K_LOGPROB,
               K_SCAN, K_LOSS, K_STATS, K_PERM, K_SQNORM, K_ADAM, K_SAMPLE, K_COUNT };
+bool prof_active();                    // cb_profile_begin .. cb_profile_end
+void prof_add_launches(uint64_t n);    // launches replayed by a CUDA graph
 struct ProfScope {      // counts `n` launches of class `cls`; records an event pair around them when profiling
   ProfScope(int cls, cudaStream_t st, int n = 1, double flops = 0.0, double bytes = 0.0);
   ~ProfScope();
@@ -144,8 +151,15 @@ int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16*
 // wgrad_tc.cu
 bool wgrad_tc_supported(const Geom& g);
 size_t wgrad_tc_partial_elems(const Geom& g);
+// the per-CTA partials of several layers, reduced by one launch (same fixed association per element as a per-layer launch)
+struct WgradReduceJob { const float* partial; int nctas, cin_k, c_off, first_block; Geom g; ParamMap pm; };
+constexpr int WGRAD_MAX_JOBS = 24;
+struct WgradReduceBatch { WgradReduceJob job[WGRAD_MAX_JOBS]; int n = 0, blocks = 0; };
+// `defer` != nullptr: a layer whose kernel wrote `partial` may append its reduction to the batch instead of launching it (the caller
+// then gives every layer its own `partial` and calls launch_wgrad_reduce_batch before the gradient is read)
 int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
-                    int* error_flag, cudaStream_t st);
+                    int* error_flag, cudaStream_t st, WgradReduceBatch* defer = nullptr);
+int launch_wgrad_reduce_batch(const WgradReduceBatch& b, float* grad, cudaStream_t st);
 
 // conv0_tc.cu
 bool conv0_tc_supported(const Geom& g);

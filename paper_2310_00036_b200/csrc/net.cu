@@ -361,6 +361,8 @@ int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx,
 template <typename AT>
 static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, float* grad, cudaStream_t st) {
   const Op* fused_pool = nullptr;      // a max-pool adjoint folded into the next (first-layer) weight gradient
+  WgradReduceBatch batch;               // tensor-core 3x3 layers: per-layer partial slots, ONE reduction launch after the loop
+  size_t tc_off = 0;
   for (size_t oi = 0; oi < net->bwd.size(); ++oi) {
     const Op& op = net->bwd[oi];
     if (op.kind == OP_POOLBWD) {
@@ -388,10 +390,15 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
     const Geom& g = L.g;
     if (op.kind == OP_WGRAD) {
       if (std::is_same<AT, bf16>::value && wgrad_tc_supported(g)) {
-        ProfScope ps(K_CONV_WGRAD, st, 2, 2.0 * 9 * g.Cin * g.Cout * (double)F * g.Ho * g.Wo,
+        const size_t slot = wgrad_tc_partial_elems(g);
+        const bool own_slot = tc_off + slot <= ws.partial_tc_elems && batch.n < WGRAD_MAX_JOBS;
+        const int jobs_before = batch.n;
+        ProfScope ps(K_CONV_WGRAD, st, own_slot ? 1 : 2, 2.0 * 9 * g.Cin * g.Cout * (double)F * g.Ho * g.Wo,
                      2.0 * F * g.H * g.W * (g.Cin + g.Cout) + 4.0 * 9 * (g.Cin + 1) * g.Cout);
-        int rc = launch_wgrad_tc(g, L.pm, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.grad[op.dy], L.relu_in, ws.partial, grad, ws.errflag, st);
+        int rc = launch_wgrad_tc(g, L.pm, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.grad[op.dy], L.relu_in, own_slot ? ws.partial_tc + tc_off : ws.partial, grad,
+                                 ws.errflag, st, own_slot ? &batch : nullptr);
         if (rc) return rc;
+        if (batch.n > jobs_before) tc_off += slot;      // otherwise the call reduced its partials itself
         continue;
       }
       if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
@@ -464,6 +471,13 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
       int rc = launch_gemm(p, 1, st);
       if (rc) return rc;
     }
+  }
+  if (batch.n > 0) {
+    double bytes = 0.0;
+    for (int j = 0; j < batch.n; ++j) bytes += 4.0 * (batch.job[j].nctas + 1) * 9 * (batch.job[j].cin_k + 1) * batch.job[j].g.Cout;
+    ProfScope ps(K_WGRAD_REDUCE, st, 1, 0.0, bytes);
+    int rc = launch_wgrad_reduce_batch(batch, grad, st);
+    if (rc) return rc;
   }
   return CB_OK;
 }

@@ -22,6 +22,9 @@ static cudaEvent_t get_event() {
   cudaEvent_t e; cudaEventCreate(&e); return e;
 }
 
+bool prof_active() { return g_on; }
+void prof_add_launches(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
 ProfScope::ProfScope(int cls, cudaStream_t s, int n, double flops, double bytes) : slot(-1), st(s) {
   g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed);
   if (!g_on || (g_only >= 0 && g_only != cls)) return;

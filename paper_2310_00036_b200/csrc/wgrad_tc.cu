@@ -326,6 +326,36 @@ __global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nc
   grad[pm.w(o, c_off + row, tap / 3, tap % 3, g)] = tot;
 }
 
+// the same reduction for a batch of layers: block b belongs to the job with first_block <= b < next first_block.  A block
+// sums RB consecutive elements: warp `part` adds the partials of CTAs [part*q, (part+1)*q) in order (one 128-byte run per
+// step), then thread (0, e) adds the RL sums in part order -- the association of wgrad_tc_reduce_kernel.
+constexpr int RB = 32;
+__global__ void __launch_bounds__(RL * RB) wgrad_tc_reduce_batch_kernel(const __grid_constant__ WgradReduceBatch b, float* __restrict__ grad) {
+  __shared__ float sums[RL][RB];
+  int j = 0;
+  while (j + 1 < b.n && (int)blockIdx.x >= b.job[j + 1].first_block) ++j;
+  const WgradReduceJob& q = b.job[j];
+  const Geom g = q.g;
+  const int cin_k = q.cin_k, nctas = q.nctas, rows = cin_k + 1, per = 9 * rows * g.Cout;
+  const int part = threadIdx.x / RB, e = threadIdx.x % RB, i = ((int)blockIdx.x - q.first_block) * RB + e;
+  const int qn = (nctas + RL - 1) / RL, z0 = part * qn, z1 = min(nctas, z0 + qn);
+  const float* __restrict__ partial = q.partial;
+  float s = 0.f;
+  if (i < per) {
+#pragma unroll 10
+    for (int z = z0; z < z1; ++z) s += partial[(size_t)z * per + i];
+  }
+  sums[part][e] = s;
+  __syncthreads();
+  if (part != 0 || i >= per) return;
+  float tot = s;
+#pragma unroll
+  for (int k = 1; k < RL; ++k) tot += sums[k][e];
+  int o = i % g.Cout, qq = i / g.Cout, row = qq % rows, tap = qq / rows;
+  if (row == cin_k) { if (tap == 0 && q.c_off == 0) grad[q.pm.b(o)] = tot; return; }
+  grad[q.pm.w(o, q.c_off + row, tap / 3, tap % 3, g)] = tot;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Swizzled variant (TMA, Cin in {16, 32}): whole pixels are landed once, one shared-memory row of 2*CIN (X) or 2*COUT (DY)
 // bytes per position, in the 32B/64B/128B swizzle pattern.  The A descriptor is MN-major with LBO = one row: the M walk
@@ -594,8 +624,15 @@ static int launch_sw(const tcw::WgradSwArgs& a, const CUtensorMap& xmap, const C
   return CB_OK;
 }
 
+int launch_wgrad_reduce_batch(const WgradReduceBatch& b, float* grad, cudaStream_t st) {
+  if (b.n == 0) return CB_OK;
+  tcw::wgrad_tc_reduce_batch_kernel<<<b.blocks, tcw::RL * tcw::RB, 0, st>>>(b, grad);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
 int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, const bf16* dy, bool relu_in, float* partial, float* grad,
-                    int* error_flag, cudaStream_t st) {
+                    int* error_flag, cudaStream_t st, WgradReduceBatch* defer) {
   if (F <= 0) return CB_OK;
   if (g.Cin == 16 || g.Cin == 32 || g.Cin == 64) {      // swizzled whole-pixel staging
     const SwPlan q = sw_plan(F, g.H, g.W, g.Cin, g.Cout);
@@ -616,6 +653,11 @@ int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, con
       else if (g.Cout == 32) rc = launch_sw<64, 32>(a, xmap, ymap, q.smem, grid, st);
       else rc = launch_sw<64, 64>(a, xmap, ymap, q.smem, grid, st);
       if (rc) return rc;
+      if (defer && defer->n < WGRAD_MAX_JOBS) {
+        defer->job[defer->n++] = WgradReduceJob{partial, grid, g.Cin, 0, defer->blocks, g, pm};
+        defer->blocks += (9 * (g.Cin + 1) * g.Cout + tcw::RB - 1) / tcw::RB;
+        return CB_OK;
+      }
       tcw::wgrad_tc_reduce_kernel<<<(tcw::RL * 9 * (g.Cin + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, g.Cin, 0, grad);
       CB_CUDA(cudaGetLastError());
       return CB_OK;

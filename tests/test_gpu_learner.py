@@ -85,6 +85,40 @@ def test_policy_forward_config1_shape():
         binding.Net(arch).policy_forward(None, dobs, precision="bf16")                   # nothing packed yet on a fresh net
 
 
+@pytest.mark.parametrize("prec", ["fp32", "bf16"])
+def test_policy_forward_graph_replay(prec):
+    """The actor trunk is replayed as a CUDA graph from the third call with the same (B, obs buffer) on: replays must follow new
+    observation CONTENTS and new parameters, match a fresh net's eager call bitwise, count the same launches, and survive a
+    workspace reallocation (a larger batch in between)."""
+    arch = SMALL_IMPALA; B = 6
+    p1, p2 = synth.gen_params(arch, 31, bias_scale=0.05), synth.gen_params(arch, 32, bias_scale=0.05)
+    o1, o2 = synth.gen_obs_uniform(B, 33, arch), synth.gen_obs_uniform(B, 34, arch)
+    big = dev(synth.gen_obs_uniform(4 * B, 35, arch))
+
+    def eager(params, obs, step):
+        return binding.Net(arch, max_frames=B).policy_forward(dev(params), dev(obs), seed=7, step=step, precision=prec)
+
+    net = binding.Net(arch, max_frames=B)
+    buf = dev(o1)
+    counts = []
+    for i in range(4):                                   # eager, capture, replay, replay
+        c0 = binding.launch_count()
+        got = net.policy_forward(dev(p1) if i == 0 else None, buf, seed=7, step=i, precision=prec)
+        counts.append(binding.launch_count() - c0)
+        ref = eager(p1, o1, i)
+        assert all(torch.equal(a, b) for a, b in zip(got, ref)), i
+    assert counts[1] == counts[2] == counts[3] == counts[0] - 1      # call 0 also packed the weights
+    buf.copy_(dev(o2))                                   # same buffer, new frames
+    got = net.policy_forward(None, buf, seed=7, step=9, precision=prec)
+    assert all(torch.equal(a, b) for a, b in zip(got, eager(p1, o2, 9)))
+    got = net.policy_forward(dev(p2), buf, seed=7, step=10, precision=prec)      # new parameters: packed, then the replay reads them
+    assert all(torch.equal(a, b) for a, b in zip(got, eager(p2, o2, 10)))
+    net.policy_forward(None, big, seed=7, step=11, precision=prec)               # grows the workspace: graphs dropped
+    for i in range(3):
+        got = net.policy_forward(None, buf, seed=7, step=12 + i, precision=prec)
+        assert all(torch.equal(a, b) for a, b in zip(got, eager(p2, o2, 12 + i))), i
+
+
 def _run_learner(arch, algo, prec, T, B, seed, blobs=False, warm=False, head_scale=0.1, **kw):
     hp, ho = _hp_pair(algo, prec, T, B, **kw)
     bt = _batch(arch, T, B, seed, blobs)
