@@ -96,7 +96,11 @@ int cb_net_init(const cb_net* net, uint64_t seed, float* params_host);
  * call on this net in the same precision mode (an actor takes new parameters from its queue once
  * per rollout, not per step: Figure 1 / PAPER.md:148-150; CB_EINVAL if there was no such call).  obs: dev uint8
  * [B,in_c,in_h,in_w].  precision: CB_PREC_*.
- * Outputs (dev): logits fp32 [B,A], value fp32 [B], actions int32 [B]; any may be NULL. */
+ * Outputs (dev): logits fp32 [B,A], value fp32 [B], actions int32 [B]; any may be NULL.
+ * Launch behaviour: from the third call with the same (precision, B, obs pointer) on, the network
+ * trunk is replayed as a CUDA graph on `stream` (captured on a library-owned stream during the
+ * second call); the frames are read from `obs` at replay time, so a rollout loop should reuse its
+ * observation buffers.  Results are bitwise those of the direct launches. */
 int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int B, uint64_t seed,
                       uint64_t step, uint32_t env_offset, int precision, float* logits, float* value,
                       int32_t* actions, void* stream);

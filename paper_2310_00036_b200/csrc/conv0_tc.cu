@@ -389,7 +389,15 @@ __global__ void conv0_wgrad_reduce_kernel(const float* __restrict__ partial, int
   const int per = 3 * 24 * g.Cout;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < per; i += gridDim.x * blockDim.x) {
     float s = 0.f;
-    for (int z = 0; z < nctas; ++z) s += partial[(size_t)z * per + i];
+    int z = 0;
+    for (; z + 16 <= nctas; z += 16) {      // 16 loads in flight, then the additions in CTA order
+      float v[16];
+#pragma unroll
+      for (int k = 0; k < 16; ++k) v[k] = __ldg(partial + (size_t)(z + k) * per + i);
+#pragma unroll
+      for (int k = 0; k < 16; ++k) s += v[k];
+    }
+    for (; z < nctas; ++z) s += partial[(size_t)z * per + i];
     int o = i % g.Cout, row = (i / g.Cout) % 24, di = i / g.Cout / 24, dj = row >> 3, c = row & 7;
     if (c < g.Cin) grad[pm.w(o, c, di, dj, g)] = s * (1.0f / 255.0f);
     else if (c == 4 && dj == 0 && di == 0) grad[pm.b(o)] = s;

@@ -240,7 +240,15 @@ __global__ void wgrad_reduce_kernel(const float* __restrict__ partial, int split
   size_t total = (size_t)M * N;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
     float s = 0.f;
-    for (int z = 0; z < splits; ++z) s += partial[(size_t)z * total + i];
+    int z = 0;
+    for (; z + 16 <= splits; z += 16) {      // 16 loads in flight, then the additions in z order
+      float v[16];
+#pragma unroll
+      for (int k = 0; k < 16; ++k) v[k] = __ldg(partial + (size_t)(z + k) * total + i);
+#pragma unroll
+      for (int k = 0; k < 16; ++k) s += v[k];
+    }
+    for (; z < splits; ++z) s += partial[(size_t)z * total + i];
     int n = (int)(i % N), m = (int)(i / N);
     if (m == Kw) { grad[pm.b(n)] = s; continue; }
     int c = m % g.Cin; int q = m / g.Cin; int dj = q % g.kw, di = q / g.kw;

@@ -214,7 +214,8 @@ __global__ void vtrace_kernel(int T, int B, const float* __restrict__ V, int ldV
   if (b >= B) return;
   float Vn = V[((size_t)T * B + b) * ldV];
   float acc = 0.f, vs_next = Vn;
-  for (int t = T - 1; t >= 0; --t) {
+#pragma unroll 4
+  for (int t = T - 1; t >= 0; --t) {      // loads of four steps in flight; the recurrence runs in the definition's order
     size_t i = (size_t)t * B + b;
     float Vt = V[i * ldV];
     float disc = gamma * (1.0f - (float)d[i]);
@@ -243,7 +244,8 @@ __global__ void gae_kernel(int T, int B, const float* __restrict__ V, int ldV, c
   int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= B) return;
   float Vn = V[((size_t)T * B + b) * ldV], a = 0.f;
-  for (int t = T - 1; t >= 0; --t) {
+#pragma unroll 4
+  for (int t = T - 1; t >= 0; --t) {      // loads of four steps in flight; the recurrence runs in the definition's order
     size_t i = (size_t)t * B + b;
     float Vt = V[i * ldV];
     float disc = gamma * (1.0f - (float)d[i]);

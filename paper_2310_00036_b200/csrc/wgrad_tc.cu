@@ -314,8 +314,15 @@ __global__ void wgrad_tc_reduce_kernel(const float* __restrict__ partial, int nc
   const int q = (nctas + RL - 1) / RL, z0 = part * q, z1 = min(nctas, z0 + q);
   float s = 0.f;
   if (i < per) {
-#pragma unroll 10
-    for (int z = z0; z < z1; ++z) s += partial[(size_t)z * per + i];
+    int z = z0;
+    for (; z + 10 <= z1; z += 10) {      // 10 loads in flight (148 CTAs / 16 lanes), then the additions in CTA order
+      float v[10];
+#pragma unroll
+      for (int k = 0; k < 10; ++k) v[k] = __ldg(partial + (size_t)(z + k) * per + i);
+#pragma unroll
+      for (int k = 0; k < 10; ++k) s += v[k];
+    }
+    for (; z < z1; ++z) s += partial[(size_t)z * per + i];
   }
   float tot = s;
 #pragma unroll
@@ -342,8 +349,15 @@ __global__ void __launch_bounds__(RL * RB) wgrad_tc_reduce_batch_kernel(const __
   const float* __restrict__ partial = q.partial;
   float s = 0.f;
   if (i < per) {
-#pragma unroll 10
-    for (int z = z0; z < z1; ++z) s += partial[(size_t)z * per + i];
+    int z = z0;
+    for (; z + 10 <= z1; z += 10) {      // 10 loads in flight (148 CTAs / 16 lanes), then the additions in CTA order
+      float v[10];
+#pragma unroll
+      for (int k = 0; k < 10; ++k) v[k] = __ldg(partial + (size_t)(z + k) * per + i);
+#pragma unroll
+      for (int k = 0; k < 10; ++k) s += v[k];
+    }
+    for (; z < z1; ++z) s += partial[(size_t)z * per + i];
   }
   sums[part][e] = s;
   __syncthreads();
