@@ -41,6 +41,7 @@ __device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr
     uint32_t px[4] = {0, 0, 0, 0};     // per channel: 4 pixels
     if (j == 0 && npre > 0) { px[0] = pre[0][0]; px[1] = pre[0][1]; px[2] = pre[0][2]; px[3] = pre[0][3]; }            // static indices: registers
     else if (j == 1 && npre > 1) { px[0] = pre[1][0]; px[1] = pre[1][1]; px[2] = pre[1][2]; px[3] = pre[1][3]; }
+    else if (j == 2 && npre > 2) { px[0] = pre[2][0]; px[1] = pre[2][1]; px[2] = pre[2][2]; px[3] = pre[2][3]; }
     else if ((unsigned)y < (unsigned)a.H)
       for (int c = 0; c < a.CIN; ++c) px[c] = *reinterpret_cast<const uint32_t*>(a.obs + ((fr * a.CIN + c) * a.H + y) * a.W + x0);
 #pragma unroll
@@ -136,16 +137,17 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
   const uint32_t a_base = smem_u32(xs), b_base = smem_u32(w_smem);
   uint32_t parity = 0;
   const int nitems = a.F * a.nbands;
+  const bool fused = a.pool_out != nullptr;
+  const int Ho = (a.H + 1) / 2, Wo = (a.W + 1) / 2;
+  int th_ = (Ho - 1) * 2 + 3 - a.H; if (th_ < 0) th_ = 0; const int ph = th_ / 2;
+  int tw_ = (Wo - 1) * 2 + 3 - a.W; if (tw_ < 0) tw_ = 0; const int pw = tw_ / 2;
+  uint32_t pre[3][4]; int npre = 0;      // this thread's first three observation quads of the NEXT item, fetched while the current one is pooled
   for (int item = blockIdx.x; item < nitems; item += gridDim.x) {
     const int f = item / a.nbands, band = item - f * a.nbands;
-    const bool fused = a.pool_out != nullptr;
-    const int Ho = (a.H + 1) / 2, Wo = (a.W + 1) / 2;
-    int th_ = (Ho - 1) * 2 + 3 - a.H; if (th_ < 0) th_ = 0; const int ph = th_ / 2;
-    int tw_ = (Wo - 1) * 2 + 3 - a.W; if (tw_ < 0) tw_ = 0; const int pw = tw_ / 2;
     const int py0 = band * a.Rp;                                   // fused: first pooled row of the band
     const int yb = fused ? max(0, 2 * py0 - ph) : band * a.R;      // first conv row computed by this item
     const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
-    stage_band(a, xs, fr, yb, tid, 256);
+    stage_band(a, xs, fr, yb, tid, 256, pre, npre);
     fence_async_smem();
     __syncthreads();
     const int ntiles = (a.R * Wp + 127) / 128;
@@ -201,6 +203,22 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
       }
       tc_fence_before();
       __syncthreads();
+    }
+    if (item + (int)gridDim.x < nitems) {      // loads of the next item's plane, consumed by its stage_band
+      const int nitem = item + (int)gridDim.x, nf = nitem / a.nbands, nband = nitem - nf * a.nbands;
+      const int nyb = fused ? max(0, 2 * nband * a.Rp - ph) : nband * a.R;
+      const size_t nfr = a.frame_idx ? (size_t)a.frame_idx[nf] : (size_t)nf;
+#pragma unroll
+      for (int j = 0; j < 3; ++j) {
+        const int i = tid + j * 256, W4 = a.W / 4, lr = i / W4, x0 = (i - lr * W4) * 4, y = nyb - 1 + lr;
+        pre[j][0] = pre[j][1] = pre[j][2] = pre[j][3] = 0;
+        if (i < (a.R + 2) * W4 && (unsigned)y < (unsigned)a.H)
+        {
+#pragma unroll
+          for (int c = 0; c < 4; ++c) if (c < a.CIN) pre[j][c] = pool::ldg_early_u32(a.obs + ((nfr * a.CIN + c) * a.H + y) * a.W + x0);      // static indices: registers
+        }
+      }
+      npre = 3;
     }
     if (fused) {
       // ---- max-pool 3x3 stride 2 SAME (A10) over the band; first maximum in row-major window order (A11) ----

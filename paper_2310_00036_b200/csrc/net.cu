@@ -46,18 +46,36 @@ __global__ void pack_all_kernel(const float* __restrict__ params, const PackDesc
   const int K = g.kh * g.kw * g.Cin;
   const size_t total = (size_t)K * g.Cout;
   AT* wf = wf_all + d.wf_off; AT* wd = wd_all + d.wf_off; float* bias = bias_all + d.bias_off;
-  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-    int n = (int)(i % g.Cout); int k = (int)(i / g.Cout);
-    int c = k % g.Cin; int q = k / g.Cin; int dj = q % g.kw, di = q / g.kw;
-    float v = params[d.pm.w(n, c, di, dj, g)];
-    stv(wf, i, v);
-    stv(wd, ((size_t)(di * g.kw + dj) * g.Cout + n) * g.Cin + c, v);
-    if (k == 0) bias[n] = params[d.pm.b(n)];
-    if (d.tc) {
-      const int tap = di * 3 + dj, tapd = (2 - di) * 3 + (2 - dj);
-      const bf16 h = __float2bfloat16_rn(v);
-      (wtf_all + d.wf_off)[(((size_t)tap * (g.Cin / 8) + c / 8) * g.Cout + n) * 8 + c % 8] = h;
-      (wtd_all + d.wf_off)[(((size_t)tapd * (g.Cout / 8) + n / 8) * g.Cin + c) * 8 + n % 8] = h;
+  // four elements per pass: their (strided) fp32 reads are issued together, then the stores follow
+  const uint32_t stride = gridDim.x * blockDim.x, tot = (uint32_t)total;
+  for (uint32_t i0 = blockIdx.x * blockDim.x + threadIdx.x; i0 < tot; i0 += 4 * stride) {
+    float v4[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t i = i0 + u * stride;
+      v4[u] = 0.f;
+      if (i < tot) {
+        int n = (int)(i % (uint32_t)g.Cout); int k = (int)(i / (uint32_t)g.Cout);
+        int c = k % g.Cin; int q = k / g.Cin; int dj = q % g.kw, di = q / g.kw;
+        v4[u] = __ldg(params + d.pm.w(n, c, di, dj, g));
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t i = i0 + u * stride;
+      if (i >= tot) break;
+      const float v = v4[u];
+      int n = (int)(i % (uint32_t)g.Cout); int k = (int)(i / (uint32_t)g.Cout);
+      int c = k % g.Cin; int q = k / g.Cin; int dj = q % g.kw, di = q / g.kw;
+      stv(wf, i, v);
+      stv(wd, ((size_t)(di * g.kw + dj) * g.Cout + n) * g.Cin + c, v);
+      if (k == 0) bias[n] = params[d.pm.b(n)];
+      if (d.tc) {
+        const int tap = di * 3 + dj, tapd = (2 - di) * 3 + (2 - dj);
+        const bf16 h = __float2bfloat16_rn(v);
+        (wtf_all + d.wf_off)[(((size_t)tap * (g.Cin / 8) + c / 8) * g.Cout + n) * 8 + c % 8] = h;
+        (wtd_all + d.wf_off)[(((size_t)tapd * (g.Cout / 8) + n / 8) * g.Cin + c) * 8 + n % 8] = h;
+      }
     }
   }
   if (d.conv0) {      // forward B image [slot = 2*di + h][chunk][o][8]: chunks (di, 2h), (di, 2h+1); channels >= Cin and dj = 3 are zero
