@@ -13,6 +13,31 @@ namespace pool {
 __device__ __forceinline__ void window_max(const uint4 (&v)[9], uint32_t valid, uint4& best, uint2& arg) {
   __nv_bfloat162 m[4];
   const uint32_t NEG_INF2 = 0xFF80FF80u;
+  if (valid == 0x1FFu) {      // interior window (all but the border ones): no per-tap predicates
+    const __nv_bfloat162* h0 = reinterpret_cast<const __nv_bfloat162*>(&v[0]);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) m[k] = h0[k];
+#pragma unroll
+    for (int t = 1; t < 9; ++t) {
+      const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v[t]);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) m[k] = __hmax2(m[k], h[k]);
+    }
+    uint32_t a[4] = {0x00080008u, 0x00080008u, 0x00080008u, 0x00080008u};      // tap 8 equals the maximum unless an earlier one does
+#pragma unroll
+    for (int t = 7; t >= 0; --t) {
+      const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v[t]);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint32_t mask = __heq2_mask(h[k], m[k]);
+        a[k] = (a[k] & ~mask) | (((uint32_t)t * 0x00010001u) & mask);
+      }
+    }
+    best.x = *reinterpret_cast<const uint32_t*>(&m[0]); best.y = *reinterpret_cast<const uint32_t*>(&m[1]);
+    best.z = *reinterpret_cast<const uint32_t*>(&m[2]); best.w = *reinterpret_cast<const uint32_t*>(&m[3]);
+    arg.x = __byte_perm(a[0], a[1], 0x6420); arg.y = __byte_perm(a[2], a[3], 0x6420);
+    return;
+  }
 #pragma unroll
   for (int k = 0; k < 4; ++k) m[k] = *reinterpret_cast<const __nv_bfloat162*>(&NEG_INF2);
 #pragma unroll
