@@ -36,8 +36,9 @@ __device__ __forceinline__ void stage_band(const Args& a, uint8_t* xs, size_t fr
   const int Wp = a.W + 2, W4 = a.W / 4, rows = a.R + 2;
   const uint32_t ONE = 0x3F80u;
   int j = 0;
+  const uint32_t magic_W4 = (uint32_t)((0x100000000ull + (uint64_t)W4 - 1) / (uint64_t)W4);      // i / W4 = umulhi(i, magic) for i * W4 < 2^32
   for (int i = tid; i < rows * W4; i += nthr, ++j) {
-    int lr = i / W4, x0 = (i - lr * W4) * 4, y = yb - 1 + lr;
+    int lr = (int)__umulhi((uint32_t)i, magic_W4), x0 = (i - lr * W4) * 4, y = yb - 1 + lr;
     uint32_t px[4] = {0, 0, 0, 0};     // per channel: 4 pixels
     if (j == 0 && npre > 0) { px[0] = pre[0][0]; px[1] = pre[0][1]; px[2] = pre[0][2]; px[3] = pre[0][3]; }            // static indices: registers
     else if (j == 1 && npre > 1) { px[0] = pre[1][0]; px[1] = pre[1][1]; px[2] = pre[1][2]; px[3] = pre[1][3]; }
@@ -225,8 +226,9 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
       const bf16* ct = reinterpret_cast<const bf16*>(xs + (size_t)a.npix_alloc * 16);
       constexpr int C8 = COUT / 8;
       const int pr = min(a.Rp, Ho - py0);
+      const uint32_t magic_Wo = (uint32_t)((0x100000000ull + (uint64_t)Wo - 1) / (uint64_t)Wo);
       for (int i = tid; i < pr * Wo * C8; i += 256) {
-        const int c8 = i % C8, q = i / C8, ox = q % Wo, oy = py0 + q / Wo;
+        const int c8 = i % C8, q = i / C8, qy = (int)__umulhi((uint32_t)q, magic_Wo), ox = q - qy * Wo, oy = py0 + qy;
         uint4 v[9]; uint32_t valid = 0;
 #pragma unroll
         for (int di = 0; di < 3; ++di) {
