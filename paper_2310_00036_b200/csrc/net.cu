@@ -169,11 +169,13 @@ __device__ __forceinline__ uint4 f_to_bf8(const float* f) {
   for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(f[2 * i], f[2 * i + 1]);
   return u;
 }
+// IT = index type of the element counter: uint32_t whenever F*Ho*Wo*C/8 < 2^32 (64-bit divisions cost more than the window maximum)
+template <typename IT>
 __global__ void pool_fwd_v8_kernel(const bf16* __restrict__ x, bf16* __restrict__ y, uint8_t* __restrict__ arg, int F, int C, int H, int W) {
   int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W), C8 = C / 8;
-  size_t total = (size_t)F * Ho * Wo * C8;
-  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-    int c8 = (int)(i % C8); size_t q = i / C8; int ox = (int)(q % Wo); q /= Wo; int oy = (int)(q % Ho); size_t f = q / Ho;
+  const IT total = (IT)F * (IT)Ho * (IT)Wo * (IT)C8;
+  for (IT i = blockIdx.x * (IT)blockDim.x + threadIdx.x; i < total; i += (IT)gridDim.x * blockDim.x) {
+    int c8 = (int)(i % (IT)C8); IT q = i / (IT)C8; int ox = (int)(q % (IT)Wo); q /= (IT)Wo; int oy = (int)(q % (IT)Ho); size_t f = (size_t)(q / (IT)Ho);
     uint4 v[9]; uint32_t valid = 0;
 #pragma unroll
     for (int di = 0; di < 3; ++di) {
@@ -189,8 +191,8 @@ __global__ void pool_fwd_v8_kernel(const bf16* __restrict__ x, bf16* __restrict_
     }
     uint4 best; uint2 pk;
     pool::window_max(v, valid, best, pk);      // packed bf16 max; first maximum in window order (A11)
-    *reinterpret_cast<uint4*>(y + i * 8) = best;
-    *reinterpret_cast<uint2*>(arg + i * 8) = pk;
+    *reinterpret_cast<uint4*>(y + (size_t)i * 8) = best;
+    *reinterpret_cast<uint2*>(arg + (size_t)i * 8) = pk;
   }
 }
 // Max-pool adjoint, scatter form: one CTA builds a band of `RB` input rows of one frame in shared memory.  Every
@@ -334,7 +336,13 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
       size_t total = (size_t)F * pool_out(op.H) * pool_out(op.W) * op.C;
       ProfScope ps(K_POOL_FWD, st, 1, 0.0, (double)sizeof(AT) * (total + (double)F * op.H * op.W * op.C));
       if (std::is_same<AT, bf16>::value && op.C % 8 == 0)
-        pool_fwd_v8_kernel<<<grid_for(total / 8), 256, 0, st>>>((const bf16*)ws.act[op.in_t], (bf16*)ws.act[op.out_t], (uint8_t*)ws.act[op.mask_t], F, op.C, op.H, op.W);
+      {
+        // grid-stride counter + one stride must stay below 2^32 for the 32-bit form
+        if (total / 8 + (size_t)grid_for(total / 8) * 256 < 0xFFFFFFFFull)
+          pool_fwd_v8_kernel<uint32_t><<<grid_for(total / 8), 256, 0, st>>>((const bf16*)ws.act[op.in_t], (bf16*)ws.act[op.out_t], (uint8_t*)ws.act[op.mask_t], F, op.C, op.H, op.W);
+        else
+          pool_fwd_v8_kernel<size_t><<<grid_for(total / 8), 256, 0, st>>>((const bf16*)ws.act[op.in_t], (bf16*)ws.act[op.out_t], (uint8_t*)ws.act[op.mask_t], F, op.C, op.H, op.W);
+      }
       else
         pool_fwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (AT*)ws.act[op.out_t], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());
