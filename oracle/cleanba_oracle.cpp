@@ -18,13 +18,18 @@
 //   softmax / entropy ........... pinned: identities (sum p = 1, H(uniform)=log A, shift invariance)
 //   Philox4x32-10 ............... pinned: cuRAND host generator (library) on 1e6 counters
 //   fixed-op log / Gumbel ....... pinned: libm log over all 2^24 uniforms, chi^2 vs softmax
-//   V-trace ..................... pinned: n-step-return closed form, c_bar=0, GAE cross-pin, T=1
+//   V-trace ..................... pinned: n-step-return closed form, c_bar=0, GAE cross-pin, T=1, the lambda mix of q_t
+//                                 (on-policy pgadv = GAE(lambda) by double sum), the off-policy definition as an
+//                                 explicit double sum with three different thresholds (rho_bar, c_bar, rho_pg_bar)
 //   GAE ......................... pinned: lambda=1 brute-force discounted return, lambda=0
 //   IMPALA / PPO losses ......... pinned: finite differences, ratio-1 invariants, sign tests
 //   clip + Adam ................. pinned: first-step closed form, constant-gradient closed form
 //   clip + RMSprop (A22) ........ pinned: first-step and constant-gradient closed forms, lr = 0
 //   env-split minibatches (A21) . pinned: mb = 1 identity, equality with per-group single steps run by hand
 //   permutation ................. pinned: bijection + brute-force reference of the index rule
+//   behaviour values (A3b) ...... pinned: step with the oracle's own recomputed (fp32-rounded) values == hand-composed
+//                                 GAE + minibatch updates; values of a different policy change the targets only
+//   PPO epoch counter (A23) ..... pinned: a second call continues the permutation epochs where the first stopped
 // =============================================================================================
 #include <cmath>
 #include <cstdint>
@@ -696,12 +701,18 @@ double orc_ppo_objective_f64(const orc_arch* a, const orc_hparams* hp, const dou
 // ---------------------------------------------------------------------------------------------
 int orc_learner_step(const orc_arch* a, const orc_hparams* hp, float* params, float* adam_m, float* adam_v, uint64_t* opt_step,
                      const uint8_t* obs, const int32_t* actions, const float* rewards, const uint8_t* dones,
-                     const float* behaviour_logits, float* stats,
+                     const float* behaviour_logits, const float* behaviour_values /*nullable, [T+1,B]*/, float* stats,
                      double* out_logits, double* out_values, double* out_t0, double* out_t1, double* out_grad) {
   Layout L = make_layout(*a); int T = hp->T, B = hp->B, N = T * B, A = a->n_actions, F = (T + 1) * B;
   size_t P = L.total; vec Pd(params, params + P);
   vec lg((size_t)F * A), V(F);
-  forward_many(*a, L, Pd.data(), obs, F, lg.data(), V.data());
+  // Reading A3b (Alg. 1 l.8-12): PPO may be handed the values the ACTOR computed at rollout time
+  // (v_t stored with the transition, v_next for the bootstrap observation); GAE then uses them and the learner's
+  // iteration-start forward is not needed.  NULL = recompute them here with the iteration-start parameters (A3).
+  // IMPALA ignores them: V-trace is defined on the current learner parameters' values (O4).
+  const bool given_values = behaviour_values && hp->algo == 1;
+  if (given_values) { for (int f = 0; f < F; ++f) V[f] = (double)behaviour_values[f]; std::fill(lg.begin(), lg.end(), 0.0); }
+  else forward_many(*a, L, Pd.data(), obs, F, lg.data(), V.data());
   if (out_logits) std::copy(lg.begin(), lg.end(), out_logits);
   if (out_values) std::copy(V.begin(), V.end(), out_values);
   vec logmu(N), r(N), lp(A), bl(A);
@@ -751,8 +762,11 @@ int orc_learner_step(const orc_arch* a, const orc_hparams* hp, float* params, fl
   int nmb = hp->minibatches, m = N / nmb, upd = 0;
   std::vector<int32_t> perm(N), act_m(m); vec adv_m(m), ret_m(m), lpo_m(m), lgm((size_t)m * A), Vm(m), dl((size_t)m * A), dV(m);
   size_t fs = (size_t)a->in_c * a->in_h * a->in_w;
+  // Reading A23: the permutation of epoch e of this call is keyed by the epoch counter (opt_step at entry / minibatches) + e,
+  // so successive calls of a training run (opt_step advances by epochs * minibatches per call) never reuse a partition.
+  const uint32_t epoch0 = (uint32_t)(*opt_step / (uint64_t)nmb);
   for (int e = 0; e < hp->epochs; ++e) {
-    permutation(hp->perm_seed, (uint32_t)e, N, perm.data());
+    permutation(hp->perm_seed, epoch0 + (uint32_t)e, N, perm.data());
     for (int k = 0; k < nmb; ++k, ++upd) {
       const int32_t* idx = &perm[(size_t)k * m];
       for (int j = 0; j < m; ++j) { act_m[j] = actions[idx[j]]; adv_m[j] = adv[idx[j]]; ret_m[j] = ret[idx[j]]; lpo_m[j] = logmu[idx[j]]; }
@@ -764,7 +778,8 @@ int orc_learner_step(const orc_arch* a, const orc_hparams* hp, float* params, fl
       backward_many(*a, L, Pd.data(), obs, idx, m, dl.data(), dV.data(), G.data());
       if (out_grad) std::copy(G.begin(), G.end(), out_grad);
       *opt_step += 1;
-      st[4] = clip_adam(P, params, adam_m, adam_v, G.data(), *opt_step, hp->lr, hp->beta1, hp->beta2, hp->adam_eps, hp->max_grad_norm);
+      if (hp->optimizer == 1) st[4] = clip_rmsprop(P, params, adam_v, G.data(), hp->lr, hp->rms_decay, hp->rms_eps, hp->max_grad_norm);
+      else st[4] = clip_adam(P, params, adam_m, adam_v, G.data(), *opt_step, hp->lr, hp->beta1, hp->beta2, hp->adam_eps, hp->max_grad_norm);
       for (int i = 0; i < ORC_N_STATS; ++i) stats[(size_t)upd * ORC_N_STATS + i] = (float)st[i];
     }
   }

@@ -269,7 +269,8 @@ def ppo_objective_f64(arch, hp, params64, obs, actions, adv, ret, logp_old, want
     return (float(L), g) if want_grad else float(L)
 
 
-def learner_step(arch, hp, params, adam_m, adam_v, opt_step, obs, actions, rewards, dones, behaviour_logits, debug=False):
+def learner_step(arch, hp, params, adam_m, adam_v, opt_step, obs, actions, rewards, dones, behaviour_logits, debug=False,
+                 behaviour_values=None):
     """One cb_learner_step on the host.  Returns dict(params, m, v, opt_step, stats[, logits, values, t0, t1, grad])."""
     T, B, A = hp.T, hp.B, arch.n_actions
     params = _c(params, np.float32).copy(); m = _c(adam_m, np.float32).copy(); v = _c(adam_v, np.float32).copy()
@@ -280,8 +281,10 @@ def learner_step(arch, hp, params, adam_m, adam_v, opt_step, obs, actions, rewar
     stats = np.zeros((n_upd, N_STATS), np.float32); step = C.c_uint64(opt_step)
     F, N = (T + 1) * B, T * B
     dbg = dict(logits=np.empty((F, A)), values=np.empty(F), t0=np.empty(N), t1=np.empty(N), grad=np.empty(params.size)) if debug else {}
+    bv = None if behaviour_values is None else _c(behaviour_values, np.float32)
+    assert bv is None or bv.size == F
     n = lib().orc_learner_step(C.byref(arch), C.byref(hp), _p(params), _p(m), _p(v), C.byref(step), _p(obs), _p(actions),
-                               _p(rewards), _p(dones), _p(bl), _p(stats), _p(dbg.get("logits")), _p(dbg.get("values")),
+                               _p(rewards), _p(dones), _p(bl), _p(bv), _p(stats), _p(dbg.get("logits")), _p(dbg.get("values")),
                                _p(dbg.get("t0")), _p(dbg.get("t1")), _p(dbg.get("grad")))
     assert n == n_upd
     out = dict(params=params, m=m, v=v, opt_step=step.value, stats=stats)

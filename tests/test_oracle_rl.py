@@ -89,6 +89,61 @@ def test_vtrace_clipping_thresholds():
     np.testing.assert_allclose(rho, np.minimum(0.8, w), rtol=1e-14)
 
 
+def brute_vtrace_definition(V, r, d, w, gamma, lam, rho_bar, c_bar):
+    """Espeholt et al. 2018, Eq. 1, written out as the explicit double sum (no recursion):
+    vs_t = V_t + sum_{k>=t} (prod_{j=t}^{k-1} disc_j c_j) rho_k (r_k + disc_k V_{k+1} - V_k), c_j = lam min(c_bar, w_j)."""
+    T, B = r.shape; vs = np.zeros((T, B))
+    for b in range(B):
+        for t in range(T):
+            acc, prod = 0.0, 1.0
+            for k in range(t, T):
+                disc = gamma * (1.0 - d[k, b])
+                acc += prod * min(rho_bar, w[k, b]) * (r[k, b] + disc * V[k + 1, b] - V[k, b])
+                prod *= disc * lam * min(c_bar, w[k, b])
+            vs[t, b] = V[t, b] + acc
+    return vs
+
+
+@pytest.mark.parametrize("lam", [0.3, 0.95])
+def test_vtrace_pgadv_lambda_mix_on_policy(lam):
+    """The lambda mix inside q_t (A2): on-policy, q_t - V_t = delta_t + disc_t lam (vs_{t+1} - V_{t+1}), and with w == 1 the
+    bracket is the GAE(lam) advantage at t+1, so pgadv_t is the GAE(lam) advantage at t -- computed here as the explicit
+    double sum of discounted TD errors.  A q_t that used vs_{t+1} alone (lam = 1) or V_{t+1} alone would fail."""
+    T, B, gam = 12, 4, 0.99
+    V, r, d, logpi, _ = traj(T, B, 21)
+    _, pg, _ = O.vtrace(V, r, d, logpi, logpi, gamma=gam, lam=lam)
+    delta = r + gam * (1.0 - d) * V[1:] - V[:-1]
+    ref = np.zeros((T, B))
+    for b in range(B):
+        for t in range(T):
+            prod = 1.0
+            for k in range(t, T):
+                ref[t, b] += prod * delta[k, b]; prod *= gam * lam * (1.0 - d[k, b])
+    np.testing.assert_allclose(pg, ref, rtol=1e-11, atol=1e-12)
+    # the two degenerate mixes differ from it by far more than the tolerance (so the pin can fail)
+    _, pg1, _ = O.vtrace(V, r, d, logpi, logpi, gamma=gam, lam=1.0)
+    assert np.abs(pg1 - ref).max() > 1e-3 and np.abs(delta - ref).max() > 1e-3
+
+
+def test_vtrace_off_policy_definition_and_separate_pg_threshold():
+    """General off-policy case against the definition as a double sum, with three DIFFERENT thresholds (rho_bar = 2,
+    c_bar = 1.5, rho_pg_bar = 0.7) and lam = 0.9: pgadv = min(rho_pg_bar, w) (r + disc (lam vs_{t+1} + (1-lam) V_{t+1}) - V)."""
+    T, B, gam, lam = 10, 16, 0.99, 0.9
+    V, r, d, logpi, logmu = traj(T, B, 22)
+    w = np.exp(logpi - logmu)
+    assert (w > 2.0).any() and ((w > 0.7) & (w < 1.5)).any() and ((w > 1.5) & (w < 2.0)).any() and (w < 0.7).any()
+    vs, pg, rho = O.vtrace(V, r, d, logpi, logmu, gamma=gam, lam=lam, rho_bar=2.0, c_bar=1.5, rho_pg_bar=0.7)
+    vs_ref = brute_vtrace_definition(V, r, d, w, gam, lam, 2.0, 1.5)
+    np.testing.assert_allclose(vs, vs_ref, rtol=1e-11, atol=1e-12)
+    vs_next = np.concatenate([vs_ref[1:], V[-1:]], axis=0)                        # vs_T = V_T
+    q = r + gam * (1.0 - d) * (lam * vs_next + (1.0 - lam) * V[1:])
+    pg_ref = np.minimum(0.7, w) * (q - V[:-1])
+    np.testing.assert_allclose(pg, pg_ref, rtol=1e-11, atol=1e-12)
+    np.testing.assert_allclose(rho, np.minimum(2.0, w), rtol=1e-14)
+    # a pgadv clipped at rho_bar instead of rho_pg_bar would be visibly different
+    assert np.abs(np.minimum(2.0, w) * (q - V[:-1]) - pg_ref).max() > 1e-2
+
+
 # ------------------------------------------------------------------ GAE (A3) ---------------------
 def test_gae_lambda_one_and_zero():
     V, r, d, _, _ = traj(17, 4, 7)
@@ -378,3 +433,72 @@ def test_impala_env_split_minibatches_equal_sequential_single_steps():
         assert out["params"].tobytes() == p.tobytes() and out["v"].tobytes() == v.tobytes()
         if opt == 1:
             assert not out["m"].any()          # RMSprop keeps its state in the second buffer only
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT row f4: actor-time values for GAE (A3b, Alg. 1 l.8-12), the epoch
+# counter of the PPO permutation (A23) and RMSprop under the PPO schedule
+# ---------------------------------------------------------------------------------------------------
+def _ppo_by_hand(oa, hp, p, m, v, k, obs, act, rew, dones, bl, values, epoch0):
+    """Alg. 1 l.11-20 composed from the separately pinned pieces: GAE on `values`, per-epoch permutation, and for every
+    minibatch the PPO objective gradient (finite-difference-pinned) followed by clip + Adam (closed-form-pinned)."""
+    T, B = hp.T, hp.B; N = T * B; A = bl.shape[-1]
+    adv, ret = O.gae(values.reshape(T + 1, B).astype(np.float64), rew, dones, hp.gamma, hp.lambda_)
+    lpb, _ = O.log_softmax(bl.reshape(N, A).astype(np.float64)); lpo = lpb[np.arange(N), act.ravel()]
+    frames = obs.reshape((T + 1) * B, *obs.shape[-3:]); mbs = N // hp.minibatches; losses = []
+    for e in range(hp.epochs):
+        perm = O.permutation(hp.perm_seed, epoch0 + e, N)
+        for j in range(hp.minibatches):
+            idx = perm[j * mbs:(j + 1) * mbs]
+            L, g = O.ppo_objective_f64(oa, hp, p.astype(np.float64), frames[idx], act.ravel()[idx], adv.ravel()[idx], ret.ravel()[idx], lpo[idx], want_grad=True)
+            k += 1
+            p, m, v, _ = O.clip_adam(p, m, v, g, k, hp.lr, hp.beta1, hp.beta2, hp.adam_eps, hp.max_grad_norm)
+            losses.append(L)
+    return p, m, v, k, np.array(losses), adv, ret
+
+
+def test_ppo_behaviour_values_and_epoch_counter():
+    arch = TINY; oa = to_orc(arch); T, B = 4, 3
+    obs, act, rew, dones, bl = make_step_inputs(T, B, 71)
+    p = synth.gen_params(arch, 13, bias_scale=0.1); z = np.zeros_like(p)
+    hp = O.make_hparams("ppo", T, B, epochs=2, minibatches=2, perm_seed=9)
+    # (1) NULL = recompute (A3): equals the hand composition on the oracle's own fp64 values
+    o0 = O.learner_step(oa, hp, p, z, z, 0, obs, act, rew, dones, bl, debug=True)
+    ph, mh, vh, kh, Lh, adv, ret = _ppo_by_hand(oa, hp, p, z, z, 0, obs, act, rew, dones, bl, o0["values"], 0)
+    assert o0["params"].tobytes() == ph.tobytes() and o0["m"].tobytes() == mh.tobytes() and o0["v"].tobytes() == vh.tobytes() and kh == 4
+    np.testing.assert_allclose(o0["stats"][:, 0], Lh, rtol=2e-6, atol=1e-7)
+    # (2) actor-time values = the same values as the ABI carries them (fp32): bit-identical to the hand composition on
+    #     those fp32 values, and within fp32 rounding of the recomputing step
+    bv = o0["values"].astype(np.float32)
+    o1 = O.learner_step(oa, hp, p, z, z, 0, obs, act, rew, dones, bl, debug=True, behaviour_values=bv)
+    ph, mh, vh, _, Lh, adv, ret = _ppo_by_hand(oa, hp, p, z, z, 0, obs, act, rew, dones, bl, bv, 0)
+    assert o1["params"].tobytes() == ph.tobytes() and o1["v"].tobytes() == vh.tobytes()
+    np.testing.assert_array_equal(o1["t0"], adv.ravel()); np.testing.assert_array_equal(o1["t1"], ret.ravel())
+    np.testing.assert_allclose(o1["t0"], o0["t0"], rtol=0, atol=1e-5)
+    # (3) values of ANOTHER policy (what the Cleanba architecture hands the learner: D of the second latest policy) change the
+    #     targets, and only through GAE: the step still equals the hand composition
+    bv2 = (bv + synth.rng(72).standard_normal(bv.size).astype(np.float32) * 0.3).astype(np.float32)
+    o2 = O.learner_step(oa, hp, p, z, z, 0, obs, act, rew, dones, bl, debug=True, behaviour_values=bv2)
+    ph, _, _, _, _, adv2, _ = _ppo_by_hand(oa, hp, p, z, z, 0, obs, act, rew, dones, bl, bv2, 0)
+    assert o2["params"].tobytes() == ph.tobytes() and np.abs(adv2 - adv).max() > 1e-2
+    # IMPALA ignores the argument (V-trace uses the current parameters' values, O4)
+    hi = O.make_hparams("impala", T, B)
+    a = O.learner_step(oa, hi, p, z, z, 0, obs, act, rew, dones, bl); b = O.learner_step(oa, hi, p, z, z, 0, obs, act, rew, dones, bl, behaviour_values=bv2)
+    assert a["params"].tobytes() == b["params"].tobytes()
+    # (4) A23: a call entered with opt_step = 4 (= after one call of 2 x 2 updates) continues with epochs 2, 3
+    o3 = O.learner_step(oa, hp, o0["params"], o0["m"], o0["v"], 4, obs, act, rew, dones, bl, debug=True)
+    ph, _, _, kh, _, _, _ = _ppo_by_hand(oa, hp, o0["params"], o0["m"], o0["v"], 4, obs, act, rew, dones, bl, o3["values"], 2)
+    assert o3["params"].tobytes() == ph.tobytes() and o3["opt_step"] == kh == 8
+    assert not np.array_equal(O.permutation(9, 2, T * B), O.permutation(9, 0, T * B))
+
+
+def test_ppo_with_rmsprop_follows_the_same_schedule():
+    """cb_hparams.optimizer = 1 under the PPO schedule (reachable through the ABI): each update is clip + RMSprop (A22)."""
+    arch = TINY; oa = to_orc(arch); T, B = 3, 2
+    obs, act, rew, dones, bl = make_step_inputs(T, B, 81)
+    p = synth.gen_params(arch, 14, bias_scale=0.1); z = np.zeros_like(p)
+    hp = O.make_hparams("ppo", T, B, epochs=1, minibatches=1, optimizer=1)
+    o = O.learner_step(oa, hp, p, z, z, 0, obs, act, rew, dones, bl, debug=True)
+    th, nu, n = O.clip_rmsprop(p, z, o["grad"], hp.lr, hp.rms_decay, hp.rms_eps, hp.max_grad_norm)
+    assert o["params"].tobytes() == th.tobytes() and o["v"].tobytes() == nu.tobytes() and not o["m"].any()
+    assert o["stats"][0, 4] == pytest.approx(n, rel=1e-6)
