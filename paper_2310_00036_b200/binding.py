@@ -19,7 +19,11 @@ ALGO = {"impala": 0, "ppo": 1}
 EXPORTS = ["cb_net_create", "cb_net_destroy", "cb_param_count", "cb_param_layout", "cb_net_init", "cb_policy_forward",
            "cb_learner_step", "cb_learner_view", "cb_sample_actions", "cb_logprob_entropy", "cb_vtrace", "cb_gae",
            "cb_permutation", "cb_clip_adam_scratch_bytes", "cb_clip_adam", "cb_last_error",
-           "cb_launch_count", "cb_profile_begin", "cb_profile_end", "cb_clip_rmsprop", "cb_linear_lr"]
+           "cb_launch_count", "cb_profile_begin", "cb_profile_end", "cb_clip_rmsprop", "cb_linear_lr",
+           "cb_learner_begin", "cb_learner_grad", "cb_learner_apply", "cb_sum_ranks", "cb_check_errors",
+           "cb_debug_inject_timeout", "cb_permutation_ws",
+           "cb_pipeline_create", "cb_pipeline_destroy", "cb_pipeline_run", "cb_pipeline_wait", "cb_pipeline_state", "cb_pipeline_records",
+           "cb_pipeline_rollout", "cb_pipeline_policy_version", "cb_env_state_ints", "cb_env_reset", "cb_env_step"]
 
 
 class CArch(C.Structure):
@@ -62,6 +66,9 @@ def lib():
         L.cb_linear_lr.argtypes = [C.c_float, C.c_uint64, C.c_uint64]
         L.cb_net_destroy.restype = None
         L.cb_net_destroy.argtypes = [C.c_void_p]
+        L.cb_pipeline_destroy.restype = None
+        L.cb_pipeline_destroy.argtypes = [C.c_void_p]
+        L.cb_env_state_ints.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -117,9 +124,7 @@ class Net:
     """cb_net handle.  Creating it and cb_net_init need no GPU; everything else does."""
 
     def __init__(self, arch: ArchSpec, max_frames=0):
-        a = CArch(); a.kind = {"nature": 0, "impala": 1}[arch.kind]
-        a.in_c, a.in_h, a.in_w = arch.in_c, arch.in_h, arch.in_w
-        a.channels[:] = list(arch.channels); a.fc = arch.fc; a.n_actions = arch.n_actions
+        a = _arch_struct(arch)
         self.arch = arch; self._h = C.c_void_p()
         _check(lib().cb_net_create(C.byref(a), C.c_int(max_frames), C.byref(self._h)))
         self.P = int(lib().cb_param_count(self._h)); self.A = arch.n_actions
@@ -164,21 +169,61 @@ class Net:
                                        _ptr(actions), _stream()))
         return logits, value, actions
 
-    def learner_step(self, params, adam_m, adam_v, opt_step, obs, actions, rewards, dones, behaviour_logits, hp, stats=None):
-        """cb_learner_step on the current torch stream; params/adam_m/adam_v are updated in place.
-        Returns (new opt_step, stats tensor [n_updates, 8])."""
+    def _learner_args(self, params, adam_m, adam_v, obs, actions, rewards, dones, behaviour_logits, behaviour_values, hp, stats):
         torch = _torch()
         for t, n in ((params, "params"), (adam_m, "adam_m"), (adam_v, "adam_v"), (rewards, "rewards"), (behaviour_logits, "behaviour_logits")):
             _dev(t, torch.float32, n)
         _dev(obs, torch.uint8, "obs"); _dev(dones, torch.uint8, "dones"); _dev(actions, torch.int32, "actions")
+        if behaviour_values is not None:
+            _dev(behaviour_values, torch.float32, "behaviour_values")
         n_upd = hp.epochs * hp.minibatches if hp.algo == 1 else max(1, hp.minibatches)
         if stats is None:
             stats = torch.zeros((n_upd, N_STATS), dtype=torch.float32, device=obs.device)
+        return n_upd, stats
+
+    def learner_step(self, params, adam_m, adam_v, opt_step, obs, actions, rewards, dones, behaviour_logits, hp, stats=None,
+                     behaviour_values=None):
+        """cb_learner_step on the current torch stream; params/adam_m/adam_v are updated in place.
+        behaviour_values: cuda fp32 [T+1,B] actor-time values (PPO, A3b) or None.
+        Returns (new opt_step, stats tensor [n_updates, 8])."""
+        n_upd, stats = self._learner_args(params, adam_m, adam_v, obs, actions, rewards, dones, behaviour_logits, behaviour_values, hp, stats)
         k = C.c_uint64(opt_step)
         rc = _check(lib().cb_learner_step(self._h, _ptr(params), _ptr(adam_m), _ptr(adam_v), C.byref(k), _ptr(obs), _ptr(actions),
-                                          _ptr(rewards), _ptr(dones), _ptr(behaviour_logits), C.byref(hp), _ptr(stats), _stream()))
+                                          _ptr(rewards), _ptr(dones), _ptr(behaviour_logits), _ptr(behaviour_values), C.byref(hp),
+                                          _ptr(stats), _stream()))
         assert rc == n_upd
         return k.value, stats
+
+    def learner_begin(self, params, adam_m, adam_v, opt_step, obs, actions, rewards, dones, behaviour_logits, hp, stats=None,
+                      behaviour_values=None):
+        """cb_learner_begin.  Returns (n_updates, stats, handle); the handle keeps every buffer (and the host step counter)
+        alive until the last learner_apply; handle.opt_step is the running update count."""
+        n_upd, stats = self._learner_args(params, adam_m, adam_v, obs, actions, rewards, dones, behaviour_logits, behaviour_values, hp, stats)
+        h = _LearnHandle(C.c_uint64(opt_step), (params, adam_m, adam_v, obs, actions, rewards, dones, behaviour_logits, behaviour_values, hp, stats))
+        rc = _check(lib().cb_learner_begin(self._h, _ptr(params), _ptr(adam_m), _ptr(adam_v), C.byref(h.k), _ptr(obs), _ptr(actions),
+                                           _ptr(rewards), _ptr(dones), _ptr(behaviour_logits), _ptr(behaviour_values), C.byref(hp),
+                                           _ptr(stats), _stream()))
+        assert rc == n_upd
+        self._learn = h
+        return n_upd, stats, h
+
+    def learner_grad(self, update):
+        """cb_learner_grad: computes update `update`'s gradient; returns it as a torch VIEW of the library-owned [P] buffer."""
+        torch = _torch()
+        g = C.c_void_p()
+        _check(lib().cb_learner_grad(self._h, C.c_int(update), C.byref(g), _stream()))
+        return torch.as_tensor(_DevView(g.value, self.P), device="cuda")
+
+    def learner_apply(self, update):
+        _check(lib().cb_learner_apply(self._h, C.c_int(update), _stream()))
+        return self._learn.opt_step
+
+    def check_errors(self):
+        """cb_check_errors: synchronises the current stream; raises if a kernel reported a pipeline time-out."""
+        _check(lib().cb_check_errors(self._h, _stream()))
+
+    def debug_inject_timeout(self, precision="bf16"):
+        _check(lib().cb_debug_inject_timeout(self._h, C.c_int(PREC.get(precision, precision)), _stream()))
 
     def learner_view(self, which):
         """Copy of a library-owned result of the last learner step (cb_learner_view) as a torch tensor."""
@@ -189,11 +234,124 @@ class Net:
         return torch.as_tensor(_DevView(p.value, n.value), device="cuda").clone()
 
 
+class _LearnHandle:
+    def __init__(self, k, keep):
+        self.k = k; self._keep = keep
+
+    @property
+    def opt_step(self):
+        return int(self.k.value)
+
+
 class _DevView:
     """__cuda_array_interface__ holder for a library-owned fp32 device buffer."""
 
     def __init__(self, ptr, n):
         self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f4", "data": (ptr, False), "version": 2}
+
+
+# ---- Cleanba's actor/learner architecture (cb_pipeline_*) and the synthetic environment ------------------
+class CPipelineCfg(C.Structure):
+    _fields_ = [("sync", C.c_int), ("actor_values", C.c_int), ("serial", C.c_int), ("env_seed", C.c_uint64), ("sample_seed", C.c_uint64)]
+
+
+class CPipelineRecord(C.Structure):
+    _fields_ = [("iteration", C.c_int), ("data_policy_version", C.c_int), ("learner_version_before", C.c_int), ("learner_version_after", C.c_int)]
+
+
+def _arch_struct(arch):
+    a = CArch(); a.kind = {"nature": 0, "impala": 1}[arch.kind]
+    a.in_c, a.in_h, a.in_w = arch.in_c, arch.in_h, arch.in_w
+    a.channels[:] = list(arch.channels); a.fc = arch.fc; a.n_actions = arch.n_actions
+    return a
+
+
+def pipeline_policy_version(sync, iteration):
+    """cb_pipeline_policy_version (host arithmetic, needs no GPU)."""
+    return int(lib().cb_pipeline_policy_version(C.c_int(1 if sync else 0), C.c_int(iteration)))
+
+
+class Pipeline:
+    """cb_pipeline handle: actor stream + learner stream with event-ordered double buffers (Figure 1 right / Table 1)."""
+
+    def __init__(self, arch, hp, params, sync=False, actor_values=False, serial=False, env_seed=1, sample_seed=2):
+        torch = _torch(); _dev(params, torch.float32, "params")
+        cfg = CPipelineCfg(1 if sync else 0, 1 if actor_values else 0, 1 if serial else 0, env_seed, sample_seed)
+        a = _arch_struct(arch)
+        self.arch, self.hp, self._h = arch, hp, C.c_void_p()
+        _check(lib().cb_pipeline_create(C.byref(a), C.byref(hp), C.byref(cfg), _ptr(params), C.byref(self._h)))
+        self.T, self.B, self.A = hp.T, hp.B, arch.n_actions
+        self.n_upd = hp.epochs * hp.minibatches if hp.algo == 1 else max(1, hp.minibatches)
+        self.P = params.numel()
+
+    def close(self):
+        if self._h:
+            lib().cb_pipeline_destroy(self._h); self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def run(self, iterations):
+        _check(lib().cb_pipeline_run(self._h, C.c_int(iterations)))
+
+    def wait(self):
+        """Waits for both streams; returns the device time (ms) of the last run()."""
+        ms = C.c_float()
+        _check(lib().cb_pipeline_wait(self._h, C.byref(ms)))
+        return float(ms.value)
+
+    def state(self):
+        """(params, adam_m, adam_v) as torch COPIES, opt_step, iterations; waits first."""
+        torch = _torch(); self.wait()
+        p, m, v = C.c_void_p(), C.c_void_p(), C.c_void_p(); k = C.c_uint64(); it = C.c_int()
+        _check(lib().cb_pipeline_state(self._h, C.byref(p), C.byref(m), C.byref(v), C.byref(k), C.byref(it)))
+        cp = lambda q: torch.as_tensor(_DevView(q.value, self.P), device="cuda").clone()
+        return cp(p), cp(m), cp(v), int(k.value), int(it.value)
+
+    def records(self, max_n=64):
+        buf = (CPipelineRecord * max_n)()
+        n = _check(lib().cb_pipeline_records(self._h, buf, C.c_int(max_n)))
+        return [(r.iteration, r.data_policy_version, r.learner_version_before, r.learner_version_after) for r in buf[:n]]
+
+    def rollout(self, iteration):
+        """Copies of the rollout storage D of `iteration` (one of the last two) and of its learner call's stats; waits first."""
+        torch = _torch(); self.wait()
+        ptr = [C.c_void_p() for _ in range(7)]
+        _check(lib().cb_pipeline_rollout(self._h, C.c_int(iteration), *[C.byref(q) for q in ptr]))
+        T, B, A, a = self.T, self.B, self.A, self.arch
+
+        def view(q, n, typestr, shape):
+            h = _DevView(q.value, n); h.__cuda_array_interface__["typestr"] = typestr
+            return torch.as_tensor(h, device="cuda").clone().reshape(shape)
+        return dict(obs=view(ptr[0], (T + 1) * B * a.in_c * a.in_h * a.in_w, "|u1", (T + 1, B, a.in_c, a.in_h, a.in_w)),
+                    actions=view(ptr[1], T * B, "<i4", (T, B)), rewards=view(ptr[2], T * B, "<f4", (T, B)), dones=view(ptr[3], T * B, "|u1", (T, B)),
+                    behaviour_logits=view(ptr[4], T * B * A, "<f4", (T, B, A)), values=view(ptr[5], (T + 1) * B, "<f4", (T + 1, B)),
+                    stats=view(ptr[6], self.n_upd * N_STATS, "<f4", (self.n_upd, N_STATS)))
+
+
+def env_state_ints():
+    return int(lib().cb_env_state_ints())
+
+
+def env_reset(seed, B, arch):
+    torch = _torch()
+    state = torch.zeros((B, env_state_ints()), dtype=torch.int32, device="cuda")
+    obs = torch.empty((B, arch.in_c, arch.in_h, arch.in_w), dtype=torch.uint8, device="cuda")
+    _check(lib().cb_env_reset(C.c_uint64(seed), C.c_int(B), C.c_int(arch.in_c), C.c_int(arch.in_h), C.c_int(arch.in_w), _ptr(state), _ptr(obs), _stream()))
+    return state, obs
+
+
+def env_step(seed, global_step, actions, state, obs):
+    """In place on `state`; returns (next obs, rewards, dones)."""
+    torch = _torch(); _dev(actions, torch.int32, "actions"); _dev(state, torch.int32, "state"); _dev(obs, torch.uint8, "obs")
+    B, Cc, H, W = obs.shape
+    out = torch.empty_like(obs); rew = torch.empty((B,), dtype=torch.float32, device="cuda"); done = torch.empty((B,), dtype=torch.uint8, device="cuda")
+    _check(lib().cb_env_step(C.c_uint64(seed), C.c_int(B), C.c_int(Cc), C.c_int(H), C.c_int(W), C.c_uint32(global_step), _ptr(actions), _ptr(state),
+                             _ptr(obs), _ptr(out), _ptr(rew), _ptr(done), _stream()))
+    return out, rew, done
 
 
 # ---- sub-step entry points --------------------------------------------------------------------------
@@ -235,6 +393,15 @@ def permutation(seed, epoch, N):
     perm = torch.empty((N,), dtype=torch.int32, device="cuda")
     _check(lib().cb_permutation(C.c_uint64(seed), C.c_uint32(epoch), C.c_int(N), _ptr(perm), _stream()))
     return perm
+
+
+def sum_ranks(slices, scale=1.0, out=None):
+    """cb_sum_ranks: slices cuda fp32 [G, n] -> scale * (sum over G in rank order), cuda fp32 [n]."""
+    torch = _torch(); _dev(slices, torch.float32, "slices"); G, n = slices.shape
+    if out is None:
+        out = torch.empty((n,), dtype=torch.float32, device=slices.device)
+    _check(lib().cb_sum_ranks(_ptr(slices), C.c_int(G), C.c_size_t(n), C.c_float(scale), _ptr(out), _stream()))
+    return out
 
 
 def clip_adam(params, adam_m, adam_v, grad, k, lr, beta1=0.9, beta2=0.999, eps=1e-5, max_norm=40.0, scratch=None):

@@ -7,6 +7,8 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 
 namespace cb {
 
@@ -167,6 +169,7 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
     CB_ALLOC(ws.wf, net->wf_total * es); CB_ALLOC(ws.wd, net->wd_total * es); CB_ALLOC(ws.bias, net->bias_total * 4);
     if (prec == CB_PREC_BF16_TC) { CB_ALLOC(ws.w0img, conv0_wimg_elems(net->layers[0].g) * 2); CB_ALLOC(ws.wtc_f, net->wf_total * 2); CB_ALLOC(ws.wtc_d, net->wf_total * 2); }
     CB_ALLOC(ws.errflag, 16); CB_CUDA(cudaMemset(ws.errflag, 0, 16));
+    CB_CUDA(cudaHostAlloc((void**)&ws.errhost, 16, cudaHostAllocMapped)); *ws.errhost = 0;      // with UVA the host address is valid on the device
     {
       std::vector<PackDesc> tab;
       for (const Layer& L : net->layers)
@@ -206,9 +209,9 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
 int ensure_learner_scratch(cb_net* net, int prec, int F, int N, int epochs) {
   Workspace& ws = net->ws[prec];
   if (ws.learn_frames >= F && ws.learn_N >= N && ws.learn_epochs >= epochs) return CB_OK;
+  F = std::max(F, ws.learn_frames); N = std::max(N, ws.learn_N); epochs = std::max(std::max(epochs, 1), ws.learn_epochs);      // grow-only: take the maxima BEFORE the old sizes are cleared
   CB_CUDA(cudaDeviceSynchronize());
   free_scratch(ws);
-  F = std::max(F, ws.learn_frames); N = std::max(N, ws.learn_N); epochs = std::max(epochs, 1);
   size_t n4 = (size_t)N * 4;
   CB_ALLOC(ws.logpi, n4); CB_ALLOC(ws.logmu, n4); CB_ALLOC(ws.ent, n4); CB_ALLOC(ws.t0, n4); CB_ALLOC(ws.t1, n4); CB_ALLOC(ws.rho, n4);
   CB_ALLOC(ws.values, (size_t)F * (net->arch.n_actions + 1) * 4);
@@ -227,6 +230,18 @@ static void philox_host(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint
     c0 = n0; c1 = (uint32_t)p1; c2 = n2; c3 = (uint32_t)p0; k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
   }
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// one opt-in per (device, kernel); the cache is guarded: cb_net objects of different host threads share it
+int ensure_dyn_smem(const void* func, size_t bytes) {
+  static std::mutex mu; static std::map<std::pair<int, const void*>, size_t> done;
+  int dev = 0; CB_CUDA(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lk(mu);
+  size_t& cur = done[{dev, func}];
+  if (bytes <= cur) return CB_OK;
+  CB_CUDA(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  cur = bytes;
+  return CB_OK;
 }
 
 }  // namespace cb
@@ -259,11 +274,12 @@ void cb_net_destroy(cb_net* net) {
   cudaDeviceSynchronize();
   drop_fwd_graphs(net);
   if (net->capture_stream) cudaStreamDestroy(net->capture_stream);
+  if (net->aux_stream) { cudaStreamDestroy(net->aux_stream); cudaEventDestroy(net->ev_fork); cudaEventDestroy(net->ev_join); }
   for (int p = 0; p < 2; ++p) {
     Workspace& ws = net->ws[p];
     if (!ws.wf) continue;
     free_workspace(ws); free_scratch(ws);
-    cudaFree(ws.packtab); cudaFree(ws.w0img); cudaFree(ws.wtc_f); cudaFree(ws.wtc_d); cudaFree(ws.errflag);
+    cudaFree(ws.packtab); cudaFree(ws.w0img); cudaFree(ws.wtc_f); cudaFree(ws.wtc_d); cudaFree(ws.errflag); cudaFreeHost(ws.errhost);
     cudaFree(ws.wf); cudaFree(ws.wd); cudaFree(ws.bias); cudaFree(ws.gradbuf); cudaFree(ws.adam_scratch); cudaFree(ws.gnorm);
   }
   delete net;
@@ -305,6 +321,20 @@ int cb_net_init(const cb_net* net, uint64_t seed, float* params_host) {
 
 static int check_prec(int prec) { if (prec != CB_PREC_FP32_REF && prec != CB_PREC_BF16_TC) { set_error("bad precision mode"); return CB_EINVAL; } return CB_OK; }
 static bool misaligned(const void* p, size_t a) { return ((uintptr_t)p & (a - 1)) != 0; }
+
+// raised host word -> CB_ECUDA once, condition cleared (cleanba.h, asynchronous errors)
+static int report_async_error(cb_net* net, cudaStream_t st) {
+  int code = 0;
+  for (int p = 0; p < 2; ++p) {
+    Workspace& ws = net->ws[p];
+    if (!ws.errhost) continue;
+    const int h = *(volatile int*)ws.errhost;
+    if (h) { code = h; *(volatile int*)ws.errhost = 0; cudaMemsetAsync(ws.errflag, 0, sizeof(int), st); ws.packed = false; }
+  }
+  if (!code) return CB_OK;
+  set_error("a tcgen05 pipeline wait timed out inside an earlier call on this net (site %d): that call's stats / logits were poisoned with NaN and its optimizer step was skipped", code);
+  return CB_ECUDA;
+}
 
 // The actor calls the trunk thousands of times with the same shapes and a handful of observation buffers, and at B = 128 its
 // ~18 kernels are shorter than their host-side launch cost (tensor-map encoding included).  The first call with a given
@@ -349,28 +379,43 @@ int cb_policy_forward(cb_net* net, const float* params, const uint8_t* obs, int 
   if (!net || !obs || B < 0) { set_error("null or negative argument"); return CB_EINVAL; }
   if (check_prec(precision)) return CB_EINVAL;
   if (params && misaligned(params, 16)) { set_error("params must be 16-byte aligned"); return CB_EINVAL; }
+  if (misaligned(obs, 4)) { set_error("obs must be 4-byte aligned"); return CB_EINVAL; }
   if (B == 0) return CB_OK;
   cudaStream_t st = (cudaStream_t)stream; int rc;
+  if ((rc = report_async_error(net, st))) return rc;
   if ((rc = ensure_workspace(net, precision, B))) return rc;
   if (params) { if ((rc = pack_weights(net, precision, params, st))) return rc; }
-  else if (!net->ws[precision].packed) { set_error("params == NULL but no weights have been packed in this precision mode yet"); return CB_EINVAL; }
+  else if (!net->ws[precision].packed) { set_error("params == NULL but this net holds no current packed weights in this precision mode (none packed yet, or a learner call has run since)"); return CB_EINVAL; }
   if ((rc = trunk_forward(net, precision, obs, B, st))) return rc;      // everything up to the hidden layer
   Workspace& ws = net->ws[precision];
   const Layer& HL = net->layers.back();
   const int A = net->arch.n_actions;
   const size_t es = precision == CB_PREC_FP32_REF ? 4 : 2;
   if ((rc = launch_heads_sample(precision, ws.act[net->hid_t], (const char*)ws.wf + HL.wf_off * es, ws.bias + HL.bias_off, B, net->arch.fc, A, seed, step,
-                                env_offset, (float*)ws.act[net->head_t], logits, value, actions, st))) return rc;
+                                env_offset, (float*)ws.act[net->head_t], logits, value, actions, st, ws.errflag, ws.errhost))) return rc;
   return CB_OK;
 }
 
-int cb_learner_step(cb_net* net, float* params, float* adam_m, float* adam_v, uint64_t* opt_step, const uint8_t* obs, const int32_t* actions,
-                    const float* rewards, const uint8_t* dones, const float* behaviour_logits, const cb_hparams* hp, float* stats, void* stream) {
+// The operand-layout weights of an update: packed from the CURRENT master parameters at the start of every gradient computation.
+static int learner_optimizer(cb_net* net, Workspace& ws, int u, cudaStream_t st) {
+  cb_net::LearnCtx& c = net->lc; const cb_hparams& hp = c.hp;
+  float* row = c.stats + (size_t)u * CB_N_STATS;
+  *c.opt_step += 1;
+  if (hp.optimizer == 1)
+    return launch_clip_rmsprop(net->P, c.params, c.adam_v, ws.gradbuf, hp.lr, hp.rms_decay, hp.rms_eps, hp.max_grad_norm, ws.gnorm, row + 4, ws.adam_scratch, st, ws.errflag, ws.errhost);
+  return launch_clip_adam(net->P, c.params, c.adam_m, c.adam_v, ws.gradbuf, *c.opt_step, hp.lr, hp.beta1, hp.beta2, hp.adam_eps, hp.max_grad_norm, ws.gnorm, row + 4,
+                          ws.adam_scratch, st, ws.errflag, ws.errhost);
+}
+
+int cb_learner_begin(cb_net* net, float* params, float* adam_m, float* adam_v, uint64_t* opt_step, const uint8_t* obs, const int32_t* actions,
+                     const float* rewards, const uint8_t* dones, const float* behaviour_logits, const float* behaviour_values, const cb_hparams* hp,
+                     float* stats, void* stream) {
   if (!net || !params || !adam_m || !adam_v || !opt_step || !obs || !actions || !rewards || !dones || !behaviour_logits || !hp || !stats) { set_error("null argument"); return CB_EINVAL; }
   if (check_prec(hp->precision)) return CB_EINVAL;
   if (hp->algo != CB_ALGO_IMPALA && hp->algo != CB_ALGO_PPO) { set_error("bad algo"); return CB_EINVAL; }
   if (hp->T < 1 || hp->B < 1) { set_error("T and B must be positive"); return CB_EINVAL; }
   if (misaligned(params, 16) || misaligned(adam_m, 16) || misaligned(adam_v, 16)) { set_error("params / adam buffers must be 16-byte aligned"); return CB_EINVAL; }
+  if (misaligned(obs, 4)) { set_error("obs must be 4-byte aligned"); return CB_EINVAL; }
   const int prec = hp->precision, T = hp->T, B = hp->B, A = net->arch.n_actions;
   if ((long long)(T + 1) * B * net->arch.in_h * net->arch.in_w >= 0x7fffffffLL) { set_error("(T+1)*B*H*W must stay below 2^31"); return CB_EINVAL; }
   const int N = T * B, F = (T + 1) * B;
@@ -380,71 +425,129 @@ int cb_learner_step(cb_net* net, float* params, float* adam_m, float* adam_v, ui
   if (!ppo && B % mb != 0) { set_error("IMPALA needs minibatches dividing B (env groups, A21)"); return CB_EINVAL; }
   if (hp->optimizer != 0 && hp->optimizer != 1) { set_error("bad optimizer"); return CB_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream; int rc;
+  net->lc.active = false;
+  if ((rc = report_async_error(net, st))) return rc;
   if ((rc = ensure_workspace(net, prec, F))) return rc;
   if ((rc = ensure_learner_scratch(net, prec, F, N, ppo ? hp->epochs : 1))) return rc;
   Workspace& ws = net->ws[prec];
-  net->last_prec = prec; net->last_F = F; net->last_N = N; net->last_ppo = ppo || mb > 1;
-  if ((rc = pack_weights(net, prec, params, st))) return rc;
-  if ((rc = forward(net, prec, obs, nullptr, F, st))) return rc;
-  float* head = (float*)ws.act[net->head_t];
+  const bool given_values = ppo && behaviour_values;
+  net->last_prec = prec; net->last_F = F; net->last_N = N; net->last_ppo = ppo || mb > 1; net->last_has_head = !given_values && (ppo || mb == 1);
+  cb_net::LearnCtx& c = net->lc;
+  c.params = params; c.adam_m = adam_m; c.adam_v = adam_v; c.opt_step = opt_step; c.obs = obs; c.actions = actions; c.rewards = rewards; c.dones = dones;
+  c.stats = stats; c.hp = *hp; c.mb = mb; c.ppo = ppo; c.next_grad = c.next_apply = 0;
+  c.n_updates = ppo ? hp->epochs * hp->minibatches : mb;
+  // old log-probs log mu(a|s) from the behaviour logits (O4 / O6)
   if ((rc = launch_logprob(behaviour_logits, A, N, A, actions, nullptr, ws.logmu, nullptr, st))) return rc;
-  auto optimizer_step = [&](float* stats_row) -> int {
-    *opt_step += 1;
-    if (hp->optimizer == 1)
-      return launch_clip_rmsprop(net->P, params, adam_v, ws.gradbuf, hp->lr, hp->rms_decay, hp->rms_eps, hp->max_grad_norm, ws.gnorm, stats_row + 4, ws.adam_scratch, st);
-    return launch_clip_adam(net->P, params, adam_m, adam_v, ws.gradbuf, *opt_step, hp->lr, hp->beta1, hp->beta2, hp->adam_eps, hp->max_grad_norm, ws.gnorm, stats_row + 4, ws.adam_scratch, st);
-  };
-  if (!ppo && mb == 1) {
-    if ((rc = launch_logprob(head, A + 1, N, A, actions, nullptr, ws.logpi, nullptr, st))) return rc;
-    if ((rc = launch_vtrace(T, B, head + A, A + 1, rewards, dones, ws.logpi, ws.logmu, hp->gamma, hp->lambda_, hp->rho_bar, hp->c_bar, hp->rho_pg_bar, ws.t0, ws.t1, ws.rho, st))) return rc;
-    if ((rc = launch_impala_loss(prec, N, A, head, actions, ws.t0, ws.t1, ws.rho, hp->vf_coef, hp->ent_coef, hp->loss_reduction, ws.grad[G_HEAD], ws.terms, ws.red, stats, st))) return rc;
-    if ((rc = backward(net, prec, obs, nullptr, N, ws.gradbuf, st))) return rc;
-    if ((rc = optimizer_step(stats))) return rc;
-    return 1;
+  float* head = (float*)ws.act[net->head_t];
+  if (ppo) {
+    // Alg. 1 l.11-12: advantages and returns, from the actor's values (A3b) or from a no-grad forward with the iteration-start
+    // parameters (A3).  The epoch permutations (A17, A23) are independent of both: they run on a side stream underneath.
+    if (!net->aux_stream) { CB_CUDA(cudaStreamCreateWithFlags(&net->aux_stream, cudaStreamNonBlocking)); CB_CUDA(cudaEventCreateWithFlags(&net->ev_fork, cudaEventDisableTiming)); CB_CUDA(cudaEventCreateWithFlags(&net->ev_join, cudaEventDisableTiming)); }
+    CB_CUDA(cudaEventRecord(net->ev_fork, st)); CB_CUDA(cudaStreamWaitEvent(net->aux_stream, net->ev_fork, 0));
+    if ((rc = launch_permutation(hp->perm_seed, (uint32_t)(*opt_step / (uint64_t)hp->minibatches), hp->epochs, N, ws.perm, ws.permj, net->aux_stream))) return rc;
+    CB_CUDA(cudaEventRecord(net->ev_join, net->aux_stream));
+    if (given_values) {
+      if ((rc = launch_gae(T, B, behaviour_values, 1, rewards, dones, hp->gamma, hp->lambda_, ws.t0, ws.t1, st))) return rc;
+    } else {
+      if ((rc = pack_weights(net, prec, params, st))) return rc;
+      if ((rc = forward(net, prec, obs, nullptr, F, st))) return rc;
+      CB_CUDA(cudaMemcpyAsync(ws.values, head, (size_t)F * (A + 1) * 4, cudaMemcpyDeviceToDevice, st));      // cb_learner_view(0)
+      if ((rc = launch_gae(T, B, ws.values + A, A + 1, rewards, dones, hp->gamma, hp->lambda_, ws.t0, ws.t1, st))) return rc;
+    }
+    CB_CUDA(cudaStreamWaitEvent(st, net->ev_join, 0));
   }
-  if (!ppo) {
+  c.active = true;
+  return c.n_updates;
+}
+
+int cb_learner_grad(cb_net* net, int u, float** grad_dev, void* stream) {
+  if (!net || !net->lc.active) { set_error("cb_learner_grad without cb_learner_begin"); return CB_EINVAL; }
+  cb_net::LearnCtx& c = net->lc; const cb_hparams& hp = c.hp;
+  if (u != c.next_grad || u != c.next_apply || u >= c.n_updates) { set_error("updates must be taken in order, each cb_learner_grad followed by its cb_learner_apply"); return CB_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream; int rc;
+  const int prec = hp.precision, T = hp.T, B = hp.B, A = net->arch.n_actions, N = T * B, F = (T + 1) * B;
+  Workspace& ws = net->ws[prec];
+  float* head = (float*)ws.act[net->head_t];
+  float* row = c.stats + (size_t)u * CB_N_STATS;
+  if (!(c.ppo && u == 0 && net->last_has_head)) { if ((rc = pack_weights(net, prec, c.params, st))) return rc; }      // PPO update 0 after the no-grad forward: same parameters, already packed
+  ws.packed = false;      // after this call the packs no longer hold what `params` holds (the optimizer runs next)
+  if (!c.ppo && c.mb == 1) {
+    if ((rc = forward(net, prec, c.obs, nullptr, F, st))) return rc;
+    if ((rc = launch_logprob(head, A + 1, N, A, c.actions, nullptr, ws.logpi, nullptr, st))) return rc;
+    if ((rc = launch_vtrace(T, B, head + A, A + 1, c.rewards, c.dones, ws.logpi, ws.logmu, hp.gamma, hp.lambda_, hp.rho_bar, hp.c_bar, hp.rho_pg_bar, ws.t0, ws.t1, ws.rho, st))) return rc;
+    if ((rc = launch_impala_loss(prec, N, A, head, c.actions, ws.t0, ws.t1, ws.rho, hp.vf_coef, hp.ent_coef, hp.loss_reduction, ws.grad[G_HEAD], ws.terms, ws.red, row, st))) return rc;
+    if ((rc = backward(net, prec, c.obs, nullptr, N, ws.gradbuf, st))) return rc;
+  } else if (!c.ppo) {
     // A21: one complete update per group of B/mb envs, in group order, each with the parameters the previous one left
-    const int Bm = B / mb, Nm = T * Bm, Fm = (T + 1) * Bm;
-    CB_CUDA(cudaMemcpyAsync(ws.values, head, (size_t)F * (A + 1) * 4, cudaMemcpyDeviceToDevice, st));      // cb_learner_view(0)
-    for (int k = 0; k < mb; ++k) {
-      float* st_out = stats + (size_t)k * CB_N_STATS;
-      if ((rc = launch_gather_traj(T, B, k * Bm, Bm, actions, rewards, dones, ws.logmu, ws.perm, ws.act_m, ws.rew_m, ws.dones_m, ws.logmu_m, st))) return rc;
-      if (k > 0) if ((rc = pack_weights(net, prec, params, st))) return rc;
-      if ((rc = forward(net, prec, obs, ws.perm, Fm, st))) return rc;
-      if ((rc = launch_logprob(head, A + 1, Nm, A, ws.act_m, nullptr, ws.logpi, nullptr, st))) return rc;
-      if ((rc = launch_vtrace(T, Bm, head + A, A + 1, ws.rew_m, ws.dones_m, ws.logpi, ws.logmu_m, hp->gamma, hp->lambda_, hp->rho_bar, hp->c_bar, hp->rho_pg_bar, ws.t0, ws.t1, ws.rho, st))) return rc;
-      if ((rc = launch_impala_loss(prec, Nm, A, head, ws.act_m, ws.t0, ws.t1, ws.rho, hp->vf_coef, hp->ent_coef, hp->loss_reduction, ws.grad[G_HEAD], ws.terms, ws.red, st_out, st))) return rc;
-      if ((rc = backward(net, prec, obs, ws.perm, Nm, ws.gradbuf, st))) return rc;
-      if ((rc = optimizer_step(st_out))) return rc;
-    }
-    return mb;
+    const int Bm = B / c.mb, Nm = T * Bm, Fm = (T + 1) * Bm;
+    if ((rc = launch_gather_traj(T, B, u * Bm, Bm, c.actions, c.rewards, c.dones, ws.logmu, ws.perm, ws.act_m, ws.rew_m, ws.dones_m, ws.logmu_m, st))) return rc;
+    if ((rc = forward(net, prec, c.obs, ws.perm, Fm, st))) return rc;
+    if ((rc = launch_logprob(head, A + 1, Nm, A, ws.act_m, nullptr, ws.logpi, nullptr, st))) return rc;
+    if ((rc = launch_vtrace(T, Bm, head + A, A + 1, ws.rew_m, ws.dones_m, ws.logpi, ws.logmu_m, hp.gamma, hp.lambda_, hp.rho_bar, hp.c_bar, hp.rho_pg_bar, ws.t0, ws.t1, ws.rho, st))) return rc;
+    if ((rc = launch_impala_loss(prec, Nm, A, head, ws.act_m, ws.t0, ws.t1, ws.rho, hp.vf_coef, hp.ent_coef, hp.loss_reduction, ws.grad[G_HEAD], ws.terms, ws.red, row, st))) return rc;
+    if ((rc = backward(net, prec, c.obs, ws.perm, Nm, ws.gradbuf, st))) return rc;
+  } else {
+    const int m = N / hp.minibatches, e = u / hp.minibatches, k = u % hp.minibatches;
+    const int32_t* idx = ws.perm + (size_t)e * N + (size_t)k * m;
+    if ((rc = forward(net, prec, c.obs, idx, m, st))) return rc;
+    if ((rc = launch_ppo_loss(prec, m, A, head, idx, c.actions, ws.t0, ws.t1, ws.logmu, hp.clip_eps, hp.vf_coef, hp.ent_coef, hp.norm_adv, ws.grad[G_HEAD], ws.terms, ws.red, ws.advstat, row, st))) return rc;
+    if ((rc = backward(net, prec, c.obs, idx, m, ws.gradbuf, st))) return rc;
   }
-  // PPO (Alg. 1 l.11-20): values and old log-probs from the iteration-start parameters
-  CB_CUDA(cudaMemcpyAsync(ws.values, head, (size_t)F * (A + 1) * 4, cudaMemcpyDeviceToDevice, st));
-  if ((rc = launch_gae(T, B, ws.values + A, A + 1, rewards, dones, hp->gamma, hp->lambda_, ws.t0, ws.t1, st))) return rc;
-  if ((rc = launch_permutation(hp->perm_seed, 0, hp->epochs, N, ws.perm, ws.permj, st))) return rc;
-  const int m = N / hp->minibatches; int upd = 0;
-  for (int e = 0; e < hp->epochs; ++e)
-    for (int k = 0; k < hp->minibatches; ++k, ++upd) {
-      const int32_t* idx = ws.perm + (size_t)e * N + (size_t)k * m;
-      if (upd > 0) if ((rc = pack_weights(net, prec, params, st))) return rc;
-      if ((rc = forward(net, prec, obs, idx, m, st))) return rc;
-      float* st_out = stats + (size_t)upd * CB_N_STATS;
-      if ((rc = launch_ppo_loss(prec, m, A, head, idx, actions, ws.t0, ws.t1, ws.logmu, hp->clip_eps, hp->vf_coef, hp->ent_coef, hp->norm_adv, ws.grad[G_HEAD], ws.terms, ws.red, ws.advstat, st_out, st))) return rc;
-      if ((rc = backward(net, prec, obs, idx, m, ws.gradbuf, st))) return rc;
-      if ((rc = optimizer_step(st_out))) return rc;
-    }
-  return upd;
+  c.next_grad = u + 1;
+  if (grad_dev) *grad_dev = ws.gradbuf;
+  return CB_OK;
+}
+
+int cb_learner_apply(cb_net* net, int u, void* stream) {
+  if (!net || !net->lc.active) { set_error("cb_learner_apply without cb_learner_begin"); return CB_EINVAL; }
+  cb_net::LearnCtx& c = net->lc;
+  if (u != c.next_apply || c.next_grad != u + 1) { set_error("cb_learner_apply(%d) must follow cb_learner_grad(%d)", u, u); return CB_EINVAL; }
+  int rc = learner_optimizer(net, net->ws[c.hp.precision], u, (cudaStream_t)stream);
+  if (rc) return rc;
+  c.next_apply = u + 1;
+  if (c.next_apply == c.n_updates) c.active = false;
+  return CB_OK;
+}
+
+int cb_learner_step(cb_net* net, float* params, float* adam_m, float* adam_v, uint64_t* opt_step, const uint8_t* obs, const int32_t* actions,
+                    const float* rewards, const uint8_t* dones, const float* behaviour_logits, const float* behaviour_values, const cb_hparams* hp,
+                    float* stats, void* stream) {
+  const int n = cb_learner_begin(net, params, adam_m, adam_v, opt_step, obs, actions, rewards, dones, behaviour_logits, behaviour_values, hp, stats, stream);
+  if (n < 0) return n;
+  for (int u = 0; u < n; ++u) {
+    int rc;
+    if ((rc = cb_learner_grad(net, u, nullptr, stream))) { net->lc.active = false; return rc; }
+    if ((rc = cb_learner_apply(net, u, stream))) { net->lc.active = false; return rc; }
+  }
+  return n;
+}
+
+int cb_check_errors(cb_net* net, void* stream) {
+  if (!net) { set_error("null argument"); return CB_EINVAL; }
+  CB_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+  return report_async_error(net, (cudaStream_t)stream);
+}
+
+int cb_debug_inject_timeout(cb_net* net, int precision, void* stream) {
+  if (!net || check_prec(precision)) return CB_EINVAL;
+  Workspace& ws = net->ws[precision];
+  if (!ws.errflag) { set_error("no workspace in this precision mode yet"); return CB_EINVAL; }
+  const int one = 99;
+  CB_CUDA(cudaMemcpyAsync(ws.errflag, &one, sizeof one, cudaMemcpyHostToDevice, (cudaStream_t)stream));
+  return CB_OK;
+}
+
+int cb_sum_ranks(const float* in, int G, size_t n, float scale, float* out, void* stream) {
+  if (!in || !out || G < 1) { set_error("bad argument"); return CB_EINVAL; }
+  return launch_sum_ranks(in, G, n, scale, out, (cudaStream_t)stream);
 }
 
 int cb_learner_view(const cb_net* net, int which, const void** dev_ptr, size_t* count) {
   if (!net || !dev_ptr || !count || net->last_prec < 0) { set_error("no learner step has run on this net"); return CB_EINVAL; }
   const Workspace& ws = net->ws[net->last_prec]; int A = net->arch.n_actions;
-  int flag = 0;
-  CB_CUDA(cudaMemcpy(&flag, ws.errflag, sizeof flag, cudaMemcpyDeviceToHost));
-  if (flag) { set_error("a tcgen05 pipeline wait timed out inside the last learner step"); return CB_ECUDA; }
   switch (which) {
-    case 0: *dev_ptr = net->last_ppo ? (const void*)ws.values : (const void*)ws.act[net->head_t]; *count = (size_t)net->last_F * (A + 1); break;
+    case 0: if (!net->last_has_head) { set_error("view 0: the last call ran no forward over all (T+1)B frames (PPO with behaviour_values, or IMPALA env groups)"); return CB_EINVAL; }
+            *dev_ptr = net->last_ppo ? (const void*)ws.values : (const void*)ws.act[net->head_t]; *count = (size_t)net->last_F * (A + 1); break;
     case 1: *dev_ptr = ws.t0; *count = net->last_N; break;
     case 2: *dev_ptr = ws.t1; *count = net->last_N; break;
     case 3: *dev_ptr = ws.gradbuf; *count = net->P; break;
@@ -482,6 +585,11 @@ int cb_permutation(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* st
   int rc = launch_permutation(seed, epoch, 1, N, perm, jb, (cudaStream_t)stream);
   cudaFreeAsync(jb, (cudaStream_t)stream);
   return rc;
+}
+int cb_permutation_ws(uint64_t seed, uint32_t epoch, int N, int32_t* perm, uint32_t* scratch, void* stream) {
+  if (N < 0 || !perm || (!scratch && N > 0)) { set_error("bad argument"); return CB_EINVAL; }
+  if (N == 0) return CB_OK;
+  return launch_permutation(seed, epoch, 1, N, perm, scratch, (cudaStream_t)stream);
 }
 int cb_clip_rmsprop(size_t P, float* params, float* nu, const float* grad, float lr, float decay, float eps, float max_norm, float* grad_norm,
                     void* scratch, void* stream) {

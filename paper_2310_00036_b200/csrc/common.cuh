@@ -79,7 +79,8 @@ struct Workspace {     // one per precision mode
   bf16* w0img = nullptr;                                           // first-layer forward B image (conv0_tc.cu)
   bf16* wtc_f = nullptr; bf16* wtc_d = nullptr;                     // tcgen05 B-operand packs (forward / dgrad), bf16 mode only
   PackDesc* packtab = nullptr;                                     // device copy of the layer table for packing
-  int* errflag = nullptr;                                          // set by a kernel whose tcgen05 pipeline timed out
+  int* errflag = nullptr;                                          // device word, set by a kernel whose tcgen05 pipeline timed out
+  int* errhost = nullptr;                                          // mapped pinned host word: set by the step's last kernel when errflag is
   float* partial = nullptr; size_t partial_elems = 0;             // wgrad split-K partials
   float* partial_tc = nullptr; size_t partial_tc_elems = 0;       // one slot per tensor-core 3x3 layer: their reductions run as ONE launch after the backward pass
   float* gradbuf = nullptr;          // [P]
@@ -111,11 +112,19 @@ struct cb_net {
   struct PT { std::string name; size_t off; int rank; int dims[4]; int fan_in; };
   std::vector<PT> ptensors;
   cb::Workspace ws[2];
-  int last_prec = -1; int last_F = 0, last_N = 0; bool last_ppo = false;
+  int last_prec = -1; int last_F = 0, last_N = 0; bool last_ppo = false; bool last_has_head = true;
+  // context of a learner call in progress (cb_learner_begin .. last cb_learner_apply)
+  struct LearnCtx {
+    bool active = false; int n_updates = 0, next_grad = 0, next_apply = 0;
+    float *params = nullptr, *adam_m = nullptr, *adam_v = nullptr; uint64_t* opt_step = nullptr;
+    const uint8_t* obs = nullptr; const int32_t* actions = nullptr; const float* rewards = nullptr; const uint8_t* dones = nullptr;
+    float* stats = nullptr; cb_hparams hp; int mb = 1; bool ppo = false;
+  } lc;
   // actor side: the trunk of cb_policy_forward replayed as a CUDA graph per (precision, B, obs pointer); see api.cu
   struct FwdGraph { int prec, B; const uint8_t* obs; cudaGraphExec_t exec; uint64_t launches; bool bad; };
   std::vector<FwdGraph> fwd_graphs;
   cudaStream_t capture_stream = nullptr;
+  cudaStream_t aux_stream = nullptr; cudaEvent_t ev_fork = nullptr, ev_join = nullptr;      // side stream of the learner (PPO permutations)
 };
 
 namespace cb {
@@ -126,7 +135,7 @@ int cuda_fail(cudaError_t e, const char* what);
 
 // prof.cu -- launch counter and per-class event timing
 enum KClass { K_PACK = 0, K_CONV_FWD, K_POOL_FWD, K_CONV_DGRAD, K_CONV_WGRAD, K_WGRAD_REDUCE, K_POOL_BWD, K_HEAD_MISC, K_LOGPROB,
-              K_SCAN, K_LOSS, K_STATS, K_PERM, K_SQNORM, K_ADAM, K_SAMPLE, K_COUNT };
+              K_SCAN, K_LOSS, K_STATS, K_PERM, K_SQNORM, K_ADAM, K_SAMPLE, K_ENV, K_COUNT };
 bool prof_active();                    // cb_profile_begin .. cb_profile_end
 void prof_add_launches(uint64_t n);    // launches replayed by a CUDA graph
 struct ProfScope {      // counts `n` launches of class `cls`; records an event pair around them when profiling
@@ -181,7 +190,8 @@ int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* 
 int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset,
                   int32_t* actions, cudaStream_t st);
 int launch_heads_sample(int prec, const void* hid, const void* wf, const float* bias, int B, int fc, int A, uint64_t seed, uint64_t step,
-                        uint32_t env_offset, float* head, float* logits, float* value, int32_t* actions, cudaStream_t st);
+                        uint32_t env_offset, float* head, float* logits, float* value, int32_t* actions, cudaStream_t st,
+                        const int* errflag = nullptr, int* errhost = nullptr);
 int launch_split_head(const float* head, int F, int A, float* logits, float* value, cudaStream_t st);
 int launch_logprob(const float* logits, int ld, int N, int A, const int32_t* actions, const int32_t* idx,
                    float* logp_a, float* entropy, cudaStream_t st);
@@ -191,6 +201,13 @@ int launch_vtrace(int T, int B, const float* V, int ldV, const float* r, const u
 int launch_gae(int T, int B, const float* V, int ldV, const float* r, const uint8_t* d, float gamma, float lam,
                float* adv, float* ret, cudaStream_t st);
 int launch_permutation(uint64_t seed, uint32_t epoch0, int n_epochs, int N, int32_t* perm, uint32_t* jbuf, cudaStream_t st);
+int launch_sum_ranks(const float* in, int G, size_t n, float scale, float* out, cudaStream_t st);
+// env.cu
+int launch_env_reset(uint64_t seed, int B, int C, int H, int W, int32_t* state, uint8_t* obs, cudaStream_t st);
+int launch_env_step(uint64_t seed, int B, int C, int H, int W, uint32_t g, const int32_t* actions, int32_t* state, const uint8_t* obs_in, uint8_t* out0,
+                    uint8_t* out1, float* rewards, uint8_t* dones, cudaStream_t st);
+// one opt-in per (device, kernel): cudaFuncAttributeMaxDynamicSharedMemorySize raised to at least `bytes`
+int ensure_dyn_smem(const void* func, size_t bytes);
 // loss kernels write dhead [N, A+1] in the mode's storage type and per-sample terms; reduce writes stats
 int launch_impala_loss(int prec, int N, int A, const float* head, const int32_t* act, const float* vs, const float* pgadv,
                        const float* rho, float c1, float c2, int reduction, void* dhead, float* terms, double* red,
@@ -199,11 +216,12 @@ int launch_ppo_loss(int prec, int m, int A, const float* head, const int32_t* id
                     const float* ret, const float* logp_old, float eps, float c1, float c2, int norm_adv, void* dhead,
                     float* terms, double* red, float* advstat, float* stats, cudaStream_t st);
 int launch_clip_rmsprop(size_t P, float* params, float* nu, const float* g, float lr, float decay, float eps, float max_norm, float* grad_norm,
-                        float* stats_slot, void* scratch, cudaStream_t st);
+                        float* stats_slot, void* scratch, cudaStream_t st, const int* errflag = nullptr, int* errhost = nullptr);
 int launch_gather_traj(int T, int B, int b0, int Bm, const int32_t* act, const float* rew, const uint8_t* dones, const float* logmu, int32_t* fidx,
                        int32_t* act_m, float* rew_m, uint8_t* dones_m, float* logmu_m, cudaStream_t st);
 size_t clip_adam_scratch_bytes(size_t P);
 int launch_clip_adam(size_t P, float* params, float* m, float* v, const float* g, uint64_t k, float lr, float b1, float b2,
-                     float eps, float max_norm, float* grad_norm, float* stats_slot, void* scratch, cudaStream_t st);
+                     float eps, float max_norm, float* grad_norm, float* stats_slot, void* scratch, cudaStream_t st,
+                     const int* errflag = nullptr, int* errhost = nullptr);
 
 }  // namespace cb

@@ -440,10 +440,7 @@ int launch_conv0_pack(const Geom& g, const ParamMap& pm, const float* params, bf
 }
 
 template <class K>
-static int set_smem(K kernel, size_t smem, size_t* configured) {
-  if (smem > *configured) { CB_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); *configured = smem; }
-  return CB_OK;
-}
+static int set_smem(K kernel, size_t smem, size_t*) { return ensure_dyn_smem((const void*)kernel, smem); }
 
 int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* frame_idx, const bf16* wimg, const float* bias, bf16* out,
                      bf16* pool_out, uint8_t* pool_arg, int* error_flag, cudaStream_t st) {

@@ -531,11 +531,7 @@ static TcPlan tc_plan(int H, int W, int cin, int cout) {
 
 template <int CIN, int COUT, int MODE>
 static int launch_one(const tc::ConvTcArgs& a, const CUtensorMap& tmap, size_t smem, int ngroups, cudaStream_t st) {
-  static size_t configured = 0;      // largest dynamic size this instantiation has been opted in for
-  if (smem > configured) {
-    CB_CUDA(cudaFuncSetAttribute(tc::conv3x3_tc_kernel<CIN, COUT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
-  }
+  { int rc = ensure_dyn_smem((const void*)tc::conv3x3_tc_kernel<CIN, COUT, MODE>, smem); if (rc) return rc; }
   int grid = std::min(ngroups, 3 * 148);
   tc::conv3x3_tc_kernel<CIN, COUT, MODE><<<grid, tc::NT, smem, st>>>(a, tmap);
   CB_CUDA(cudaGetLastError());
@@ -590,11 +586,7 @@ bool conv_tc_fits(int H, int W, int cin, int cout) { return pipe_plan(148, H, W,
 
 template <int CIN, int COUT, int MODE>
 static int launch_pipe(const tc::PipeArgs& a, const CUtensorMap& tmap, size_t smem, int nitems, cudaStream_t st) {
-  static size_t configured = 0;
-  if (smem > configured) {
-    CB_CUDA(cudaFuncSetAttribute(tc::conv3x3_tc_pipe_kernel<CIN, COUT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
-  }
+  { int rc = ensure_dyn_smem((const void*)tc::conv3x3_tc_pipe_kernel<CIN, COUT, MODE>, smem); if (rc) return rc; }
   tc::conv3x3_tc_pipe_kernel<CIN, COUT, MODE><<<std::min(nitems, 148), tc::PIPE_THREADS, smem, st>>>(a, tmap);
   CB_CUDA(cudaGetLastError());
   return CB_OK;

@@ -220,8 +220,7 @@ static int launch_d(const dn::Args& a, dim3 grid, cudaStream_t st) {
   if (a.ksplit > 1) grid.z = a.ksplit;
   constexpr size_t PA = (MODE != 1 ? 128 : dn::BK) * 16 + 16;
   constexpr size_t smem = dn::NSTAGE * ((MODE != 1 ? dn::BK / 8 : 16) * PA + (MODE == 2 ? (dn::BK / 8) * (BN * 16 + 16) : (BN / 8) * dn::PB));
-  static bool configured = false;
-  if (!configured) { CB_CUDA(cudaFuncSetAttribute(dn::dense_tc_kernel<MODE, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); configured = true; }
+  { int rc = ensure_dyn_smem((const void*)dn::dense_tc_kernel<MODE, BN>, smem); if (rc) return rc; }
   dn::dense_tc_kernel<MODE, BN><<<grid, dn::NLOAD + 32, smem, st>>>(a);
   CB_CUDA(cudaGetLastError());
   return CB_OK;

@@ -411,8 +411,7 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         int RB = (int)std::min<size_t>((size_t)op.H, std::max<size_t>(2, (size_t)(40 * 1024) / row_bytes));
         const int nb = (op.H + RB - 1) / RB; RB = (op.H + nb - 1) / nb;
         const size_t smem = (size_t)RB * row_bytes;
-        static size_t configured = 48 * 1024;
-        if (smem > configured) { CB_CUDA(cudaFuncSetAttribute(pool_bwd_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); configured = smem; }
+        if (smem > 48 * 1024) { int rc = ensure_dyn_smem((const void*)pool_bwd_scatter_kernel, smem); if (rc) return rc; }
         pool_bwd_scatter_kernel<<<std::min(F * nb, 148 * 8), 256, smem, st>>>((const uint8_t*)ws.act[op.mask_t], (const bf16*)ws.grad[op.dy], (bf16*)ws.grad[op.dx],
                                                                              F, op.C, op.H, op.W, RB, nb);
       } else

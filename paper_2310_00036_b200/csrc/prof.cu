@@ -9,7 +9,7 @@
 namespace cb {
 
 static const char* kNames[K_COUNT] = {"pack_weights", "conv_fwd", "pool_fwd", "conv_dgrad", "conv_wgrad", "wgrad_reduce", "pool_bwd", "head_misc",
-                                      "logprob", "scan", "loss", "stats", "permutation", "sqnorm", "adam", "sample"};
+                                      "logprob", "scan", "loss", "stats", "permutation", "sqnorm", "adam", "sample", "env_step"};
 static std::atomic<uint64_t> g_launches{0};
 static std::mutex g_mu;
 static bool g_on = false; static int g_only = -1;

@@ -84,10 +84,20 @@ int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint
 template <typename AT>
 __global__ void heads_sample_kernel(const AT* __restrict__ hid, const AT* __restrict__ wf, const float* __restrict__ bias, int B, int fc, int A,
                                     uint32_t k0, uint32_t k1, uint32_t step_lo, uint32_t step_hi, uint32_t env_offset,
-                                    float* __restrict__ head, float* __restrict__ logits, float* __restrict__ value, int32_t* __restrict__ actions) {
+                                    float* __restrict__ head, float* __restrict__ logits, float* __restrict__ value, int32_t* __restrict__ actions,
+                                    const int* __restrict__ errflag, int* errhost) {
   const int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (b >= B) return;
   const int N = A + 1;
+  if (errflag && *errflag) {      // a tcgen05 pipeline of the trunk timed out: poison the outputs, tell the host (cleanba.h, asynchronous errors)
+    if (lane < N) {
+      if (head) head[(size_t)b * N + lane] = NAN;
+      if (lane < A) { if (logits) logits[(size_t)b * A + lane] = NAN; } else if (value) value[b] = NAN;
+    }
+    if (lane == 0 && actions) actions[b] = -1;
+    if (b == 0 && lane == 0 && errhost) *errhost = *errflag;
+    return;
+  }
   float acc[MAX_A];
 #pragma unroll
   for (int n = 0; n < MAX_A; ++n) acc[n] = 0.f;
@@ -132,17 +142,18 @@ __global__ void heads_sample_kernel(const AT* __restrict__ hid, const AT* __rest
 }
 
 int launch_heads_sample(int prec, const void* hid, const void* wf, const float* bias, int B, int fc, int A, uint64_t seed, uint64_t step,
-                        uint32_t env_offset, float* head, float* logits, float* value, int32_t* actions, cudaStream_t st) {
+                        uint32_t env_offset, float* head, float* logits, float* value, int32_t* actions, cudaStream_t st,
+                        const int* errflag, int* errhost) {
   if (B <= 0) return CB_OK;
   if (A + 1 > MAX_A) { set_error("n_actions too large"); return CB_EINVAL; }
   ProfScope ps(K_SAMPLE, st);
   const int grid = (B * 32 + 127) / 128;
   if (prec == CB_PREC_FP32_REF)
     heads_sample_kernel<float><<<grid, 128, 0, st>>>((const float*)hid, (const float*)wf, bias, B, fc, A, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step,
-                                                      (uint32_t)(step >> 32), env_offset, head, logits, value, actions);
+                                                      (uint32_t)(step >> 32), env_offset, head, logits, value, actions, errflag, errhost);
   else
     heads_sample_kernel<bf16><<<grid, 128, 0, st>>>((const bf16*)hid, (const bf16*)wf, bias, B, fc, A, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step,
-                                                     (uint32_t)(step >> 32), env_offset, head, logits, value, actions);
+                                                     (uint32_t)(step >> 32), env_offset, head, logits, value, actions, errflag, errhost);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
@@ -191,7 +202,7 @@ __global__ void logprob_kernel(const float* __restrict__ logits, int ld, int N, 
   if (n >= N) return;
   double lp[MAX_A], H;
   log_softmax<double>(logits + (size_t)n * ld, A, lp, &H);
-  int a = actions[idx ? idx[n] : n];
+  int a = min(max(actions[idx ? idx[n] : n], 0), A - 1);      // never index out of bounds with a bad action (cleanba.h)
   if (logp_a) logp_a[n] = (float)lp[a];
   if (entropy) entropy[n] = (float)H;
 }
@@ -267,7 +278,11 @@ int launch_gae(int T, int B, const float* V, int ldV, const float* r, const uint
 // perm_seed; for i = N-1 .. 1: j = (x_q * (i+1)) >> 32, swap(perm[i], perm[j]).  The draws are
 // computed in parallel, the swaps (inherently serial) by one thread; one block per epoch.
 // ------------------------------------------------------------------------------------------------
+// SMEM: the index array lives in shared memory during the swap loop (one dependent shared-memory round trip per swap
+// instead of an L2 round trip); N * 4 bytes must fit the opt-in limit, otherwise the loop runs on the global array.
+template <bool SMEM>
 __global__ void permutation_kernel(uint32_t k0, uint32_t k1, uint32_t epoch0, int N, int32_t* __restrict__ perm_all, uint32_t* __restrict__ j_all) {
+  extern __shared__ int32_t sperm[];
   uint32_t epoch = epoch0 + blockIdx.x;
   int32_t* perm = perm_all + (size_t)blockIdx.x * N;
   uint32_t* jb = j_all + (size_t)blockIdx.x * N;
@@ -278,18 +293,64 @@ __global__ void permutation_kernel(uint32_t k0, uint32_t k1, uint32_t epoch0, in
       if (i >= 1) jb[q] = (uint32_t)(((uint64_t)r[w] * (uint64_t)(i + 1)) >> 32);
     }
   }
-  for (int i = threadIdx.x; i < N; i += blockDim.x) perm[i] = i;
+  int32_t* wk = SMEM ? sperm : perm;
+  for (int i = threadIdx.x; i < N; i += blockDim.x) wk[i] = i;
   __syncthreads();
   if (threadIdx.x == 0) {
-    for (int i = N - 1, q = 0; i >= 1; --i, ++q) {
-      uint32_t j = jb[q]; int32_t a = perm[i], b = perm[j]; perm[i] = b; perm[j] = a;
+    int i = N - 1, q = 0;
+    for (; i >= 8; i -= 8, q += 8) {      // the eight draws of a pass are fetched together; the swaps stay in order
+      uint32_t j[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) j[u] = jb[q + u];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) { int32_t a = wk[i - u], b = wk[j[u]]; wk[i - u] = b; wk[j[u]] = a; }
     }
+    for (; i >= 1; --i, ++q) { uint32_t j = jb[q]; int32_t a = wk[i], b = wk[j]; wk[i] = b; wk[j] = a; }
+  }
+  if (SMEM) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < N; i += blockDim.x) perm[i] = sperm[i];
   }
 }
 int launch_permutation(uint64_t seed, uint32_t epoch0, int n_epochs, int N, int32_t* perm, uint32_t* jbuf, cudaStream_t st) {
   if (N <= 0 || n_epochs <= 0) return CB_OK;
   ProfScope ps(K_PERM, st);
-  permutation_kernel<<<n_epochs, 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), epoch0, N, perm, jbuf);
+  const size_t smem = (size_t)N * 4;
+  if (smem <= 200 * 1024) {
+    if (smem > 48 * 1024) { int rc = ensure_dyn_smem((const void*)permutation_kernel<true>, smem); if (rc) return rc; }
+    permutation_kernel<true><<<n_epochs, 256, smem, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), epoch0, N, perm, jbuf);
+  } else
+    permutation_kernel<false><<<n_epochs, 256, 0, st>>>((uint32_t)seed, (uint32_t)(seed >> 32), epoch0, N, perm, jbuf);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
+}
+
+// fixed-order sum over ranks (cb_sum_ranks): out[i] = scale * (in[0][i] + ... + in[G-1][i]), added in rank order
+template <bool VEC>      // VEC: n % 4 == 0 and 16-byte aligned buffers, so that every rank's slice can be read as float4
+__global__ void __launch_bounds__(256) sum_ranks_kernel(const float* __restrict__ in, int G, size_t n, float scale, float* __restrict__ out) {
+  if (VEC) {
+    const size_t nv = n / 4;
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nv; i += (size_t)gridDim.x * blockDim.x) {
+      float4 s = reinterpret_cast<const float4*>(in)[i];
+      for (int r = 1; r < G; ++r) { const float4 x = reinterpret_cast<const float4*>(in + (size_t)r * n)[i]; s.x += x.x; s.y += x.y; s.z += x.z; s.w += x.w; }
+      s.x *= scale; s.y *= scale; s.z *= scale; s.w *= scale;
+      reinterpret_cast<float4*>(out)[i] = s;
+    }
+  } else {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+      float s = in[i];
+      for (int r = 1; r < G; ++r) s += in[(size_t)r * n + i];
+      out[i] = s * scale;
+    }
+  }
+}
+int launch_sum_ranks(const float* in, int G, size_t n, float scale, float* out, cudaStream_t st) {
+  if (n == 0 || G <= 0) return CB_OK;
+  ProfScope ps(K_HEAD_MISC, st, 1, 0.0, (double)n * 4 * (G + 1));
+  const bool vec = (n & 3) == 0 && (((uintptr_t)in | (uintptr_t)out) & 15) == 0;
+  int grid = (int)std::min<size_t>(((vec ? n / 4 : n) + 255) / 256, (size_t)148 * 8); if (grid < 1) grid = 1;
+  if (vec) sum_ranks_kernel<true><<<grid, 256, 0, st>>>(in, G, n, scale, out);
+  else sum_ranks_kernel<false><<<grid, 256, 0, st>>>(in, G, n, scale, out);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
@@ -319,7 +380,7 @@ __global__ void impala_loss_kernel(int N, int A, const float* __restrict__ head,
   const float* l = head + (size_t)n * (A + 1);
   R lp[MAX_A], H;
   log_softmax<R>(l, A, lp, &H);
-  int a = act[n];
+  int a = min(max(act[n], 0), A - 1);
   R pg = (R)pgadv[n], err = (R)vs[n] - (R)l[A];
   for (int i = 0; i < A; ++i) {
     R p = rexp<R>(lp[i]);
@@ -392,7 +453,7 @@ __global__ void ppo_loss_kernel(int m, int A, const float* __restrict__ head, co
   const float* l = head + (size_t)n * (A + 1);
   R lp[MAX_A], H;
   log_softmax<R>(l, A, lp, &H);
-  int a = act[src];
+  int a = min(max(act[src], 0), A - 1);
   R inv = (R)(1.0 / (double)m);
   R At = norm_adv ? (R)(((double)adv[src] - red[0]) / (red[1] + 1e-8)) : (R)adv[src];
   R logr = lp[a] - (R)logp_old[src], r = rexp<R>(logr);
@@ -451,12 +512,20 @@ __global__ void __launch_bounds__(256) sqnorm_partial_kernel(size_t P, const flo
   if (threadIdx.x == 0) partial[blockIdx.x] = s;
 }
 
-__global__ void __launch_bounds__(256) sqnorm_final_kernel(int nparts, const double* __restrict__ partial, double* __restrict__ norm_out, float* __restrict__ gn0, float* __restrict__ gn1) {
+// gn1 = slot 4 of the update's stats record (or NULL).  errflag set (a tcgen05 pipeline timed out somewhere in this step): the
+// norm becomes NaN, which makes the optimizer kernel skip the update, the record's loss and grad norm read NaN, and the host
+// word is raised (cleanba.h, asynchronous errors).
+__global__ void __launch_bounds__(256) sqnorm_final_kernel(int nparts, const double* __restrict__ partial, double* __restrict__ norm_out, float* __restrict__ gn0, float* __restrict__ gn1,
+                                                           const int* __restrict__ errflag, int* errhost) {
   __shared__ double sh[256];
   double v = 0.0;
   for (int i = threadIdx.x; i < nparts; i += 256) v += partial[i];
   double s = block_sum<256>(v, sh);
-  if (threadIdx.x == 0) { double n = sqrt(s); *norm_out = n; if (gn0) *gn0 = (float)n; if (gn1) *gn1 = (float)n; }
+  if (threadIdx.x == 0) {
+    double n = sqrt(s);
+    if (errflag && *errflag) { n = (double)NAN; if (gn1) gn1[-4] = NAN; if (errhost) *errhost = *errflag; }
+    *norm_out = n; if (gn0) *gn0 = (float)n; if (gn1) *gn1 = (float)n;
+  }
 }
 
 __device__ __forceinline__ void adam_one(float& th, float& m, float& v, float g, float scale, float b1, float omb1, float b2, float omb2,
@@ -471,6 +540,7 @@ __global__ void __launch_bounds__(256) adam_kernel(size_t P, float* __restrict__
                                                    const double* __restrict__ norm, float max_norm, float b1, float omb1, float b2, float omb2, float ibc1,
                                                    float ibc2, float lr, float eps) {
   double n = *norm;
+  if (n != n) return;      // poisoned step: leave params and optimizer state untouched
   float scale = (float)((double)max_norm / fmax(n, (double)max_norm));
   size_t nv = P / 4;
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nv; i += (size_t)gridDim.x * blockDim.x) {
@@ -488,29 +558,41 @@ __global__ void __launch_bounds__(256) adam_kernel(size_t P, float* __restrict__
   }
 }
 
-// A22: RMSprop with eps inside the root; nu_0 = 0
+// A22: RMSprop with eps inside the root; nu_0 = 0.  16-byte loads and stores like adam_kernel.
+__device__ __forceinline__ void rms_one(float& th, float& nu, float g, float scale, float decay, float omd, float lr, float eps) {
+  const float gi = g * scale;
+  nu = fmaf(decay, nu, omd * gi * gi);
+  th -= lr * gi / sqrtf(nu + eps);
+}
 __global__ void __launch_bounds__(256) rmsprop_kernel(size_t P, float* __restrict__ th, float* __restrict__ nu, const float* __restrict__ g,
                                                       const double* __restrict__ norm, float max_norm, float decay, float omd, float lr, float eps) {
   const double n = *norm;
+  if (n != n) return;      // poisoned step
   const float scale = (float)((double)max_norm / fmax(n, (double)max_norm));
-  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < P; i += (size_t)gridDim.x * blockDim.x) {
-    const float gi = g[i] * scale;
-    const float ni = fmaf(decay, nu[i], omd * gi * gi);
-    nu[i] = ni;
-    th[i] -= lr * gi / sqrtf(ni + eps);
+  const size_t nv = P / 4;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < nv; i += (size_t)gridDim.x * blockDim.x) {
+    float4 t4 = reinterpret_cast<float4*>(th)[i], n4 = reinterpret_cast<float4*>(nu)[i];
+    const float4 g4 = reinterpret_cast<const float4*>(g)[i];
+    rms_one(t4.x, n4.x, g4.x, scale, decay, omd, lr, eps); rms_one(t4.y, n4.y, g4.y, scale, decay, omd, lr, eps);
+    rms_one(t4.z, n4.z, g4.z, scale, decay, omd, lr, eps); rms_one(t4.w, n4.w, g4.w, scale, decay, omd, lr, eps);
+    reinterpret_cast<float4*>(th)[i] = t4; reinterpret_cast<float4*>(nu)[i] = n4;
+  }
+  if (blockIdx.x == 0 && threadIdx.x < (P & 3)) {
+    const size_t i = nv * 4 + threadIdx.x;
+    rms_one(th[i], nu[i], g[i], scale, decay, omd, lr, eps);
   }
 }
 
 int launch_clip_rmsprop(size_t P, float* params, float* nu, const float* g, float lr, float decay, float eps, float max_norm, float* grad_norm,
-                        float* stats_slot, void* scratch, cudaStream_t st) {
+                        float* stats_slot, void* scratch, cudaStream_t st, const int* errflag, int* errhost) {
   if (P == 0) return CB_OK;
   int nparts = (int)((P + NORM_CHUNK - 1) / NORM_CHUNK);
   double* partial = (double*)scratch + 1; double* norm = (double*)scratch;
   { ProfScope ps(K_SQNORM, st, 2, 0.0, (double)P * 4);
   sqnorm_partial_kernel<<<nparts, 256, 0, st>>>(P, g, partial);
-  sqnorm_final_kernel<<<1, 256, 0, st>>>(nparts, partial, norm, grad_norm, stats_slot); }
+  sqnorm_final_kernel<<<1, 256, 0, st>>>(nparts, partial, norm, grad_norm, stats_slot, errflag, errhost); }
   ProfScope ps(K_ADAM, st, 1, 0.0, (double)P * 20);
-  int grid = (int)std::min<size_t>((P + 255) / 256, (size_t)148 * 8);
+  int grid = (int)std::min<size_t>((P / 4 + 255) / 256, (size_t)148 * 8); if (grid < 1) grid = 1;
   rmsprop_kernel<<<grid, 256, 0, st>>>(P, params, nu, g, norm, max_norm, decay, (float)(1.0 - (double)decay), lr, eps);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -538,13 +620,13 @@ int launch_gather_traj(int T, int B, int b0, int Bm, const int32_t* act, const f
 size_t clip_adam_scratch_bytes(size_t P) { return (((P + NORM_CHUNK - 1) / NORM_CHUNK) + 2) * sizeof(double); }
 
 int launch_clip_adam(size_t P, float* params, float* m, float* v, const float* g, uint64_t k, float lr, float b1, float b2, float eps,
-                     float max_norm, float* grad_norm, float* stats_slot, void* scratch, cudaStream_t st) {
+                     float max_norm, float* grad_norm, float* stats_slot, void* scratch, cudaStream_t st, const int* errflag, int* errhost) {
   if (P == 0) return CB_OK;
   int nparts = (int)((P + NORM_CHUNK - 1) / NORM_CHUNK);
   double* partial = (double*)scratch + 1; double* norm = (double*)scratch;
   { ProfScope ps(K_SQNORM, st, 2, 0.0, (double)P * 4);
   sqnorm_partial_kernel<<<nparts, 256, 0, st>>>(P, g, partial);
-  sqnorm_final_kernel<<<1, 256, 0, st>>>(nparts, partial, norm, grad_norm, stats_slot); }
+  sqnorm_final_kernel<<<1, 256, 0, st>>>(nparts, partial, norm, grad_norm, stats_slot, errflag, errhost); }
   double bc1 = 1.0 - pow((double)b1, (double)k), bc2 = 1.0 - pow((double)b2, (double)k);
   int grid = (int)std::min<size_t>((P / 4 + 255) / 256, (size_t)148 * 8); if (grid < 1) grid = 1;
   ProfScope ps(K_ADAM, st, 1, 0.0, (double)P * 28);

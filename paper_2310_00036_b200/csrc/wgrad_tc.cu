@@ -582,11 +582,7 @@ static WPlan wgrad_plan(int H, int W, int cin, int cout) {
 
 template <int CIN, int COUT>
 static int launch_w(const tcw::WgradTcArgs& a, const CUtensorMap& xmap, const CUtensorMap& ymap, size_t smem, int grid, cudaStream_t st) {
-  static size_t configured = 0;
-  if (smem > configured) {
-    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
-  }
+  { int rc = ensure_dyn_smem((const void*)tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true>, smem); if (rc) return rc; }
   tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true><<<grid, tcw::NLOAD + 64, smem, st>>>(a, xmap, ymap);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
@@ -628,11 +624,7 @@ static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
 
 template <int CIN, int COUT>
 static int launch_sw(const tcw::WgradSwArgs& a, const CUtensorMap& xmap, const CUtensorMap& ymap, size_t smem, int grid, cudaStream_t st) {
-  static size_t configured = 0;
-  if (smem > configured) {
-    CB_CUDA(cudaFuncSetAttribute(tcw::wgrad3x3_sw_kernel<CIN, COUT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    configured = smem;
-  }
+  { int rc = ensure_dyn_smem((const void*)tcw::wgrad3x3_sw_kernel<CIN, COUT>, smem); if (rc) return rc; }
   tcw::wgrad3x3_sw_kernel<CIN, COUT><<<grid, tcw::NLOAD + 64, smem, st>>>(a, xmap, ymap);
   CB_CUDA(cudaGetLastError());
   return CB_OK;

@@ -170,3 +170,94 @@ def gen_learner_batch(cfg_index, arch=None, T=None, B=None, forward_fn=None, see
         pol = None if forward_fn is None else forward_fn(obs[:T].reshape(T * B, arch.in_c, arch.in_h, arch.in_w))
     bl, actions = gen_behaviour(T, B, arch.n_actions, seed + 2, pol)
     return dict(obs=obs, actions=actions, rewards=rewards, dones=dones, behaviour_logits=bl)
+
+
+# ---- a seeded synthetic ENVIRONMENT (stand-in for EnvPool Atari) -------------------------------------------
+# Used by the actor/learner pipeline: `E.step(a_t) -> s_next, r_t, d_next` (Alg. 1 l.9) has to exist on the device so
+# that a rollout never leaves it.  This numpy class is the DEFINITION; csrc/env.cu restates it and is tested bit for bit against it.
+# Integer arithmetic only (uint32 wrap-around hashes, integer pyramids instead of Gaussians), so "bit for bit" is well defined.
+# The world: NB pyramid-shaped blobs on an H x W grey frame.  Blob 0 is the agent's (moved by the action: a % 3 - 1 and (a / 3) % 3 - 1 are
+# its x / y direction, actions 0-8 move 2 px, the others 1 px); blobs 1.. drift and bounce.  Touching blob 1 (L1 distance <= 8) pays +1 and
+# re-spawns it; touching blob 2 (L1 distance <= 5) pays -1 and ends the episode; an episode also ends with probability 1/64 per step.
+# Observations are the last C rendered frames (all C equal after a reset), plus hashed noise in {0..15}: the format of PAPER.md:166.
+ENV_NB = 4
+ENV_NS = 6 * ENV_NB + 1          # per blob: cx, cy, vx, vy, amp, R; then the episode counter
+
+
+def mix32(x):
+    """32-bit integer mixer (multiply-xorshift); x: uint32 array."""
+    x = np.asarray(x, dtype=np.uint64) & 0xFFFFFFFF
+    x ^= x >> 16; x = (x * 0x7FEB352D) & 0xFFFFFFFF
+    x ^= x >> 15; x = (x * 0x846CA68B) & 0xFFFFFFFF
+    x ^= x >> 16
+    return x
+
+
+def env_hash(seed, a, b, c):
+    """h(seed, a, b, c) = mix(s ^ mix(a ^ mix(b ^ mix(c)))), s = mix(seed_lo) ^ seed_hi; all uint32, broadcast."""
+    s = int(mix32(np.uint64(seed & 0xFFFFFFFF))) ^ ((seed >> 32) & 0xFFFFFFFF)
+    a = np.asarray(a, np.uint64) & 0xFFFFFFFF; b = np.asarray(b, np.uint64) & 0xFFFFFFFF; c = np.asarray(c, np.uint64) & 0xFFFFFFFF
+    return mix32(np.uint64(s) ^ mix32(a ^ mix32(b ^ mix32(c))))
+
+
+class BlobEnv:
+    """B independent environments.  reset() -> obs uint8 [B,C,H,W]; step(actions int [B], g) -> (obs, reward f32 [B], done u8 [B]) where g
+    is the global step counter of the caller (it keys every random draw, so a trajectory is a pure function of (seed, actions))."""
+
+    def __init__(self, B, seed, arch=IMPALA):
+        self.B, self.seed, self.C, self.H, self.W = B, seed, arch.in_c, arch.in_h, arch.in_w
+        self.state = np.zeros((B, ENV_NS), np.int64)
+        self.obs = np.zeros((B, self.C, self.H, self.W), np.uint8)
+
+    def _spawn(self, envs, key):
+        """(Re)draw every blob of the listed envs from h(seed, env, key, 8k + field)."""
+        e = np.asarray(envs, np.int64)
+        for k in range(ENV_NB):
+            hh = [env_hash(self.seed, e, key, 8 * k + f).astype(np.int64) for f in range(6)]
+            s = self.state
+            s[e, 6 * k + 0] = hh[0] % self.W; s[e, 6 * k + 1] = hh[1] % self.H
+            s[e, 6 * k + 2] = hh[2] % 5 - 2; s[e, 6 * k + 3] = hh[3] % 5 - 2
+            s[e, 6 * k + 4] = 40 + hh[4] % 161; s[e, 6 * k + 5] = 6 + hh[5] % 15
+
+    def _render(self, g):
+        B, H, W = self.B, self.H, self.W
+        y = np.arange(H, dtype=np.int64)[None, :, None]; x = np.arange(W, dtype=np.int64)[None, None, :]
+        img = np.zeros((B, H, W), np.int64)
+        for k in range(ENV_NB):
+            cx, cy, amp, R = (self.state[:, 6 * k + f][:, None, None] for f in (0, 1, 4, 5))
+            img += amp * np.maximum(0, R - np.abs(x - cx)) * np.maximum(0, R - np.abs(y - cy)) // (R * R)
+        e = np.arange(B, dtype=np.int64)[:, None, None]
+        img += (env_hash(self.seed, e, g, 1000 + y * W + x) & 15).astype(np.int64)
+        return np.minimum(img, 255).astype(np.uint8)
+
+    def reset(self):
+        self.state[:] = 0
+        self._spawn(np.arange(self.B), 0xFFFFFFFF)
+        self.obs[:] = self._render(0xFFFFFFFF)[:, None]
+        return self.obs.copy()
+
+    def step(self, actions, g):
+        s = self.state; B, H, W = self.B, self.H, self.W
+        a = np.asarray(actions, np.int64); e = np.arange(B, dtype=np.int64)
+        speed = np.where(a < 9, 2, 1)
+        s[:, 0] = np.clip(s[:, 0] + (a % 3 - 1) * speed, 0, W - 1); s[:, 1] = np.clip(s[:, 1] + ((a // 3) % 3 - 1) * speed, 0, H - 1)
+        for k in range(1, ENV_NB):
+            for ax, lim in ((0, W), (1, H)):
+                p = s[:, 6 * k + ax] + s[:, 6 * k + 2 + ax]
+                out = (p < 0) | (p >= lim)
+                s[:, 6 * k + 2 + ax] = np.where(out, -s[:, 6 * k + 2 + ax], s[:, 6 * k + 2 + ax])
+                s[:, 6 * k + ax] = np.clip(p, 0, lim - 1)
+        d1 = np.abs(s[:, 0] - s[:, 6]) + np.abs(s[:, 1] - s[:, 7]); d2 = np.abs(s[:, 0] - s[:, 12]) + np.abs(s[:, 1] - s[:, 13])
+        catch = d1 <= 8; hit = d2 <= 5
+        s[:, 6] = np.where(catch, env_hash(self.seed, e, g, 100).astype(np.int64) % W, s[:, 6])
+        s[:, 7] = np.where(catch, env_hash(self.seed, e, g, 101).astype(np.int64) % H, s[:, 7])
+        reward = np.where(hit, -1.0, np.where(catch, 1.0, 0.0)).astype(np.float32)
+        done = hit | (env_hash(self.seed, e, g, 102) % 64 == 0)
+        if done.any():
+            de = np.nonzero(done)[0]
+            s[de, ENV_NS - 1] += 1
+            self._spawn(de, (np.uint64(g) * np.uint64(2654435761) + s[de, ENV_NS - 1].astype(np.uint64)) & np.uint64(0xFFFFFFFF))
+        frame = self._render(g)
+        self.obs[:, :-1] = self.obs[:, 1:]; self.obs[:, -1] = frame
+        self.obs[done] = frame[done][:, None]
+        return self.obs.copy(), reward, done.astype(np.uint8)

@@ -80,7 +80,8 @@ def test_bad_arguments_are_errors_not_crashes():
     net = binding.Net(synth.NATURE)
     assert lib.cb_param_layout(net._h, 999, None, None, None, None) == -1
     assert lib.cb_policy_forward(net._h, None, None, 4, 0, 0, 0, 0, None, None, None, None) == -1
-    assert lib.cb_learner_step(net._h, None, None, None, None, None, None, None, None, None, None, None, None) == -1
+    assert lib.cb_learner_step(net._h, None, None, None, None, None, None, None, None, None, None, None, None, None) == -1
+    assert lib.cb_learner_grad(net._h, 0, None, None) == -1 and lib.cb_learner_apply(net._h, 0, None) == -1      # no cb_learner_begin
     with pytest.raises(binding.CleanbaError):
         binding.Net(synth.ArchSpec("nature", (32, 64, 64), 512, 18, 4, 20, 20))
 

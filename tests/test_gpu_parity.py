@@ -42,7 +42,7 @@ def test_sampling_ties_and_dominant_logit():
     assert len(np.unique(a0)) == 18
 
 
-@pytest.mark.parametrize("N", [1, 2, 3, 5, 256, 1000, 8192])
+@pytest.mark.parametrize("N", [1, 2, 3, 5, 8, 9, 10, 256, 1000, 8192, 12289, 51201, 60001])      # <= 12288: 48 KB shared; <= 51200: opt-in shared; above: global
 def test_permutation_bit_exact(N):
     for seed, epoch in [(1, 0), (1, 3), (2 ** 63 + 11, 7)]:
         got = host(binding.permutation(seed, epoch, N))
