@@ -184,6 +184,18 @@ int cb_vtrace(int T, int B, const float* V, const float* r, const uint8_t* d, co
 /* O6 GAE (A3): -> adv, ret [T,B]. */
 int cb_gae(int T, int B, const float* V, const float* r, const uint8_t* d, float gamma, float lambda_,
            float* adv, float* ret, void* stream);
+/* O5 / O7: the loss of one update with its adjoint seeds (a8).  head: dev fp32 [N, A+1] (A logits, then the value); dhead: dev
+ * [N, A+1] in the precision mode's storage type (fp32 / bf16) = dL/dlogits, dL/dV; stats: dev fp32 [CB_N_STATS] (slot 4, the
+ * gradient norm, is left 0); scratch: dev, >= cb_loss_scratch_bytes(N) bytes.  IMPALA (A4-A6): vs, pgadv, rho [N] from cb_vtrace.
+ * PPO (Eq. 2-3; A5-A8): sample n of the minibatch is row idx[n] (idx NULL: n) of actions / adv / ret / logp_old
+ * while head row n is the minibatch's own forward; norm_adv = per-minibatch advantage normalisation. */
+size_t cb_loss_scratch_bytes(int N);
+int cb_impala_loss(int N, int A, const float* head, const int32_t* actions, const float* vs, const float* pgadv, const float* rho,
+                   float vf_coef, float ent_coef, int loss_reduction, int precision, void* dhead, float* stats, void* scratch,
+                   void* stream);
+int cb_ppo_loss(int m, int A, const float* head, const int32_t* idx, const int32_t* actions, const float* adv, const float* ret,
+                const float* logp_old, float clip_eps, float vf_coef, float ent_coef, int norm_adv, int precision, void* dhead,
+                float* stats, void* scratch, void* stream);
 /* A17: Fisher-Yates permutation of N indices for (seed, epoch) -> perm int32 [N]. */
 int cb_permutation(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* stream);
 /* The same with caller-provided scratch (dev uint32 [N]), so that no allocation happens inside the call. */

@@ -23,7 +23,8 @@ EXPORTS = ["cb_net_create", "cb_net_destroy", "cb_param_count", "cb_param_layout
            "cb_learner_begin", "cb_learner_grad", "cb_learner_apply", "cb_sum_ranks", "cb_check_errors",
            "cb_debug_inject_timeout", "cb_permutation_ws",
            "cb_pipeline_create", "cb_pipeline_destroy", "cb_pipeline_run", "cb_pipeline_wait", "cb_pipeline_state", "cb_pipeline_records",
-           "cb_pipeline_rollout", "cb_pipeline_policy_version", "cb_env_state_ints", "cb_env_reset", "cb_env_step"]
+           "cb_pipeline_rollout", "cb_pipeline_policy_version", "cb_env_state_ints", "cb_env_reset", "cb_env_step",
+           "cb_loss_scratch_bytes", "cb_impala_loss", "cb_ppo_loss"]
 
 
 class CArch(C.Structure):
@@ -69,6 +70,7 @@ def lib():
         L.cb_pipeline_destroy.restype = None
         L.cb_pipeline_destroy.argtypes = [C.c_void_p]
         L.cb_env_state_ints.restype = C.c_size_t
+        L.cb_loss_scratch_bytes.restype = C.c_size_t
         _lib = L
     return _lib
 
@@ -386,6 +388,34 @@ def gae(V, r, d, gamma=0.99, lam=0.95):
     adv = torch.empty_like(r); ret = torch.empty_like(r)
     _check(lib().cb_gae(C.c_int(T), C.c_int(B), _ptr(V), _ptr(r), _ptr(d), C.c_float(gamma), C.c_float(lam), _ptr(adv), _ptr(ret), _stream()))
     return adv, ret
+
+
+def _loss_out(head, precision):
+    torch = _torch(); _dev(head, torch.float32, "head")
+    bf = PREC.get(precision, precision) == 1
+    dhead = torch.empty(head.shape, dtype=torch.bfloat16 if bf else torch.float32, device=head.device)
+    stats = torch.zeros((N_STATS,), dtype=torch.float32, device=head.device)
+    scratch = torch.empty((int(lib().cb_loss_scratch_bytes(C.c_int(head.shape[0]))) + 7) // 8, dtype=torch.float64, device=head.device)
+    return dhead, stats, scratch
+
+
+def impala_loss(head, actions, vs, pgadv, rho, vf_coef=0.5, ent_coef=0.01, loss_reduction=0, precision="fp32", out=None):
+    """cb_impala_loss: head cuda fp32 [N, A+1] -> (dhead [N, A+1] in the mode's storage type, stats [8])."""
+    dhead, stats, scratch = out if out is not None else _loss_out(head, precision)
+    N, A1 = head.shape
+    _check(lib().cb_impala_loss(C.c_int(N), C.c_int(A1 - 1), _ptr(head), _ptr(actions), _ptr(vs), _ptr(pgadv), _ptr(rho), C.c_float(vf_coef), C.c_float(ent_coef),
+                                C.c_int(loss_reduction), C.c_int(PREC.get(precision, precision)), _ptr(dhead), _ptr(stats), _ptr(scratch), _stream()))
+    return dhead, stats
+
+
+def ppo_loss(head, idx, actions, adv, ret, logp_old, clip_eps=0.1, vf_coef=0.5, ent_coef=0.01, norm_adv=1, precision="fp32", out=None):
+    """cb_ppo_loss: head cuda fp32 [m, A+1] (the minibatch's forward), idx int32 [m] or None -> (dhead, stats [8])."""
+    dhead, stats, scratch = out if out is not None else _loss_out(head, precision)
+    m, A1 = head.shape
+    _check(lib().cb_ppo_loss(C.c_int(m), C.c_int(A1 - 1), _ptr(head), _ptr(idx), _ptr(actions), _ptr(adv), _ptr(ret), _ptr(logp_old), C.c_float(clip_eps),
+                             C.c_float(vf_coef), C.c_float(ent_coef), C.c_int(norm_adv), C.c_int(PREC.get(precision, precision)), _ptr(dhead), _ptr(stats),
+                             _ptr(scratch), _stream()))
+    return dhead, stats
 
 
 def permutation(seed, epoch, N):

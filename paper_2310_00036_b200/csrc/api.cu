@@ -577,6 +577,23 @@ int cb_gae(int T, int B, const float* V, const float* r, const uint8_t* d, float
   if (!V || !r || !d || !adv || !ret) { set_error("null argument"); return CB_EINVAL; }
   return launch_gae(T, B, V, 1, r, d, gamma, lambda_, adv, ret, (cudaStream_t)stream);
 }
+size_t cb_loss_scratch_bytes(int N) { return (size_t)(N < 0 ? 0 : N) * 5 * 4 + 128; }
+int cb_impala_loss(int N, int A, const float* head, const int32_t* actions, const float* vs, const float* pgadv, const float* rho, float vf_coef,
+                   float ent_coef, int loss_reduction, int precision, void* dhead, float* stats, void* scratch, void* stream) {
+  if (N < 0 || A < 1 || A > 31 || check_prec(precision)) { set_error("bad argument"); return CB_EINVAL; }
+  if (N == 0) return CB_OK;
+  if (!head || !actions || !vs || !pgadv || !dhead || !stats || !scratch || misaligned(scratch, 16)) { set_error("null or misaligned argument"); return CB_EINVAL; }
+  double* red = (double*)scratch; float* terms = (float*)((char*)scratch + 128);
+  return launch_impala_loss(precision, N, A, head, actions, vs, pgadv, rho, vf_coef, ent_coef, loss_reduction, dhead, terms, red, stats, (cudaStream_t)stream);
+}
+int cb_ppo_loss(int m, int A, const float* head, const int32_t* idx, const int32_t* actions, const float* adv, const float* ret, const float* logp_old,
+                float clip_eps, float vf_coef, float ent_coef, int norm_adv, int precision, void* dhead, float* stats, void* scratch, void* stream) {
+  if (m < 0 || A < 1 || A > 31 || check_prec(precision)) { set_error("bad argument"); return CB_EINVAL; }
+  if (m == 0) return CB_OK;
+  if (!head || !actions || !adv || !ret || !logp_old || !dhead || !stats || !scratch || misaligned(scratch, 16)) { set_error("null or misaligned argument"); return CB_EINVAL; }
+  double* red = (double*)scratch; float* terms = (float*)((char*)scratch + 128);
+  return launch_ppo_loss(precision, m, A, head, idx, actions, adv, ret, logp_old, clip_eps, vf_coef, ent_coef, norm_adv, dhead, terms, red, nullptr, stats, (cudaStream_t)stream);
+}
 int cb_permutation(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* stream) {
   if (N < 0 || !perm) { set_error("bad argument"); return CB_EINVAL; }
   if (N == 0) return CB_OK;

@@ -124,3 +124,55 @@ def test_clip_adam_lr0_leaves_params_bit_identical():
     th = g.standard_normal(P).astype(np.float32); dth = dev(th)
     binding.clip_adam(dth, dev(np.zeros(P, np.float32)), dev(np.zeros(P, np.float32)), dev(g.standard_normal(P).astype(np.float32)), 1, 0.0)
     assert host(dth).tobytes() == th.tobytes()
+
+
+# ---------------------------------------------------------------------------------------------------
+# losses with their adjoint seeds (a8), element by element: O5 (A4-A6) and O7 (Eq. 2-3, A5-A8)
+# ---------------------------------------------------------------------------------------------------
+def _loss_inputs(N, A, seed):
+    g = synth.rng(seed)
+    head = np.concatenate([g.standard_normal((N, A)) * 2.0, g.standard_normal((N, 1))], axis=1).astype(np.float32)
+    act = g.integers(0, A, N).astype(np.int32)
+    return g, head, act
+
+
+@pytest.mark.parametrize("N,A", [(2560, 18), (1, 18), (131, 6), (20480, 18)])
+@pytest.mark.parametrize("prec,red", [("fp32", 0), ("fp32", 1), ("bf16", 0)])
+def test_impala_loss_seeds_parity(N, A, prec, red):
+    g, head, act = _loss_inputs(N, A, N + A)
+    vs = g.standard_normal(N).astype(np.float32); pg = g.standard_normal(N).astype(np.float32); rho = g.random(N).astype(np.float32)
+    dhead, stats = binding.impala_loss(dev(head), dev(act), dev(vs), dev(pg), dev(rho), 0.5, 0.01, red, prec)
+    st, dl, dV = oracle.impala_loss(head[:, :A], head[:, A], act, vs, pg, rho, 0.5, 0.01, red)
+    got = host(dhead.float()); ref = np.concatenate([dl, dV[:, None]], axis=1)
+    if prec == "fp32":
+        close(got, ref, 1e-5, what="impala seeds")
+    else:      # computed in fp32, stored as bf16: one rounding of relative size 2^-9
+        assert (np.abs(got - ref) <= 2.0 ** -8 * np.abs(ref) + 1e-4 * np.sqrt(np.mean(ref ** 2))).all()
+    gs = host(stats).astype(np.float64); scale = abs(st[1]) + abs(st[2]) + 1e-3
+    tol = 1e-6 if prec == "fp32" else 2e-5
+    for i in (0, 1, 2, 3, 7):
+        assert abs(gs[i] - st[i]) <= tol * (abs(st[i]) + scale), (oracle.STAT_NAMES[i], gs[i], st[i])
+
+
+@pytest.mark.parametrize("m,A,norm", [(2048, 18, 1), (2048, 18, 0), (3, 18, 1), (517, 6, 1)])
+@pytest.mark.parametrize("prec", ["fp32", "bf16"])
+def test_ppo_loss_seeds_parity(m, A, norm, prec):
+    g, head, act_m = _loss_inputs(m, A, m + A + norm)
+    N = 4 * m + 5                                                     # the minibatch gathers rows idx of the rollout arrays
+    idx = g.permutation(N)[:m].astype(np.int32)
+    act = g.integers(0, A, N).astype(np.int32); adv = g.standard_normal(N).astype(np.float32); ret = g.standard_normal(N).astype(np.float32)
+    lp, _ = oracle.log_softmax(head[:, :A].astype(np.float64))
+    lpo = np.zeros(N, np.float32); lpo[idx] = (lp[np.arange(m), act[idx]] + 0.15 * g.standard_normal(m)).astype(np.float32)      # ratios on both sides of the clip
+    dhead, stats = binding.ppo_loss(dev(head), dev(idx), dev(act), dev(adv), dev(ret), dev(lpo), 0.1, 0.5, 0.01, norm, prec)
+    st, dl, dV = oracle.ppo_loss(head[:, :A], head[:, A], act[idx], adv[idx], ret[idx], lpo[idx], 0.1, 0.5, 0.01, norm)
+    assert m < 100 or 0.05 < st[6] < 0.95                              # clipped and unclipped samples both present
+    got = host(dhead.float()); ref = np.concatenate([dl, dV[:, None]], axis=1)
+    if prec == "fp32":
+        close(got, ref, 1e-5, what="ppo seeds")
+    else:
+        # fp32 arithmetic: a ratio within 1e-6 of the clip boundary may fall on the other side (gradient switched off); none in this draw
+        assert (np.abs(got - ref) <= 2.0 ** -8 * np.abs(ref) + 1e-4 * np.sqrt(np.mean(ref ** 2))).all()
+    gs = host(stats).astype(np.float64); scale = abs(st[1]) + abs(st[2]) + 1e-3
+    tol = 1e-6 if prec == "fp32" else 2e-5
+    for i in (0, 1, 2, 3, 5, 6):
+        assert abs(gs[i] - st[i]) <= tol * (abs(st[i]) + scale) + (1e-6 if i == 5 else 0), (oracle.STAT_NAMES[i], gs[i], st[i])
