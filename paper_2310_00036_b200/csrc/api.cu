@@ -90,7 +90,11 @@ static int build_program(cb_net* net) {
     }
   }
   if (b.H < 1 || b.W < 1) { set_error("input too small for this architecture"); return CB_EINVAL; }
-  int fc = b.conv("fc", b.cur, a.fc, b.H, b.W, 1, 0, true, -1);
+  // the feature map is only ever consumed through a ReLU (by fc; its sign gates fc's dgrad all the same): the last conv stores relu(output)
+  // and fc loads it as is
+  net->layers.back().relu_out = true;
+  int fc = b.conv("fc", b.cur, a.fc, b.H, b.W, 1, 0, false, -1);
+  net->layers[fc].gate_in = true;
   net->hid_t = net->layers[fc].out_t;
   {  // the ABI reports fc.w as [out, in] with `in` flattened (C,H,W)
     cb_net::PT& t = net->ptensors[net->ptensors.size() - 2];
@@ -174,7 +178,8 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
       std::vector<PackDesc> tab;
       for (const Layer& L : net->layers)
         tab.push_back({L.g, L.pm, L.wf_off, L.bias_off, (prec == CB_PREC_BF16_TC && conv_tc_supported(L.g)) ? 1 : 0,
-                       (prec == CB_PREC_BF16_TC && L.u8_in && conv0_tc_supported(L.g)) ? 1 : 0});
+                       (prec == CB_PREC_BF16_TC && L.u8_in && conv0_tc_supported(L.g)) ? 1 : 0,
+                       (prec == CB_PREC_BF16_TC && !L.u8_in && !L.f32_out && !L.relu_in && dense_tc_supported(L.g)) ? 1 : 0});
       CB_ALLOC(ws.packtab, tab.size() * sizeof(PackDesc));
       CB_CUDA(cudaMemcpy(ws.packtab, tab.data(), tab.size() * sizeof(PackDesc), cudaMemcpyHostToDevice));
     }
@@ -194,7 +199,7 @@ int ensure_workspace(cb_net* net, int prec, int frames) {
     pe = std::max(pe, wgrad_partial_elems(L.g, frames));
     if (wgrad_tc_supported(L.g)) pe = std::max(pe, wgrad_tc_partial_elems(L.g));
     if (L.u8_in && conv0_tc_supported(L.g)) pe = std::max(pe, conv0_partial_elems(L.g));
-    if (dense_tc_supported(L.g)) pe = std::max(pe, (size_t)8 * std::min(frames, 1024) * L.g.Cout);
+    if (dense_tc_supported(L.g)) pe = std::max(pe, dense_partial_elems(L.g, frames));
   }
   CB_ALLOC(ws.partial, pe * 4); ws.partial_elems = pe;
   if (prec == CB_PREC_BF16_TC) {
@@ -215,7 +220,7 @@ int ensure_learner_scratch(cb_net* net, int prec, int F, int N, int epochs) {
   size_t n4 = (size_t)N * 4;
   CB_ALLOC(ws.logpi, n4); CB_ALLOC(ws.logmu, n4); CB_ALLOC(ws.ent, n4); CB_ALLOC(ws.t0, n4); CB_ALLOC(ws.t1, n4); CB_ALLOC(ws.rho, n4);
   CB_ALLOC(ws.values, (size_t)F * (net->arch.n_actions + 1) * 4);
-  CB_ALLOC(ws.terms, n4 * 5); CB_ALLOC(ws.red, 64); CB_ALLOC(ws.advstat, 16);
+  CB_ALLOC(ws.terms, 16); CB_ALLOC(ws.red, 256 + (size_t)((N + 127) / 128) * 40); CB_ALLOC(ws.advstat, 16);      // red: [0..1] advantage mean / std, [8..] per-block loss-term partials
   CB_ALLOC(ws.perm, std::max(n4 * epochs, (size_t)F * 4)); CB_ALLOC(ws.permj, n4 * epochs);
   CB_ALLOC(ws.act_m, n4); CB_ALLOC(ws.rew_m, n4); CB_ALLOC(ws.dones_m, (size_t)N); CB_ALLOC(ws.logmu_m, n4);
   ws.learn_frames = F; ws.learn_N = N; ws.learn_epochs = epochs;
@@ -577,13 +582,13 @@ int cb_gae(int T, int B, const float* V, const float* r, const uint8_t* d, float
   if (!V || !r || !d || !adv || !ret) { set_error("null argument"); return CB_EINVAL; }
   return launch_gae(T, B, V, 1, r, d, gamma, lambda_, adv, ret, (cudaStream_t)stream);
 }
-size_t cb_loss_scratch_bytes(int N) { return (size_t)(N < 0 ? 0 : N) * 5 * 4 + 128; }
+size_t cb_loss_scratch_bytes(int N) { return 256 + (size_t)(((N < 0 ? 0 : N) + 127) / 128) * 40; }
 int cb_impala_loss(int N, int A, const float* head, const int32_t* actions, const float* vs, const float* pgadv, const float* rho, float vf_coef,
                    float ent_coef, int loss_reduction, int precision, void* dhead, float* stats, void* scratch, void* stream) {
   if (N < 0 || A < 1 || A > 31 || check_prec(precision)) { set_error("bad argument"); return CB_EINVAL; }
   if (N == 0) return CB_OK;
   if (!head || !actions || !vs || !pgadv || !dhead || !stats || !scratch || misaligned(scratch, 16)) { set_error("null or misaligned argument"); return CB_EINVAL; }
-  double* red = (double*)scratch; float* terms = (float*)((char*)scratch + 128);
+  double* red = (double*)scratch; float* terms = nullptr;
   return launch_impala_loss(precision, N, A, head, actions, vs, pgadv, rho, vf_coef, ent_coef, loss_reduction, dhead, terms, red, stats, (cudaStream_t)stream);
 }
 int cb_ppo_loss(int m, int A, const float* head, const int32_t* idx, const int32_t* actions, const float* adv, const float* ret, const float* logp_old,
@@ -591,7 +596,7 @@ int cb_ppo_loss(int m, int A, const float* head, const int32_t* idx, const int32
   if (m < 0 || A < 1 || A > 31 || check_prec(precision)) { set_error("bad argument"); return CB_EINVAL; }
   if (m == 0) return CB_OK;
   if (!head || !actions || !adv || !ret || !logp_old || !dhead || !stats || !scratch || misaligned(scratch, 16)) { set_error("null or misaligned argument"); return CB_EINVAL; }
-  double* red = (double*)scratch; float* terms = (float*)((char*)scratch + 128);
+  double* red = (double*)scratch; float* terms = nullptr;
   return launch_ppo_loss(precision, m, A, head, idx, actions, adv, ret, logp_old, clip_eps, vf_coef, ent_coef, norm_adv, dhead, terms, red, nullptr, stats, (cudaStream_t)stream);
 }
 int cb_permutation(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* stream) {

@@ -66,7 +66,7 @@ struct Op {
 };
 
 // one entry per layer of the single-launch weight-packing kernel
-struct PackDesc { Geom g; ParamMap pm; size_t wf_off, bias_off; int tc, conv0; };
+struct PackDesc { Geom g; ParamMap pm; size_t wf_off, bias_off; int tc, conv0, dense; };
 
 struct Tensor { size_t per_frame; bool f32; int esize; };   // esize: bytes per element, 0 = the mode's storage type
 
@@ -86,8 +86,8 @@ struct Workspace {     // one per precision mode
   float* gradbuf = nullptr;          // [P]
   // learner scratch (fp32 unless noted)
   float *logpi = nullptr, *logmu = nullptr, *ent = nullptr, *t0 = nullptr, *t1 = nullptr, *rho = nullptr, *values = nullptr;
-  float* terms = nullptr;            // [5, N] per-sample loss terms
-  double* red = nullptr;             // reduction scratch
+  float* terms = nullptr;            // (unused since the loss kernels sum their terms per block)
+  double* red = nullptr;             // [0..1] advantage mean / std; [8..] per-block partial sums of the five loss terms
   float* advstat = nullptr;          // [2] mean, 1/(std+eps)
   int32_t* perm = nullptr;           // [epochs, N]  (IMPALA env groups: frame indices [(T+1) * B/mb])
   int32_t* act_m = nullptr; float* rew_m = nullptr; uint8_t* dones_m = nullptr; float* logmu_m = nullptr;   // env-group copies [T, B/mb]
@@ -182,9 +182,12 @@ int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* 
 
 // dense_tc.cu
 bool dense_tc_supported(const Geom& g);
-int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wf, const float* bias, bf16* out, bool relu_in, float* partial, int* error_flag, cudaStream_t st);
+size_t dense_partial_elems(const Geom& g, long long frames);
+// wt = weight pack [N][K] (K-major, k in (y, x, c) order), wf = the SIMT forward pack [K][N]; the feature map is read as stored (the layer's
+// relu_in must be false: its producer stores through the ReLU)
+int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wt, const float* bias, bf16* out, float* partial, int* error_flag, cudaStream_t st);
 int launch_dense_dgrad_tc(const Geom& g, int F, const bf16* dy, const bf16* wf, const bf16* mask, bf16* dx, int* error_flag, cudaStream_t st);
-int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* A, const bf16* dy, bool relu_in, float* grad, int* error_flag, cudaStream_t st);
+int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* A, const bf16* dy, float* grad, int* error_flag, cudaStream_t st);
 
 // rl.cu
 int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint64_t step, uint32_t env_offset,

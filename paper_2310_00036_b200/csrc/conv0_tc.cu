@@ -120,16 +120,16 @@ template <int COUT>
 __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr uint32_t W_BYTES = 6u * 2u * COUT * 16u;
-  constexpr int TILES_PER_BATCH = TMEM_COLS / COUT;
-  __shared__ __align__(8) uint64_t bar_storage;
+  constexpr int TILES_PER_BATCH = TMEM_COLS / COUT / 2;      // per accumulator half
+  __shared__ __align__(8) uint64_t bar_storage[2];
   __shared__ uint32_t tmem_base_smem;
   __shared__ __align__(16) float bias_s[32];
   const int tid = threadIdx.x, warp = tid >> 5, wg = warp >> 2, lane_row = tid & 127, Wp = a.W + 2;      // two warpgroups
   const uint32_t magic_Wp = (uint32_t)((0x100000000ull + (uint64_t)Wp - 1) / (uint64_t)Wp);      // q / Wp = umulhi(q, magic) for q * Wp < 2^32
   if (tid < COUT) bias_s[tid] = a.bias[tid];
   uint8_t* w_smem = smem; uint8_t* xs = smem + W_BYTES;
-  const uint32_t bar = smem_u32(&bar_storage);
-  if (tid == 0) mbar_init(bar, 1);
+  const uint32_t bar = smem_u32(&bar_storage[0]);
+  if (tid == 0) { mbar_init(bar, 1); mbar_init(bar + 8u, 1); }
   if (warp == 0) tmem_alloc(smem_u32(&tmem_base_smem), TMEM_COLS);
   for (uint32_t i = tid; i < W_BYTES / 16; i += 256) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w)[i];
   for (int i = tid; i < a.npix_alloc; i += 256) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
@@ -152,27 +152,35 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
     fence_async_smem();
     __syncthreads();
     const int ntiles = (a.R * Wp + 127) / 128;
-    for (int t0 = 0; t0 < ntiles; t0 += TILES_PER_BATCH) {
-      const int nt = min(TILES_PER_BATCH, ntiles - t0);
-      if (warp == 0) {        // the whole warp runs the loop, one elected lane issues
-        tc_fence_after();
-        const uint32_t a_lo = ((a_base >> 4) & 0x3FFFu) | (1u << 16), a_hi = 8u | (1u << 14);               // LBO 16 B, SBO 128 B
-        const uint32_t b_lo = ((b_base >> 4) & 0x3FFFu) | ((uint32_t)COUT << 16), b_hi = 8u | (1u << 14);   // LBO COUT*16 B, SBO 128 B
-        for (int s = 0; s < nt; ++s) {
-          const uint32_t q0 = (uint32_t)(t0 + s) * 128u;
+    const int nbatch = (ntiles + TILES_PER_BATCH - 1) / TILES_PER_BATCH;
+    // The accumulator is split into two halves of TILES_PER_BATCH tiles: the MMAs of batch k+1 are issued BEFORE batch k is drained, so the
+    // tensor core works underneath the epilogue (every operand of the band is already staged).  One mbarrier per half.
+    auto issue = [&](int bi) {        // warp 0, converged: one elected lane issues
+      const int t0 = bi * TILES_PER_BATCH, nt = min(TILES_PER_BATCH, ntiles - t0), half = bi & 1;
+      tc_fence_after();
+      const uint32_t a_lo = ((a_base >> 4) & 0x3FFFu) | (1u << 16), a_hi = 8u | (1u << 14);               // LBO 16 B, SBO 128 B
+      const uint32_t b_lo = ((b_base >> 4) & 0x3FFFu) | ((uint32_t)COUT << 16), b_hi = 8u | (1u << 14);   // LBO COUT*16 B, SBO 128 B
+      for (int s = 0; s < nt; ++s) {
+        const uint32_t q0 = (uint32_t)(t0 + s) * 128u;
 #pragma unroll
-          for (int slot = 0; slot < 6; ++slot) {
-            const uint32_t shift = (uint32_t)((slot >> 1) * Wp + (slot & 1) * 2);
-            const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(a_lo + q0 + shift);
-            const uint64_t bd = ((uint64_t)b_hi << 32) | (uint64_t)(b_lo + (uint32_t)slot * 2u * COUT);
-            if (elect_one()) mma_f16(tmem_base + (uint32_t)(s * COUT), ad, bd, idesc, slot ? 1u : 0u);
-          }
+        for (int slot = 0; slot < 6; ++slot) {
+          const uint32_t shift = (uint32_t)((slot >> 1) * Wp + (slot & 1) * 2);
+          const uint64_t ad = ((uint64_t)a_hi << 32) | (uint64_t)(a_lo + q0 + shift);
+          const uint64_t bd = ((uint64_t)b_hi << 32) | (uint64_t)(b_lo + (uint32_t)slot * 2u * COUT);
+          if (elect_one()) mma_f16(tmem_base + (uint32_t)((half * TILES_PER_BATCH + s) * COUT), ad, bd, idesc, slot ? 1u : 0u);
         }
-        if (elect_one()) mma_commit(bar);
-        __syncwarp();
       }
-      if (warp == 0 && !mbar_wait(bar, parity)) { if (a.error_flag) *a.error_flag = 3; }      // one warp polls; the rest sleep in the barrier
-      parity ^= 1;
+      if (elect_one()) mma_commit(bar + 8u * (uint32_t)half);
+      __syncwarp();
+    };
+    if (warp == 0) issue(0);
+    for (int bi = 0; bi < nbatch; ++bi) {
+      const int t0 = bi * TILES_PER_BATCH, nt = min(TILES_PER_BATCH, ntiles - t0), half = bi & 1;
+      if (warp == 0) {
+        if (bi + 1 < nbatch) issue(bi + 1);      // the other half was drained before the barrier that ended the previous iteration
+        if (!mbar_wait(bar + 8u * (uint32_t)half, (parity >> half) & 1u)) { if (a.error_flag) *a.error_flag = 3; }      // one warp polls; the rest sleep in the barrier
+      }
+      parity ^= 1u << half;
       __syncthreads();
       tc_fence_after();
       for (int s = wg; s < nt; s += 2) {      // each warpgroup drains every second accumulator tile
@@ -182,7 +190,7 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
 #pragma unroll
         for (int c0 = 0; c0 < COUT; c0 += 16) {
           float v[16];
-          tmem_ld16(tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(s * COUT + c0), v);
+          tmem_ld16(tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((half * TILES_PER_BATCH + s) * COUT + c0), v);
           if (!valid) continue;
           uint4 o0, o1;
           __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);

@@ -1,260 +1,292 @@
-// tcgen05 / TMEM GEMMs for the dense trunk (fc layer) in CB_PREC_BF16_TC:
-//   MODE 0  forward:  hid[f][n]  = sum_k relu(A[f][k]) * Wf[k][n] + b[n]        (M = frames,   contraction = features)
-//   MODE 1  wgrad:    dW[k][n]   = sum_f relu(A[f][k]) * dY[f][n]               (M = features, contraction = frames)
-//   MODE 2  dgrad:    dA[f][k]   = [A[f][k] > 0] sum_n dY[f][n] * Wf[k][n]      (M = frames,   contraction = outputs)
-// A is the NHWC-flattened feature map [F][K] (bf16), Wf the forward weight pack [K][N], dY [F][N].
-// Operands are staged by 8 loader warps as 16-byte units into padded planes so that they are canonical
-// no-swizzle UMMA layouts (rows of a core matrix 16 B apart): forward A is K-major (LBO = plane), every other
-// operand is MN-major (LBO = 128 B, SBO = plane).  4-stage mbarrier pipeline: loaders run ahead of the
-// single MMA-issuing thread; the fp32 accumulator [128 x BN] lives in TMEM; warps 0-3 drain it.
+// tcgen05 / TMEM GEMMs for the dense trunk (fc layer) in CB_PREC_BF16_TC, fed by TMA:
+//   MODE 0  forward:  hid[f][n]  = sum_k A[f][k] * Wt[n][k] + b[n]               (M = frames,   N = outputs,  contraction = features)
+//   MODE 2  dgrad:    dA[f][k]   = [A[f][k] > 0] sum_n dY[f][n] * Wf[k][n]       (M = frames,   N = features, contraction = outputs)
+//   wgrad:            dW[k][n]   = sum_f A[f][k] * dY[f][n]                      (M = features, N = outputs,  contraction = frames)
+// A is the NHWC-flattened feature map [F][K] (bf16; the producing layer stores it through its ReLU, api.cu), Wt / Wf the two weight
+// packs ([N][K] and [K][N]), dY [F][N].  Every operand tile is landed by 2-D `cp.async.bulk.tensor` boxes of 64 columns (128 bytes) in
+// the 128-byte swizzle pattern, i.e. directly in the canonical swizzled UMMA layout: K-major for MODE 0 / 2 (the contraction index is
+// the contiguous one in memory), MN-major for the weight gradient (frames are the rows of both operands; LBO = one 64-column block).
+// Out-of-range rows / columns of a box are zero-filled by the TMA unit, so ragged F and K need no special case.  A CTA owns a
+// [128 x 256] accumulator in TMEM; warp 0 produces (4-stage mbarrier ring), warp 1 issues the MMAs, warps 2-5 drain the accumulator.
+// MODE 0 splits the contraction over gridDim.z CTAs (a constant of the layer, never of F, so that a frame's result does not depend on
+// the batch it is in) and a second kernel adds the partials in split order, the bias, and rounds to bf16.
 #include "common.cuh"
 #include "tc_ptx.cuh"
+#include "tma.cuh"
 
 namespace cb {
 namespace dn {
 using namespace ptx;
 
 struct Args {
-  const bf16* A;      // MODE 0/1: features [F][K];  MODE 2: dY [F][N]
-  const bf16* B;      // MODE 0/2: Wf [K][N];  MODE 1: dY [F][N]
-  const bf16* mask;   // MODE 2: feature pre-activations [F][K] gating the result (nullable)
-  const float* bias;  // MODE 0
-  bf16* out;          // MODE 0: [F][N]
-  float* grad;        // MODE 1: canonical fp32 gradient buffer
-  int F, K, N, relu_in;
-  float* part; int ksplit;      // MODE 0 with ksplit > 1: fp32 partial sums [ksplit][F][N] instead of out
-  int H, W, C; size_t w_off;   // MODE 1: feature k = (y*W + x)*C + c  ->  canonical fc.w index n*K + (c*H + y)*W + x
+  const float* bias;  // MODE 0 (applied by the reduce kernel)
+  const bf16* mask;   // MODE 2: feature map [F][K] whose sign gates the result (nullable)
+  bf16* out;          // MODE 2: dA [F][K]
+  float* part;        // MODE 0: fp32 partial sums [ksplit][F][N]
+  float* grad;        // wgrad: canonical fp32 gradient buffer
+  int F, K, N;
+  int H, W, C; size_t w_off;   // wgrad: feature k = (y*W + x)*C + c  ->  canonical fc.w index n*K + (c*H + y)*W + x
   int* error_flag;
 };
 
-constexpr int NLOAD = 256, BK = 64, NSTAGE = 4;
-constexpr uint32_t PB = BK * 16 + 16;
+constexpr int BK = 64, NST = 4, BM = 128, BN = 256, NTHREADS = 6 * 32;
+constexpr uint32_t A_BYTES = BM * BK * 2, B_BYTES = BN * BK * 2, STAGE = A_BYTES + B_BYTES, SMEM = NST * STAGE + 1024;
+// MODE 2 contracts over the layer's outputs (4 tiles for fc = 256): two stages, so that two CTAs share an SM and overlap their load / MMA / drain phases
+constexpr int NST2 = 2; constexpr uint32_t SMEM2 = NST2 * STAGE + 1024;
+constexpr uint32_t BLK = 64 * 128;      // one box: 64 rows of 128 bytes
 
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n"
+               :: "r"(dst), "l"((uint64_t)map), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
-__device__ __forceinline__ uint4 relu8(uint4 v) {
-  __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
-  const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
-#pragma unroll
-  for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
-  return v;
+// SW128 descriptor: start address, LBO (bytes; MN-major: distance between 64-element blocks along M / N), SBO = 1024 B (8 rows of 128 B)
+__device__ __forceinline__ uint64_t sw128_desc(uint32_t saddr, uint32_t lbo_bytes) {
+  return (uint64_t)((saddr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) | ((uint64_t)(1024u >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
 }
 
-template <int MODE, int BN>
-__global__ void __launch_bounds__(NLOAD + 32) dense_tc_kernel(const Args a) {
-  extern __shared__ __align__(128) uint8_t smem[];
-  constexpr uint32_t PA = (MODE != 1 ? 128 : BK) * 16 + 16;
-  constexpr int APL = MODE != 1 ? BK / 8 : 16, BPL = MODE == 2 ? BK / 8 : BN / 8;
-  constexpr uint32_t PBK = BN * 16 + 16;                 // MODE 2: K-major B planes [contraction/8][BN rows][16 B]
-  constexpr uint32_t STAGE = APL * PA + BPL * (MODE == 2 ? PBK : PB);
-  constexpr uint32_t TCOLS = BN < 32 ? 32 : BN;
-  __shared__ __align__(8) uint64_t bars[2 * NSTAGE + 1];
+// MODE 0 / 2: both operands K-major.  amap: rows = frames, columns = contraction; bmap: rows = N index, columns = contraction.
+template <int MODE>
+__global__ void __launch_bounds__(NTHREADS) dense_kmajor_kernel(const Args a, const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap bmap) {
+  constexpr int NST = MODE == 2 ? NST2 : dn::NST;
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t bars[2 * NST + 1];
   __shared__ uint32_t tmem_base_smem;
   const int tid = threadIdx.x, warp = tid >> 5;
-  const uint32_t bar0 = smem_u32(&bars[0]);
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u, bar0 = smem_u32(&bars[0]);
   if (tid == 0) {
-    for (int i = 0; i < 2 * NSTAGE + 1; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
+    for (int i = 0; i < 2 * NST + 1; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    tma::prefetch_map(&amap); tma::prefetch_map(&bmap);
   }
-  if (warp == NLOAD / 32) tmem_alloc(smem_u32(&tmem_base_smem), TCOLS);
+  if (warp == 1) tmem_alloc(smem_u32(&tmem_base_smem), BN);
   tc_fence_before(); __syncthreads(); tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
-  const int m0 = blockIdx.x * 128, n0 = blockIdx.y * BN;
-  const int L = MODE == 0 ? a.K : (MODE == 1 ? a.F : a.N);      // contraction length
-  const int lda = MODE == 2 ? a.N : a.K;                         // row length of A
-  const int all_tiles = (L + BK - 1) / BK;
-  const int per_z = (all_tiles + (int)gridDim.z - 1) / (int)gridDim.z;
-  const int tbeg = (int)blockIdx.z * per_z, ntiles = max(0, min(all_tiles, tbeg + per_z) - tbeg);      // this CTA's k-tiles
-
-  if (warp < NLOAD / 32) {
+  const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+  const int L = MODE == 0 ? a.K : a.N;                                   // contraction length
+  const int all_tiles = (L + BK - 1) / BK, per_z = (all_tiles + (int)gridDim.z - 1) / (int)gridDim.z;
+  const int tbeg = (int)blockIdx.z * per_z, ntiles = max(0, min(all_tiles, tbeg + per_z) - tbeg);
+  if (warp == 0) {
+    // ================= TMA producer =================
     for (int t = 0; t < ntiles; ++t) {
-      const int s = t % NSTAGE, use = t / NSTAGE, l0 = (tbeg + t) * BK;
-      if (use > 0 && !mbar_wait(bar0 + 8u * (NSTAGE + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 5; }
-      uint8_t* as = smem + (size_t)s * STAGE; uint8_t* bs = as + APL * PA;
-      // ---- A tile ----
-      constexpr int AWORK = 128 * (BK / 8);               // 16-byte units (both modes: 128 x 64 elements)
+      const int s = t % NST, use = t / NST, l0 = (tbeg + t) * BK;
+      if (use > 0 && !mbar_wait(bar0 + 8u * (NST + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 5; }
+      if (elect_one()) {
+        const uint32_t dst = sbase + (uint32_t)s * STAGE, full = bar0 + 8u * s;
+        tma::arrive_expect_tx(full, STAGE);
+        tma_load_2d(dst, &amap, l0, m0, full); tma_load_2d(dst + BLK, &amap, l0, m0 + 64, full);
 #pragma unroll
-      for (int i0 = 0; i0 < AWORK; i0 += NLOAD) {
-        const int i = i0 + tid;
-        uint4 v = make_uint4(0, 0, 0, 0); uint32_t dst;
-        if (MODE != 1) {
-          const int row = i >> 3, j = i & 7, f = m0 + row, k = l0 + 8 * j;
-          dst = (uint32_t)j * PA + (uint32_t)row * 16u;
-          if (f < a.F && k < L) v = *reinterpret_cast<const uint4*>(a.A + (size_t)f * lda + k);
-        } else {
-          const int frow = i >> 4, g = i & 15, f = l0 + frow, k = m0 + 8 * g;
-          dst = (uint32_t)g * PA + (uint32_t)frow * 16u;
-          if (f < a.F && k < a.K) v = *reinterpret_cast<const uint4*>(a.A + (size_t)f * a.K + k);
-        }
-        if (MODE != 2 && a.relu_in) v = relu8(v);
-        *reinterpret_cast<uint4*>(as + dst) = v;
+        for (int j = 0; j < BN / 64; ++j) tma_load_2d(dst + A_BYTES + (uint32_t)j * BLK, &bmap, l0, n0 + 64 * j, full);
       }
-      if (MODE == 2) {
-        // ---- B tile (K-major): rows = outputs k = n0 .. n0+BN of Wf [K][N], contraction columns l0 .. l0+BK ----
-        for (int i = tid; i < BN * (BK / 8); i += NLOAD) {
-          const int row = i >> 3, j = i & 7, k = n0 + row, n = l0 + 8 * j;
-          uint4 v = make_uint4(0, 0, 0, 0);
-          if (k < a.K && n < a.N) v = *reinterpret_cast<const uint4*>(a.B + (size_t)k * a.N + n);
-          *reinterpret_cast<uint4*>(bs + (uint32_t)j * PBK + (uint32_t)row * 16u) = v;
-        }
-      }
-      // ---- B tile: BK rows of [rows][N] starting at row l0, columns n0 .. n0+BN ----
-      constexpr int BWORK = MODE == 2 ? 0 : BK * BPL;
-      for (int i = tid; i < BWORK; i += NLOAD) {
-        const int r = i / BPL, g = i - r * BPL, row = l0 + r, n = n0 + 8 * g;
-        uint4 v = make_uint4(0, 0, 0, 0);
-        if (row < L && n < a.N) v = *reinterpret_cast<const uint4*>(a.B + (size_t)row * a.N + n);
-        *reinterpret_cast<uint4*>(bs + (uint32_t)g * PB + (uint32_t)r * 16u) = v;
-      }
-      fence_async_smem();
-      asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
-      if (tid == 0) mbar_arrive(bar0 + 8u * s);
-    }
-    if (warp < 4) {
-      if (ntiles > 0 && !mbar_wait(bar0 + 8u * (2 * NSTAGE), 0u)) { if (a.error_flag) *a.error_flag = 5; }
-      tc_fence_after();
-      const int row = m0 + tid;
-#pragma unroll
-      for (int c0 = 0; c0 < BN; c0 += 16) {
-        float v[16];
-        tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)c0, v);
-        const int n = n0 + c0;
-        if (n >= (MODE == 2 ? a.K : a.N)) continue;
-        if (MODE == 2) {
-          if (row >= a.F) continue;
-          const size_t o = (size_t)row * a.K + n;
-          if (a.mask) {
-            uint4 s0 = *reinterpret_cast<const uint4*>(a.mask + o), s1 = *reinterpret_cast<const uint4*>(a.mask + o + 8);
-            const bf16* h0 = reinterpret_cast<const bf16*>(&s0); const bf16* h1 = reinterpret_cast<const bf16*>(&s1);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) { if (!(__bfloat162float(h0[i]) > 0.f)) v[i] = 0.f; if (!(__bfloat162float(h1[i]) > 0.f)) v[8 + i] = 0.f; }
-          }
-          uint4 o0, o1;
-          __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
-#pragma unroll
-          for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
-          *reinterpret_cast<uint4*>(a.out + o) = o0;
-          *reinterpret_cast<uint4*>(a.out + o + 8) = o1;
-        } else if (MODE == 0) {
-          if (row >= a.F) continue;
-          if (a.ksplit > 1) {
-#pragma unroll
-            for (int i = 0; i < 16; ++i) a.part[((size_t)blockIdx.z * a.F + row) * a.N + n + i] = ntiles > 0 ? v[i] : 0.f;
-            continue;
-          }
-#pragma unroll
-          for (int i = 0; i < 16; ++i) v[i] += a.bias[n + i];
-          uint4 o0, o1;
-          __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
-#pragma unroll
-          for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
-          *reinterpret_cast<uint4*>(a.out + (size_t)row * a.N + n) = o0;
-          *reinterpret_cast<uint4*>(a.out + (size_t)row * a.N + n + 8) = o1;
-        } else {
-          if (row >= a.K) continue;
-          const int c = row % a.C, pix = row / a.C, y = pix / a.W, x = pix - y * a.W;
-          const size_t kc = ((size_t)c * a.H + y) * a.W + x;
-#pragma unroll
-          for (int i = 0; i < 16; ++i) a.grad[a.w_off + (size_t)(n + i) * a.K + kc] = v[i];
-        }
-      }
-    }
-  } else {      // warp NLOAD / 32: the whole warp runs the loop, one elected lane issues
-    const uint32_t idesc = make_idesc(128, BN, MODE == 1 ? 1 : 0, MODE == 2 ? 0 : 1);
-    for (int t = 0; t < ntiles; ++t) {
-      const int s = t % NSTAGE, use = t / NSTAGE;
-      if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 5; }
-      tc_fence_after();
-      const uint32_t ab = smem_u32(smem + (size_t)s * STAGE), bb = ab + APL * PA;
-#pragma unroll
-      for (int ks = 0; ks < BK / 16; ++ks) {
-        const uint64_t ad = MODE != 1 ? make_desc(ab + (uint32_t)(2 * ks) * PA, PA, 128u) : make_desc(ab + (uint32_t)ks * 256u, 128u, PA);
-        const uint64_t bd = MODE == 2 ? make_desc(bb + (uint32_t)(2 * ks) * PBK, PBK, 128u) : make_desc(bb + (uint32_t)ks * 256u, 128u, PB);
-        if (elect_one()) mma_f16(tmem_base, ad, bd, idesc, (t | ks) ? 1u : 0u);
-      }
-      if (elect_one()) mma_commit(bar0 + 8u * (NSTAGE + s));
       __syncwarp();
     }
-    if (ntiles > 0 && elect_one()) mma_commit(bar0 + 8u * (2 * NSTAGE));
+  } else if (warp == 1) {
+    // ================= MMA issuer =================
+    const uint32_t idesc = make_idesc(BM, BN, 0, 0);
+    for (int t = 0; t < ntiles; ++t) {
+      const int s = t % NST, use = t / NST;
+      if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 5; }
+      tc_fence_after();
+      const uint32_t ab = sbase + (uint32_t)s * STAGE, bb = ab + A_BYTES;
+#pragma unroll
+      for (int ks = 0; ks < BK / 16; ++ks)      // 16 contraction elements = 32 bytes further along the swizzled 128-byte row
+        if (elect_one()) mma_f16(tmem_base, sw128_desc(ab + 32u * ks, 16u), sw128_desc(bb + 32u * ks, 16u), idesc, (t | ks) ? 1u : 0u);
+      if (elect_one()) mma_commit(bar0 + 8u * (NST + s));
+      __syncwarp();
+    }
+    if (ntiles > 0 && elect_one()) mma_commit(bar0 + 8u * (2 * NST));
     __syncwarp();
+  } else {
+    // ================= epilogue: warp w drains TMEM lanes 32 (w % 4) .. +31 =================
+    if (ntiles > 0 && !mbar_wait(bar0 + 8u * (2 * NST), 0u)) { if (a.error_flag) *a.error_flag = 5; }
+    tc_fence_after();
+    const int q = warp & 3, row = m0 + q * 32 + (tid & 31);
+#pragma unroll 2
+    for (int c0 = 0; c0 < BN; c0 += 16) {
+      float v[16];
+      tmem_ld16(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, v);
+      const int n = n0 + c0;
+      if (row >= a.F || n >= (MODE == 0 ? a.N : a.K)) continue;
+      if (MODE == 0) {
+        float4* dst = reinterpret_cast<float4*>(a.part + ((size_t)blockIdx.z * a.F + row) * a.N + n);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) dst[i] = ntiles > 0 ? make_float4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]) : make_float4(0.f, 0.f, 0.f, 0.f);
+      } else {
+        const size_t o = (size_t)row * a.K + n;
+        if (a.mask) {
+          const uint4 s0 = *reinterpret_cast<const uint4*>(a.mask + o), s1 = *reinterpret_cast<const uint4*>(a.mask + o + 8);
+          const bf16* h0 = reinterpret_cast<const bf16*>(&s0); const bf16* h1 = reinterpret_cast<const bf16*>(&s1);
+#pragma unroll
+          for (int i = 0; i < 8; ++i) { if (!(__bfloat162float(h0[i]) > 0.f)) v[i] = 0.f; if (!(__bfloat162float(h1[i]) > 0.f)) v[8 + i] = 0.f; }
+        }
+        uint4 o0, o1;
+        __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
+        *reinterpret_cast<uint4*>(a.out + o) = o0;
+        *reinterpret_cast<uint4*>(a.out + o + 8) = o1;
+      }
+    }
   }
   tc_fence_before(); __syncthreads();
-  if (warp == NLOAD / 32) tmem_dealloc(tmem_base, TCOLS);
+  if (warp == 1) tmem_dealloc(tmem_base, BN);
 }
 
-// out[f][n] = bf16(sum_z part[z][f][n] + bias[n]), z in order
-__global__ void dense_reduce_kernel(const float* __restrict__ part, int S, int F, int N, const float* __restrict__ bias, bf16* __restrict__ out) {
-  size_t total = (size_t)F * N;
-  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
-    float s = 0.f;
-    for (int z = 0; z < S; ++z) s += part[(size_t)z * total + i];
-    out[i] = __float2bfloat16_rn(s + bias[i % N]);
+// Weight gradient: both operands MN-major.  amap = feature map [F][K], bmap = dY [F][N]; a stage holds 64 frames (contraction rows) of
+// 128 feature columns (two boxes) and 256 output columns (four boxes).
+__global__ void __launch_bounds__(NTHREADS) dense_wgrad_kernel(const Args a, const __grid_constant__ CUtensorMap amap, const __grid_constant__ CUtensorMap bmap) {
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t bars[2 * NST + 1];
+  __shared__ uint32_t tmem_base_smem;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u, bar0 = smem_u32(&bars[0]);
+  if (tid == 0) {
+    for (int i = 0; i < 2 * NST + 1; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+    tma::prefetch_map(&amap); tma::prefetch_map(&bmap);
   }
-}
-
-// db[n] = sum_f dY[f][n]: 16 lanes per column, lane k sums frames [k*q, (k+1)*q) in order, then the 16 sums are added in
-// lane order (fixed association => reproducible)
-__global__ void colsum_kernel(const bf16* __restrict__ dy, int F, int N, float* __restrict__ out) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x, n = t >> 4, part = t & 15;
-  const int q = (F + 15) / 16, f0 = part * q, f1 = min(F, f0 + q);
-  float s = 0.f;
-  if (n < N) {
-#pragma unroll 8
-    for (int f = f0; f < f1; ++f) s += __bfloat162float(dy[(size_t)f * N + n]);
-  }
-  float tot = s;
+  if (warp == 1) tmem_alloc(smem_u32(&tmem_base_smem), BN);
+  tc_fence_before(); __syncthreads(); tc_fence_after();
+  const uint32_t tmem_base = tmem_base_smem;
+  const int m0 = blockIdx.x * BM, n0 = blockIdx.y * BN;
+  const int ntiles = (a.F + BK - 1) / BK;
+  if (warp == 0) {
+    for (int t = 0; t < ntiles; ++t) {
+      const int s = t % NST, use = t / NST, f0 = t * BK;
+      if (use > 0 && !mbar_wait(bar0 + 8u * (NST + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 5; }
+      if (elect_one()) {
+        const uint32_t dst = sbase + (uint32_t)s * STAGE, full = bar0 + 8u * s;
+        tma::arrive_expect_tx(full, STAGE);
+        tma_load_2d(dst, &amap, m0, f0, full); tma_load_2d(dst + BLK, &amap, m0 + 64, f0, full);
 #pragma unroll
-  for (int k = 1; k < 16; ++k) tot += __shfl_down_sync(0xffffffffu, s, k);
-  if (part == 0 && n < N) out[n] = tot;
+        for (int j = 0; j < BN / 64; ++j) tma_load_2d(dst + A_BYTES + (uint32_t)j * BLK, &bmap, n0 + 64 * j, f0, full);
+      }
+      __syncwarp();
+    }
+  } else if (warp == 1) {
+    const uint32_t idesc = make_idesc(BM, BN, 1, 1);
+    for (int t = 0; t < ntiles; ++t) {
+      const int s = t % NST, use = t / NST;
+      if (!mbar_wait(bar0 + 8u * s, (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 5; }
+      tc_fence_after();
+      const uint32_t ab = sbase + (uint32_t)s * STAGE, bb = ab + A_BYTES;
+#pragma unroll
+      for (int ks = 0; ks < BK / 16; ++ks)      // 16 contraction rows = 16 * 128 bytes further down every block
+        if (elect_one()) mma_f16(tmem_base, sw128_desc(ab + 2048u * ks, BLK), sw128_desc(bb + 2048u * ks, BLK), idesc, (t | ks) ? 1u : 0u);
+      if (elect_one()) mma_commit(bar0 + 8u * (NST + s));
+      __syncwarp();
+    }
+    if (ntiles > 0 && elect_one()) mma_commit(bar0 + 8u * (2 * NST));
+    __syncwarp();
+  } else {
+    if (ntiles > 0 && !mbar_wait(bar0 + 8u * (2 * NST), 0u)) { if (a.error_flag) *a.error_flag = 5; }
+    tc_fence_after();
+    const int q = warp & 3, row = m0 + q * 32 + (tid & 31);      // feature index k
+    const int c = row % a.C, pix = row / a.C, y = pix / a.W, x = pix - y * a.W;
+    const size_t kc = ((size_t)c * a.H + y) * a.W + x;
+#pragma unroll 2
+    for (int c0 = 0; c0 < BN; c0 += 16) {
+      float v[16];
+      tmem_ld16(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)c0, v);
+      const int n = n0 + c0;
+      if (row >= a.K || n >= a.N) continue;
+#pragma unroll
+      for (int i = 0; i < 16; ++i) a.grad[a.w_off + (size_t)(n + i) * a.K + kc] = ntiles > 0 ? v[i] : 0.f;
+    }
+  }
+  tc_fence_before(); __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, BN);
+}
+
+// out[f][n] = bf16(sum_z part[z][f][n] + bias[n]), z in order; four outputs per thread
+__global__ void __launch_bounds__(256) dense_reduce_kernel(const float* __restrict__ part, int S, int F, int N, const float* __restrict__ bias, bf16* __restrict__ out) {
+  const size_t total4 = (size_t)F * N / 4;
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < total4; i += (size_t)gridDim.x * blockDim.x) {
+    float4 s = reinterpret_cast<const float4*>(part)[i];
+    for (int z = 1; z < S; ++z) { const float4 p = reinterpret_cast<const float4*>(part)[(size_t)z * total4 + i]; s.x += p.x; s.y += p.y; s.z += p.z; s.w += p.w; }
+    const float4 b = *reinterpret_cast<const float4*>(bias + (int)((i * 4) % (size_t)N));
+    __nv_bfloat162 o[2] = {__floats2bfloat162_rn(s.x + b.x, s.y + b.y), __floats2bfloat162_rn(s.z + b.z, s.w + b.w)};
+    *reinterpret_cast<uint2*>(out + i * 4) = *reinterpret_cast<const uint2*>(o);
+  }
+}
+
+// db[n] = sum_f dY[f][n].  A block owns 8 columns (one 16-byte vector per frame): thread t sums frames t, t + 256, ... in order, then
+// the 256 thread sums of a column are added by a fixed shared-memory tree (fixed association => reproducible).
+__global__ void __launch_bounds__(256) colsum_kernel(const bf16* __restrict__ dy, int F, int N, float* __restrict__ out) {
+  __shared__ float sh[256][9];
+  const int n0 = blockIdx.x * 8;
+  float s[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  for (int f = threadIdx.x; f < F; f += 256) {
+    const uint4 v = *reinterpret_cast<const uint4*>(dy + (size_t)f * N + n0);
+    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&v);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { const float2 t = __bfloat1622float2(h[k]); s[2 * k] += t.x; s[2 * k + 1] += t.y; }
+  }
+#pragma unroll
+  for (int k = 0; k < 8; ++k) sh[threadIdx.x][k] = s[k];
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if ((int)threadIdx.x < w) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) sh[threadIdx.x][k] += sh[threadIdx.x + w][k];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x < 8) out[n0 + threadIdx.x] = sh[0][threadIdx.x];
 }
 
 }  // namespace dn
 
 bool dense_tc_supported(const Geom& g) {
-  return g.Ho == 1 && g.Wo == 1 && g.kh == g.H && g.kw == g.W && g.p == 0 && g.Cin % 8 == 0 && g.Cout % 64 == 0;
+  const int K = g.H * g.W * g.Cin;
+  return g.Ho == 1 && g.Wo == 1 && g.kh == g.H && g.kw == g.W && g.p == 0 && g.Cin % 8 == 0 && K % 16 == 0 && g.Cout % 64 == 0 && tma::encode_fn() != nullptr;
 }
 
-template <int MODE, int BN>
-static int launch_d(const dn::Args& a, dim3 grid, cudaStream_t st) {
-  if (a.ksplit > 1) grid.z = a.ksplit;
-  constexpr size_t PA = (MODE != 1 ? 128 : dn::BK) * 16 + 16;
-  constexpr size_t smem = dn::NSTAGE * ((MODE != 1 ? dn::BK / 8 : 16) * PA + (MODE == 2 ? (dn::BK / 8) * (BN * 16 + 16) : (BN / 8) * dn::PB));
-  { int rc = ensure_dyn_smem((const void*)dn::dense_tc_kernel<MODE, BN>, smem); if (rc) return rc; }
-  dn::dense_tc_kernel<MODE, BN><<<grid, dn::NLOAD + 32, smem, st>>>(a);
-  CB_CUDA(cudaGetLastError());
-  return CB_OK;
-}
+// the contraction of the forward GEMM is split over this many CTAs whatever the batch size (A16: a frame's hidden vector must not
+// depend on how many other frames are in the call)
+constexpr int DENSE_KSPLIT = 8;
+size_t dense_partial_elems(const Geom& g, long long frames) { return (size_t)DENSE_KSPLIT * (size_t)frames * g.Cout; }
 
-int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wf, const float* bias, bf16* out, bool relu_in, float* partial, int* error_flag, cudaStream_t st) {
+static bool map2d(CUtensorMap* m, const void* base, int rows, int cols) { return tma::make_2d_map(m, base, rows, cols, 64, 64); }
+
+int launch_dense_fwd_tc(const Geom& g, int F, const bf16* A, const bf16* wt, const float* bias, bf16* out, float* partial, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
   const int K = g.H * g.W * g.Cin, N = g.Cout;
-  const int ksplit = (F <= 1024 && partial) ? 8 : 1;      // few frames (actor side): split the contraction so that the grid fills the GPU
-  dn::Args a{A, wf, nullptr, bias, out, nullptr, F, K, N, relu_in ? 1 : 0, partial, ksplit, g.H, g.W, g.Cin, 0, error_flag};
-  int rc = launch_d<0, 32>(a, dim3((F + 127) / 128, (N + 31) / 32), st);
-  if (rc || ksplit == 1) return rc;
-  dn::dense_reduce_kernel<<<std::min((F * N + 255) / 256, 1184), 256, 0, st>>>(partial, ksplit, F, N, bias, out);
+  CUtensorMap am, bm;
+  if (!map2d(&am, A, F, K) || !map2d(&bm, wt, N, K)) { set_error("cuTensorMapEncodeTiled refused a dense-layer map"); return CB_ECUDA; }
+  dn::Args a{bias, nullptr, nullptr, partial, nullptr, F, K, N, g.H, g.W, g.Cin, 0, error_flag};
+  int rc = ensure_dyn_smem((const void*)dn::dense_kmajor_kernel<0>, dn::SMEM); if (rc) return rc;
+  dn::dense_kmajor_kernel<0><<<dim3((F + dn::BM - 1) / dn::BM, (N + dn::BN - 1) / dn::BN, DENSE_KSPLIT), dn::NTHREADS, dn::SMEM, st>>>(a, am, bm);
+  CB_CUDA(cudaGetLastError());
+  dn::dense_reduce_kernel<<<(int)std::min<size_t>(((size_t)F * N / 4 + 255) / 256, 148 * 8), 256, 0, st>>>(partial, DENSE_KSPLIT, F, N, bias, out);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
 
-int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* A, const bf16* dy, bool relu_in, float* grad, int* error_flag, cudaStream_t st) {
+int launch_dense_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* A, const bf16* dy, float* grad, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
   const int K = g.H * g.W * g.Cin, N = g.Cout;
-  dn::Args a{A, dy, nullptr, nullptr, nullptr, grad, F, K, N, relu_in ? 1 : 0, nullptr, 1, g.H, g.W, g.Cin, pm.w_off, error_flag};
-  int rc = launch_d<1, 64>(a, dim3((K + 127) / 128, (N + 63) / 64), st);
-  if (rc) return rc;
-  dn::colsum_kernel<<<(16 * N + 255) / 256, 256, 0, st>>>(dy, F, N, grad + pm.b_off);
+  CUtensorMap am, bm;
+  if (!map2d(&am, A, F, K) || !map2d(&bm, dy, F, N)) { set_error("cuTensorMapEncodeTiled refused a dense-layer map"); return CB_ECUDA; }
+  dn::Args a{nullptr, nullptr, nullptr, nullptr, grad, F, K, N, g.H, g.W, g.Cin, pm.w_off, error_flag};
+  int rc = ensure_dyn_smem((const void*)dn::dense_wgrad_kernel, dn::SMEM); if (rc) return rc;
+  dn::dense_wgrad_kernel<<<dim3((K + dn::BM - 1) / dn::BM, (N + dn::BN - 1) / dn::BN), dn::NTHREADS, dn::SMEM, st>>>(a, am, bm);
+  CB_CUDA(cudaGetLastError());
+  dn::colsum_kernel<<<N / 8, 256, 0, st>>>(dy, F, N, grad + pm.b_off);      // N % 64 == 0 (dense_tc_supported)
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
 
-// dgrad of the fc layer: dx [F][K] = gate(dY [F][N] . Wf^T), gated by the stored feature pre-activations
+// dgrad of the fc layer: dx [F][K] = gate(dY [F][N] . Wf^T), gated by the sign of the stored feature map
 int launch_dense_dgrad_tc(const Geom& g, int F, const bf16* dy, const bf16* wf, const bf16* mask, bf16* dx, int* error_flag, cudaStream_t st) {
   if (F <= 0) return CB_OK;
   const int K = g.H * g.W * g.Cin, N = g.Cout;
-  dn::Args a{dy, wf, mask, nullptr, dx, nullptr, F, K, N, 0, nullptr, 1, g.H, g.W, g.Cin, 0, error_flag};
-  return launch_d<2, 64>(a, dim3((F + 127) / 128, (K + 63) / 64), st);
+  CUtensorMap am, bm;
+  if (!map2d(&am, dy, F, N) || !map2d(&bm, wf, K, N)) { set_error("cuTensorMapEncodeTiled refused a dense-layer map"); return CB_ECUDA; }
+  dn::Args a{nullptr, mask, dx, nullptr, nullptr, F, K, N, g.H, g.W, g.Cin, 0, error_flag};
+  int rc = ensure_dyn_smem((const void*)dn::dense_kmajor_kernel<2>, dn::SMEM2); if (rc) return rc;
+  dn::dense_kmajor_kernel<2><<<dim3((F + dn::BM - 1) / dn::BM, (K + dn::BN - 1) / dn::BN, 1), dn::NTHREADS, dn::SMEM2, st>>>(a, am, bm);
+  CB_CUDA(cudaGetLastError());
+  return CB_OK;
 }
 
 }  // namespace cb

@@ -78,6 +78,21 @@ __global__ void pack_all_kernel(const float* __restrict__ params, const PackDesc
       }
     }
   }
+  if (d.dense) {      // dense_tc.cu forward B operand [N][K] (k = (y, x, c)): thread = (n, 8-channel group, pixel), pixel fastest, so that the canonical
+    // [n][c][y][x] reads are contiguous across threads; each thread writes one 16-byte vector
+    const uint32_t npix = (uint32_t)(g.kh * g.kw), c8n = (uint32_t)g.Cin / 8, totd = (uint32_t)g.Cout * c8n * npix;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < totd; i += stride) {
+      const uint32_t pix = i % npix, q = i / npix, c8 = q % c8n, n = q / c8n;
+      const int di = (int)(pix / (uint32_t)g.kw), dj = (int)(pix % (uint32_t)g.kw);
+      float f[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) f[j] = __ldg(params + d.pm.w((int)n, (int)(c8 * 8 + j), di, dj, g));
+      __nv_bfloat162 o[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) o[j] = __floats2bfloat162_rn(f[2 * j], f[2 * j + 1]);
+      *reinterpret_cast<uint4*>(wtf_all + d.wf_off + (size_t)n * K + (size_t)pix * g.Cin + c8 * 8) = *reinterpret_cast<const uint4*>(o);
+    }
+  }
   if (d.conv0) {      // forward B image [slot = 2*di + h][chunk][o][8]: chunks (di, 2h), (di, 2h+1); channels >= Cin and dj = 3 are zero
     const int tot0 = 6 * 2 * g.Cout * 8;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < tot0; i += gridDim.x * blockDim.x) {
@@ -360,13 +375,13 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
       continue;
     }
     double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
-    ProfScope ps(K_CONV_FWD, st, 1, 2.0 * M * N * K, in_bytes + (double)M * N * (L.f32_out ? 4 : sizeof(AT)) * (skip ? 2 : 1) + (double)K * N * sizeof(AT));
+    ProfScope ps(K_CONV_FWD, st, (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && !L.relu_in && dense_tc_supported(g)) ? 2 : 1, 2.0 * M * N * K, in_bytes + (double)M * N * (L.f32_out ? 4 : sizeof(AT)) * (skip ? 2 : 1) + (double)K * N * sizeof(AT));
     int rc;
     if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out && conv_tc_fits(g.H, g.W, g.Cin, g.Cout)) {
       rc = launch_conv_tc(0, F, g.H, g.W, g.Cin, g.Cout, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (const bf16*)skip, nullptr,
                           (bf16*)ws.act[L.out_t], L.relu_in, L.relu_out, ws.errflag, st);
-    } else if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
-      rc = launch_dense_fwd_tc(g, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.wf + L.wf_off, bias, (bf16*)ws.act[L.out_t], L.relu_in, ws.partial, ws.errflag, st);
+    } else if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && !L.relu_in && dense_tc_supported(g)) {
+      rc = launch_dense_fwd_tc(g, F, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (bf16*)ws.act[L.out_t], ws.partial, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && L.u8_in && conv0_tc_supported(g)) {
       const Op* nx = oi + 1 < net->fwd.size() ? &net->fwd[oi + 1] : nullptr;
       pool_fused = nx && nx->kind == OP_POOL && nx->in_t == L.out_t && nx->C % 8 == 0 && g.W % 2 == 0;
@@ -434,9 +449,9 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         if (batch.n > jobs_before) tc_off += slot;      // otherwise the call reduced its partials itself
         continue;
       }
-      if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && dense_tc_supported(g)) {
+      if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && !L.relu_in && dense_tc_supported(g)) {
         ProfScope ps(K_CONV_WGRAD, st, 2, 2.0 * g.H * g.W * g.Cin * g.Cout * (double)F, 2.0 * F * (g.H * g.W * g.Cin + g.Cout) + 4.0 * g.H * g.W * g.Cin * g.Cout);
-        int rc = launch_dense_wgrad_tc(g, L.pm, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.grad[op.dy], L.relu_in, grad, ws.errflag, st);
+        int rc = launch_dense_wgrad_tc(g, L.pm, F, (const bf16*)ws.act[L.in_t], (const bf16*)ws.grad[op.dy], grad, ws.errflag, st);
         if (rc) return rc;
         continue;
       }

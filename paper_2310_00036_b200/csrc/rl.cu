@@ -184,32 +184,55 @@ template <> __device__ __forceinline__ float rlog<float>(float x) { return logf(
 template <> __device__ __forceinline__ double rlog<double>(double x) { return log(x); }
 
 
+// lse and entropy of one row without a per-thread array (a runtime-indexed array would live in local memory): log p_i = l_i - lse is
+// recomputed where it is needed.
 template <typename R>
-__device__ __forceinline__ void log_softmax(const float* l, int A, R* lp, R* H) {
+__device__ __forceinline__ void lse_entropy(const float* l, int A, R* lse_out, R* H) {
   R m = (R)l[0];
   for (int i = 1; i < A; ++i) m = max(m, (R)l[i]);
   R s = 0;
   for (int i = 0; i < A; ++i) s += rexp<R>((R)l[i] - m);
-  R lse = m + rlog<R>(s);
+  const R lse = m + rlog<R>(s);
   R h = 0;
-  for (int i = 0; i < A; ++i) { lp[i] = (R)l[i] - lse; h -= rexp<R>(lp[i]) * lp[i]; }
-  *H = h;
+  for (int i = 0; i < A; ++i) { const R lp = (R)l[i] - lse; h -= rexp<R>(lp) * lp; }
+  *lse_out = lse; *H = h;
 }
 
-__global__ void logprob_kernel(const float* __restrict__ logits, int ld, int N, int A, const int32_t* __restrict__ actions,
-                               const int32_t* __restrict__ idx, float* __restrict__ logp_a, float* __restrict__ entropy) {
-  int n = blockIdx.x * blockDim.x + threadIdx.x;
+// Rows of `ld` floats (A logits first) for ROWS consecutive samples are contiguous in global memory: the block copies them to shared
+// memory with coalesced loads (row pitch ld + (ld even): odd, so that a thread walking its own row does not collide with its
+// neighbours' banks), one thread then owns one sample.
+constexpr int LP_ROWS = 128;
+__device__ __forceinline__ int lp_pitch(int ld) { return ld | 1; }
+__device__ __forceinline__ void stage_rows(const float* __restrict__ g, int ld, int n0, int nrows, float* sh) {
+  const int tot = nrows * ld, pitch = lp_pitch(ld);
+  const float* src = g + (size_t)n0 * ld;
+  const int dr = (int)blockDim.x / ld, dc = (int)blockDim.x - dr * ld;      // (row, column) advance per pass: no division in the loop
+  int r = (int)threadIdx.x / ld, c = (int)threadIdx.x - r * ld;
+  for (int i = threadIdx.x; i < tot; i += blockDim.x) {
+    sh[r * pitch + c] = src[i];
+    r += dr; c += dc; if (c >= ld) { c -= ld; ++r; }
+  }
+}
+
+__global__ void __launch_bounds__(LP_ROWS) logprob_kernel(const float* __restrict__ logits, int ld, int N, int A, const int32_t* __restrict__ actions,
+                                                          const int32_t* __restrict__ idx, float* __restrict__ logp_a, float* __restrict__ entropy) {
+  extern __shared__ float lp_sh[];
+  const int n0 = blockIdx.x * LP_ROWS, nrows = min(LP_ROWS, N - n0), n = n0 + threadIdx.x;
+  stage_rows(logits, ld, n0, nrows, lp_sh);
+  __syncthreads();
   if (n >= N) return;
-  double lp[MAX_A], H;
-  log_softmax<double>(logits + (size_t)n * ld, A, lp, &H);
+  const float* l = lp_sh + threadIdx.x * lp_pitch(ld);
+  double lse, H;
+  lse_entropy<double>(l, A, &lse, &H);
   int a = min(max(actions[idx ? idx[n] : n], 0), A - 1);      // never index out of bounds with a bad action (cleanba.h)
-  if (logp_a) logp_a[n] = (float)lp[a];
+  if (logp_a) logp_a[n] = (float)((double)l[a] - lse);
   if (entropy) entropy[n] = (float)H;
 }
 int launch_logprob(const float* logits, int ld, int N, int A, const int32_t* actions, const int32_t* idx, float* logp_a, float* entropy, cudaStream_t st) {
   if (N <= 0) return CB_OK;
-  ProfScope ps(K_LOGPROB, st, 1, 0.0, (double)N * (ld * 4.0 + 12));
-  logprob_kernel<<<(N + 127) / 128, 128, 0, st>>>(logits, ld, N, A, actions, idx, logp_a, entropy);
+  if (ld > 64) { set_error("logprob: row length > 64"); return CB_EINVAL; }
+  ProfScope ps(K_LOGPROB, st, 1, 0.0, (double)N * (ld * 4.0 + 4 + (logp_a ? 4 : 0) + (entropy ? 4 : 0)));
+  logprob_kernel<<<(N + LP_ROWS - 1) / LP_ROWS, LP_ROWS, (size_t)LP_ROWS * (ld | 1) * 4, st>>>(logits, ld, N, A, actions, idx, logp_a, entropy);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
@@ -225,8 +248,8 @@ __global__ void vtrace_kernel(int T, int B, const float* __restrict__ V, int ldV
   if (b >= B) return;
   float Vn = V[((size_t)T * B + b) * ldV];
   float acc = 0.f, vs_next = Vn;
-#pragma unroll 4
-  for (int t = T - 1; t >= 0; --t) {      // loads of four steps in flight; the recurrence runs in the definition's order
+#pragma unroll 8
+  for (int t = T - 1; t >= 0; --t) {      // loads of eight steps in flight; the recurrence runs in the definition's order
     size_t i = (size_t)t * B + b;
     float Vt = V[i * ldV];
     float disc = gamma * (1.0f - (float)d[i]);
@@ -255,8 +278,8 @@ __global__ void gae_kernel(int T, int B, const float* __restrict__ V, int ldV, c
   int b = blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= B) return;
   float Vn = V[((size_t)T * B + b) * ldV], a = 0.f;
-#pragma unroll 4
-  for (int t = T - 1; t >= 0; --t) {      // loads of four steps in flight; the recurrence runs in the definition's order
+#pragma unroll 8
+  for (int t = T - 1; t >= 0; --t) {      // loads of eight steps in flight; the recurrence runs in the definition's order
     size_t i = (size_t)t * B + b;
     float Vt = V[i * ldV];
     float disc = gamma * (1.0f - (float)d[i]);
@@ -370,39 +393,75 @@ template <typename AT> __device__ __forceinline__ void st_grad(AT* p, size_t i, 
 template <> __device__ __forceinline__ void st_grad<float>(float* p, size_t i, float v) { p[i] = v; }
 template <> __device__ __forceinline__ void st_grad<bf16>(bf16* p, size_t i, float v) { p[i] = __float2bfloat16_rn(v); }
 
-// O5 IMPALA loss terms + adjoint seeds (A4-A6).  terms: [5][N] = pg, v, H, rho, 0.
-template <typename AT, typename R>
-__global__ void impala_loss_kernel(int N, int A, const float* __restrict__ head, const int32_t* __restrict__ act, const float* __restrict__ vs,
-                                   const float* __restrict__ pgadv, const float* __restrict__ rho, float c1, float c2, float inv,
-                                   AT* __restrict__ dhead, float* __restrict__ terms) {
-  int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n >= N) return;
-  const float* l = head + (size_t)n * (A + 1);
-  R lp[MAX_A], H;
-  log_softmax<R>(l, A, lp, &H);
-  int a = min(max(act[n], 0), A - 1);
-  R pg = (R)pgadv[n], err = (R)vs[n] - (R)l[A];
-  for (int i = 0; i < A; ++i) {
-    R p = rexp<R>(lp[i]);
-    R g = (R)inv * (-pg * ((i == a ? (R)1 : (R)0) - p) + (R)c2 * p * (lp[i] + H));
-    st_grad<AT>(dhead, (size_t)n * (A + 1) + i, (float)g);
+// ---- losses (a8).  One thread per sample, LP_ROWS samples per block.  The block's head rows come in through shared memory
+// (coalesced), the seeds leave through shared memory (coalesced), and the five per-sample terms are summed per block in fp64 (fixed
+// tree) into partial[block][5]; stats_final_kernel adds the block partials in block order.  The association is a function of N only.
+template <typename AT>
+__device__ __forceinline__ void store_seed_rows(AT* __restrict__ dhead, int ld, int n0, int nrows, const float* sh) {
+  const int tot = nrows * ld, pitch = lp_pitch(ld);
+  AT* dst = dhead + (size_t)n0 * ld;
+  const int dr = (int)blockDim.x / ld, dc = (int)blockDim.x - dr * ld;
+  int r = (int)threadIdx.x / ld, c = (int)threadIdx.x - r * ld;
+  for (int i = threadIdx.x; i < tot; i += blockDim.x) {
+    st_grad<AT>(dst, (size_t)i, sh[r * pitch + c]);
+    r += dr; c += dc; if (c >= ld) { c -= ld; ++r; }
   }
-  st_grad<AT>(dhead, (size_t)n * (A + 1) + A, (float)(-(R)c1 * err * (R)inv));
-  terms[n] = (float)(-pg * lp[a]);
-  terms[(size_t)N + n] = (float)((R)0.5 * err * err);
-  terms[(size_t)2 * N + n] = (float)H;
-  terms[(size_t)3 * N + n] = rho ? rho[n] : 0.f;
-  terms[(size_t)4 * N + n] = 0.f;
+}
+// the five per-sample terms summed over the block in fp64: xor-shuffle tree inside each warp (a fixed association), then the warp sums
+// in warp order
+__device__ __forceinline__ void block_terms(double (&t)[5], double* shd, double* __restrict__ partial) {
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    double v = t[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if ((threadIdx.x & 31) == 0) shd[(threadIdx.x >> 5) * 5 + k] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 5) {
+    double s = 0.0;
+    for (int w = 0; w < LP_ROWS / 32; ++w) s += shd[w * 5 + threadIdx.x];
+    partial[(size_t)blockIdx.x * 5 + threadIdx.x] = s;
+  }
 }
 
-// sums the 5 term arrays in fp64 (fixed order) and writes the stats record.  mode 0 IMPALA, 1 PPO.
-__global__ void __launch_bounds__(1024) stats_kernel(int N, const float* __restrict__ terms, int mode, float c1, float c2, int reduction, float* __restrict__ stats) {
-  __shared__ double sh[1024];
+// O5 IMPALA loss terms + adjoint seeds (A4-A6).  terms = pg, v, H, rho, 0.
+template <typename AT, typename R>
+__global__ void __launch_bounds__(LP_ROWS) impala_loss_kernel(int N, int A, const float* __restrict__ head, const int32_t* __restrict__ act, const float* __restrict__ vs,
+                                                              const float* __restrict__ pgadv, const float* __restrict__ rho, float c1, float c2, float inv,
+                                                              AT* __restrict__ dhead, double* __restrict__ partial) {
+  extern __shared__ float lp_sh[];
+  __shared__ double shd[LP_ROWS];
+  const int ld = A + 1, n0 = blockIdx.x * LP_ROWS, nrows = min(LP_ROWS, N - n0), n = n0 + threadIdx.x;
+  stage_rows(head, ld, n0, nrows, lp_sh);
+  __syncthreads();
+  double t[5] = {0, 0, 0, 0, 0};
+  if (n < N) {
+    float* l = lp_sh + threadIdx.x * lp_pitch(ld);
+    R lse, H;
+    lse_entropy<R>(l, A, &lse, &H);
+    const int a = min(max(act[n], 0), A - 1);
+    const R pg = (R)pgadv[n], err = (R)vs[n] - (R)l[A], lpa = (R)l[a] - lse;
+    for (int i = 0; i < A; ++i) {
+      const R lp = (R)l[i] - lse, p = rexp<R>(lp);
+      l[i] = (float)((R)inv * (-pg * ((i == a ? (R)1 : (R)0) - p) + (R)c2 * p * (lp + H)));      // the row is overwritten by its seeds
+    }
+    l[A] = (float)(-(R)c1 * err * (R)inv);
+    t[0] = (double)(float)(-pg * lpa); t[1] = (double)(float)((R)0.5 * err * err); t[2] = (double)(float)H; t[3] = rho ? (double)rho[n] : 0.0;
+  }
+  __syncthreads();
+  store_seed_rows<AT>(dhead, ld, n0, nrows, lp_sh);
+  block_terms(t, shd, partial);
+}
+
+// adds the block partials [nblk][5] in block order (fp64) and writes the stats record.  mode 0 IMPALA, 1 PPO.
+__global__ void __launch_bounds__(256) stats_final_kernel(int N, int nblk, const double* __restrict__ partial, int mode, float c1, float c2, int reduction, float* __restrict__ stats) {
+  __shared__ double sh[256];
   double s[5];
   for (int k = 0; k < 5; ++k) {
     double v = 0.0;
-    for (int i = threadIdx.x; i < N; i += 1024) v += (double)terms[(size_t)k * N + i];
-    s[k] = block_sum<1024>(v, sh);
+    for (int i = threadIdx.x; i < nblk; i += 256) v += partial[(size_t)i * 5 + k];
+    s[k] = block_sum<256>(v, sh);
   }
   if (threadIdx.x == 0) {
     double invN = 1.0 / (double)N, inv = (mode == 0 && reduction == 1) ? 1.0 : invN;
@@ -416,16 +475,19 @@ __global__ void __launch_bounds__(1024) stats_kernel(int N, const float* __restr
   }
 }
 
+size_t loss_partial_doubles(int N) { return (size_t)((N + LP_ROWS - 1) / LP_ROWS) * 5 + 8; }
+
 int launch_impala_loss(int prec, int N, int A, const float* head, const int32_t* act, const float* vs, const float* pgadv, const float* rho,
-                       float c1, float c2, int reduction, void* dhead, float* terms, double*, float* stats, cudaStream_t st) {
-  if (A > MAX_A) { set_error("n_actions > %d", MAX_A); return CB_EINVAL; }
+                       float c1, float c2, int reduction, void* dhead, float*, double* red, float* stats, cudaStream_t st) {
+  if (A + 1 > MAX_A) { set_error("n_actions > %d", MAX_A - 1); return CB_EINVAL; }
   float inv = reduction == 0 ? (float)(1.0 / (double)N) : 1.0f;
-  int grid = (N + 127) / 128;
-  { ProfScope ps(K_LOSS, st, 1, 0.0, (double)N * ((A + 1) * (4.0 + (prec ? 2 : 4)) + 16 + 20));
-  if (prec == CB_PREC_FP32_REF) impala_loss_kernel<float, double><<<grid, 128, 0, st>>>(N, A, head, act, vs, pgadv, rho, c1, c2, inv, (float*)dhead, terms);
-  else impala_loss_kernel<bf16, float><<<grid, 128, 0, st>>>(N, A, head, act, vs, pgadv, rho, c1, c2, inv, (bf16*)dhead, terms); }
-  ProfScope ps2(K_STATS, st, 1, 0.0, (double)N * 20);
-  stats_kernel<<<1, 1024, 0, st>>>(N, terms, 0, c1, c2, reduction, stats);
+  const int grid = (N + LP_ROWS - 1) / LP_ROWS; const size_t smem = (size_t)LP_ROWS * ((A + 1) | 1) * 4;
+  double* partial = red + 8;
+  { ProfScope ps(K_LOSS, st, 1, 0.0, (double)N * ((A + 1) * (4.0 + (prec ? 2 : 4)) + 16));
+  if (prec == CB_PREC_FP32_REF) impala_loss_kernel<float, double><<<grid, LP_ROWS, smem, st>>>(N, A, head, act, vs, pgadv, rho, c1, c2, inv, (float*)dhead, partial);
+  else impala_loss_kernel<bf16, float><<<grid, LP_ROWS, smem, st>>>(N, A, head, act, vs, pgadv, rho, c1, c2, inv, (bf16*)dhead, partial); }
+  ProfScope ps2(K_STATS, st, 1, 0.0, (double)grid * 40);
+  stats_final_kernel<<<1, 256, 0, st>>>(N, grid, partial, 0, c1, c2, reduction, stats);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
@@ -442,52 +504,59 @@ __global__ void __launch_bounds__(1024) adv_stats_kernel(int m, const int32_t* _
   if (threadIdx.x == 0) { red[0] = mean; red[1] = sqrt(var); }
 }
 
-// O7 PPO loss terms + adjoint seeds (Eq. 2-3; A5-A8).  terms: [5][m] = pg, v, H, kl, clip.
+// O7 PPO loss terms + adjoint seeds (Eq. 2-3; A5-A8).  terms = pg, v, H, kl, clip.
 template <typename AT, typename R>
-__global__ void ppo_loss_kernel(int m, int A, const float* __restrict__ head, const int32_t* __restrict__ idx, const int32_t* __restrict__ act,
-                                const float* __restrict__ adv, const float* __restrict__ ret, const float* __restrict__ logp_old, float eps,
-                                float c1, float c2, int norm_adv, const double* __restrict__ red, AT* __restrict__ dhead, float* __restrict__ terms) {
-  int n = blockIdx.x * blockDim.x + threadIdx.x;
-  if (n >= m) return;
-  int src = idx ? idx[n] : n;
-  const float* l = head + (size_t)n * (A + 1);
-  R lp[MAX_A], H;
-  log_softmax<R>(l, A, lp, &H);
-  int a = min(max(act[src], 0), A - 1);
-  R inv = (R)(1.0 / (double)m);
-  R At = norm_adv ? (R)(((double)adv[src] - red[0]) / (red[1] + 1e-8)) : (R)adv[src];
-  R logr = lp[a] - (R)logp_old[src], r = rexp<R>(logr);
-  R lo = (R)1 - (R)eps, hi = (R)1 + (R)eps;
-  R rc = min(max(r, lo), hi);
-  R l1 = -At * r, l2 = -At * rc;
-  bool clipped = (At > 0 && r > hi) || (At < 0 && r < lo);   // strictly clipped on the penalised side (A7)
-  R dlogp = clipped ? (R)0 : -At * r * inv;
-  R err = (R)l[A] - (R)ret[src];
-  for (int i = 0; i < A; ++i) {
-    R p = rexp<R>(lp[i]);
-    R g = dlogp * ((i == a ? (R)1 : (R)0) - p) + inv * (R)c2 * p * (lp[i] + H);
-    st_grad<AT>(dhead, (size_t)n * (A + 1) + i, (float)g);
+__global__ void __launch_bounds__(LP_ROWS) ppo_loss_kernel(int m, int A, const float* __restrict__ head, const int32_t* __restrict__ idx, const int32_t* __restrict__ act,
+                                                           const float* __restrict__ adv, const float* __restrict__ ret, const float* __restrict__ logp_old, float eps,
+                                                           float c1, float c2, int norm_adv, const double* __restrict__ red, AT* __restrict__ dhead,
+                                                           double* __restrict__ partial) {
+  extern __shared__ float lp_sh[];
+  __shared__ double shd[LP_ROWS];
+  const int ld = A + 1, n0 = blockIdx.x * LP_ROWS, nrows = min(LP_ROWS, m - n0), n = n0 + threadIdx.x;
+  stage_rows(head, ld, n0, nrows, lp_sh);
+  __syncthreads();
+  double t[5] = {0, 0, 0, 0, 0};
+  if (n < m) {
+    const int src = idx ? idx[n] : n;
+    float* l = lp_sh + threadIdx.x * lp_pitch(ld);
+    R lse, H;
+    lse_entropy<R>(l, A, &lse, &H);
+    const int a = min(max(act[src], 0), A - 1);
+    const R inv = (R)(1.0 / (double)m);
+    const R At = norm_adv ? (R)(((double)adv[src] - red[0]) / (red[1] + 1e-8)) : (R)adv[src];
+    const R logr = ((R)l[a] - lse) - (R)logp_old[src], r = rexp<R>(logr);
+    const R lo = (R)1 - (R)eps, hi = (R)1 + (R)eps;
+    const R rc = min(max(r, lo), hi);
+    const R l1 = -At * r, l2 = -At * rc;
+    const bool clipped = (At > 0 && r > hi) || (At < 0 && r < lo);   // strictly clipped on the penalised side (A7)
+    const R dlogp = clipped ? (R)0 : -At * r * inv;
+    const R err = (R)l[A] - (R)ret[src];
+    for (int i = 0; i < A; ++i) {
+      const R lp = (R)l[i] - lse, p = rexp<R>(lp);
+      l[i] = (float)(dlogp * ((i == a ? (R)1 : (R)0) - p) + inv * (R)c2 * p * (lp + H));
+    }
+    l[A] = (float)((R)c1 * err * inv);
+    R ar = r - (R)1; if (ar < 0) ar = -ar;
+    t[0] = (double)(float)max(l1, l2); t[1] = (double)(float)((R)0.5 * err * err); t[2] = (double)(float)H;
+    t[3] = (double)(float)((r - (R)1) - logr); t[4] = ar > (R)eps ? 1.0 : 0.0;
   }
-  st_grad<AT>(dhead, (size_t)n * (A + 1) + A, (float)((R)c1 * err * inv));
-  R ar = r - (R)1; if (ar < 0) ar = -ar;
-  terms[n] = (float)max(l1, l2);
-  terms[(size_t)m + n] = (float)((R)0.5 * err * err);
-  terms[(size_t)2 * m + n] = (float)H;
-  terms[(size_t)3 * m + n] = (float)((r - (R)1) - logr);
-  terms[(size_t)4 * m + n] = ar > (R)eps ? 1.f : 0.f;
+  __syncthreads();
+  store_seed_rows<AT>(dhead, ld, n0, nrows, lp_sh);
+  block_terms(t, shd, partial);
 }
 
 int launch_ppo_loss(int prec, int m, int A, const float* head, const int32_t* idx, const int32_t* act, const float* adv, const float* ret,
-                    const float* logp_old, float eps, float c1, float c2, int norm_adv, void* dhead, float* terms, double* red, float*,
+                    const float* logp_old, float eps, float c1, float c2, int norm_adv, void* dhead, float*, double* red, float*,
                     float* stats, cudaStream_t st) {
-  if (A > MAX_A) { set_error("n_actions > %d", MAX_A); return CB_EINVAL; }
+  if (A + 1 > MAX_A) { set_error("n_actions > %d", MAX_A - 1); return CB_EINVAL; }
   if (norm_adv) { ProfScope ps0(K_STATS, st); adv_stats_kernel<<<1, 1024, 0, st>>>(m, idx, adv, red); }
-  int grid = (m + 127) / 128;
-  { ProfScope ps(K_LOSS, st, 1, 0.0, (double)m * ((A + 1) * (4.0 + (prec ? 2 : 4)) + 20 + 20));
-  if (prec == CB_PREC_FP32_REF) ppo_loss_kernel<float, double><<<grid, 128, 0, st>>>(m, A, head, idx, act, adv, ret, logp_old, eps, c1, c2, norm_adv, red, (float*)dhead, terms);
-  else ppo_loss_kernel<bf16, float><<<grid, 128, 0, st>>>(m, A, head, idx, act, adv, ret, logp_old, eps, c1, c2, norm_adv, red, (bf16*)dhead, terms); }
-  ProfScope ps2(K_STATS, st, 1, 0.0, (double)m * 20);
-  stats_kernel<<<1, 1024, 0, st>>>(m, terms, 1, c1, c2, 0, stats);
+  const int grid = (m + LP_ROWS - 1) / LP_ROWS; const size_t smem = (size_t)LP_ROWS * ((A + 1) | 1) * 4;
+  double* partial = red + 8;
+  { ProfScope ps(K_LOSS, st, 1, 0.0, (double)m * ((A + 1) * (4.0 + (prec ? 2 : 4)) + 20));
+  if (prec == CB_PREC_FP32_REF) ppo_loss_kernel<float, double><<<grid, LP_ROWS, smem, st>>>(m, A, head, idx, act, adv, ret, logp_old, eps, c1, c2, norm_adv, red, (float*)dhead, partial);
+  else ppo_loss_kernel<bf16, float><<<grid, LP_ROWS, smem, st>>>(m, A, head, idx, act, adv, ret, logp_old, eps, c1, c2, norm_adv, red, (bf16*)dhead, partial); }
+  ProfScope ps2(K_STATS, st, 1, 0.0, (double)grid * 40);
+  stats_final_kernel<<<1, 256, 0, st>>>(m, grid, partial, 1, c1, c2, 0, stats);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }
