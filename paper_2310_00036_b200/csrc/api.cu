@@ -477,8 +477,7 @@ int cb_learner_grad(cb_net* net, int u, float** grad_dev, void* stream) {
   if (!(c.ppo && u == 0 && net->last_has_head)) { if ((rc = pack_weights(net, prec, c.params, st))) return rc; }      // PPO update 0 after the no-grad forward: same parameters, already packed
   ws.packed = false;      // after this call the packs no longer hold what `params` holds (the optimizer runs next)
   if (!c.ppo && c.mb == 1) {
-    if ((rc = forward(net, prec, c.obs, nullptr, F, st))) return rc;
-    if ((rc = launch_logprob(head, A + 1, N, A, c.actions, nullptr, ws.logpi, nullptr, st))) return rc;
+    if ((rc = forward(net, prec, c.obs, nullptr, F, st, false, c.actions, N, ws.logpi))) return rc;      // log pi(a_t) comes out of the heads kernel
     if ((rc = launch_vtrace(T, B, head + A, A + 1, c.rewards, c.dones, ws.logpi, ws.logmu, hp.gamma, hp.lambda_, hp.rho_bar, hp.c_bar, hp.rho_pg_bar, ws.t0, ws.t1, ws.rho, st))) return rc;
     if ((rc = launch_impala_loss(prec, N, A, head, c.actions, ws.t0, ws.t1, ws.rho, hp.vf_coef, hp.ent_coef, hp.loss_reduction, ws.grad[G_HEAD], ws.terms, ws.red, row, st))) return rc;
     if ((rc = backward(net, prec, c.obs, nullptr, N, ws.gradbuf, st))) return rc;
@@ -486,8 +485,7 @@ int cb_learner_grad(cb_net* net, int u, float** grad_dev, void* stream) {
     // A21: one complete update per group of B/mb envs, in group order, each with the parameters the previous one left
     const int Bm = B / c.mb, Nm = T * Bm, Fm = (T + 1) * Bm;
     if ((rc = launch_gather_traj(T, B, u * Bm, Bm, c.actions, c.rewards, c.dones, ws.logmu, ws.perm, ws.act_m, ws.rew_m, ws.dones_m, ws.logmu_m, st))) return rc;
-    if ((rc = forward(net, prec, c.obs, ws.perm, Fm, st))) return rc;
-    if ((rc = launch_logprob(head, A + 1, Nm, A, ws.act_m, nullptr, ws.logpi, nullptr, st))) return rc;
+    if ((rc = forward(net, prec, c.obs, ws.perm, Fm, st, false, ws.act_m, Nm, ws.logpi))) return rc;
     if ((rc = launch_vtrace(T, Bm, head + A, A + 1, ws.rew_m, ws.dones_m, ws.logpi, ws.logmu_m, hp.gamma, hp.lambda_, hp.rho_bar, hp.c_bar, hp.rho_pg_bar, ws.t0, ws.t1, ws.rho, st))) return rc;
     if ((rc = launch_impala_loss(prec, Nm, A, head, ws.act_m, ws.t0, ws.t1, ws.rho, hp.vf_coef, hp.ent_coef, hp.loss_reduction, ws.grad[G_HEAD], ws.terms, ws.red, row, st))) return rc;
     if ((rc = backward(net, prec, c.obs, ws.perm, Nm, ws.gradbuf, st))) return rc;

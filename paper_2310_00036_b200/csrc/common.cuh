@@ -148,7 +148,9 @@ struct ProfScope {      // counts `n` launches of class `cls`; records an event 
 int ensure_workspace(cb_net* net, int prec, int frames);
 int ensure_learner_scratch(cb_net* net, int prec, int F, int N, int epochs);
 int pack_weights(cb_net* net, int prec, const float* params, cudaStream_t st);
-int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads = false);
+// taken / n_taken / logp_taken: the heads kernel also writes log pi(taken[n]) for frames n < n_taken (learner side; nullable)
+int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads = false,
+            const int32_t* taken = nullptr, int n_taken = 0, float* logp_taken = nullptr);
 int backward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, float* grad, cudaStream_t st);
 
 // conv_tc.cu
@@ -194,7 +196,7 @@ int launch_sample(const float* logits, int ld, int B, int A, uint64_t seed, uint
                   int32_t* actions, cudaStream_t st);
 int launch_heads_sample(int prec, const void* hid, const void* wf, const float* bias, int B, int fc, int A, uint64_t seed, uint64_t step,
                         uint32_t env_offset, float* head, float* logits, float* value, int32_t* actions, cudaStream_t st,
-                        const int* errflag = nullptr, int* errhost = nullptr);
+                        const int* errflag = nullptr, int* errhost = nullptr, const int32_t* taken = nullptr, int n_taken = 0, float* logp_taken = nullptr);
 int launch_split_head(const float* head, int F, int A, float* logits, float* value, cudaStream_t st);
 int launch_logprob(const float* logits, int ld, int N, int A, const int32_t* actions, const int32_t* idx,
                    float* logp_a, float* entropy, cudaStream_t st);

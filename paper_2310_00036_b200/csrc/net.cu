@@ -341,7 +341,8 @@ size_t wgrad_partial_elems(const Geom& g, long long frames) {
 static inline int grid_for(size_t total) { return (int)std::min<size_t>((total + 255) / 256, (size_t)148 * 16); }
 
 template <typename AT>
-static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads) {
+static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads,
+                     const int32_t* taken, int n_taken, float* logp_taken) {
   bool pool_fused = false;      // the first layer's kernel also produced the pooled map: skip the following POOL op
   for (size_t oi = 0; oi < net->fwd.size(); ++oi) {
     const Op& op = net->fwd[oi];
@@ -370,7 +371,7 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     const AT* skip = L.skip_t >= 0 ? (const AT*)ws.act[L.skip_t] : nullptr;
     if (L.f32_out && L.relu_in && g.kh == 1 && g.kw == 1 && g.H == 1 && g.W == 1 && N <= 32 && !skip) {      // the heads: one warp per frame (its own profile class)
       int rc = launch_heads_sample(std::is_same<AT, bf16>::value ? CB_PREC_BF16_TC : CB_PREC_FP32_REF, ws.act[L.in_t], wf, bias, M, K, N - 1, 0, 0, 0,
-                                   (float*)ws.act[L.out_t], nullptr, nullptr, nullptr, st);
+                                   (float*)ws.act[L.out_t], nullptr, nullptr, nullptr, st, nullptr, nullptr, taken, n_taken, logp_taken);
       if (rc) return rc;
       continue;
     }
@@ -402,9 +403,11 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
   return CB_OK;
 }
 
-int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads) {
+int forward(cb_net* net, int prec, const uint8_t* obs, const int32_t* frame_idx, int F, cudaStream_t st, bool skip_heads, const int32_t* taken, int n_taken,
+            float* logp_taken) {
   Workspace& ws = net->ws[prec];
-  return prec == CB_PREC_FP32_REF ? forward_t<float>(net, ws, obs, frame_idx, F, st, skip_heads) : forward_t<bf16>(net, ws, obs, frame_idx, F, st, skip_heads);
+  return prec == CB_PREC_FP32_REF ? forward_t<float>(net, ws, obs, frame_idx, F, st, skip_heads, taken, n_taken, logp_taken)
+                                  : forward_t<bf16>(net, ws, obs, frame_idx, F, st, skip_heads, taken, n_taken, logp_taken);
 }
 
 template <typename AT>

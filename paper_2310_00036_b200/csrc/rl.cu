@@ -85,7 +85,7 @@ template <typename AT>
 __global__ void heads_sample_kernel(const AT* __restrict__ hid, const AT* __restrict__ wf, const float* __restrict__ bias, int B, int fc, int A,
                                     uint32_t k0, uint32_t k1, uint32_t step_lo, uint32_t step_hi, uint32_t env_offset,
                                     float* __restrict__ head, float* __restrict__ logits, float* __restrict__ value, int32_t* __restrict__ actions,
-                                    const int* __restrict__ errflag, int* errhost) {
+                                    const int* __restrict__ errflag, int* errhost, const int32_t* __restrict__ taken, int n_taken, float* __restrict__ logp_taken) {
   const int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (b >= B) return;
   const int N = A + 1;
@@ -124,6 +124,20 @@ __global__ void heads_sample_kernel(const AT* __restrict__ hid, const AT* __rest
     if (head) head[(size_t)b * N + lane] = mine;
     if (lane < A) { if (logits) logits[(size_t)b * A + lane] = mine; } else if (value) value[b] = mine;
   }
+  if (logp_taken && b < n_taken) {
+    // learner side (a4): log pi(a_t | s_t) of the action the rollout took, from the warp's own logits: lse = max + log sum exp(l - max)
+    // in fp64 with a fixed xor-shuffle tree (the arithmetic of logprob_kernel, without a second pass over the logits)
+    const double l = lane < A ? (double)mine : -INFINITY;
+    double m = l;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    double s = lane < A ? exp(l - m) : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    const int a = min(max(taken[b], 0), A - 1);
+    const double la = __shfl_sync(0xffffffffu, l, a);
+    if (lane == 0) logp_taken[b] = (float)(la - (m + log(s)));
+  }
   if (actions) {
     float sc = -INFINITY;
     if (lane < A) {
@@ -143,17 +157,17 @@ __global__ void heads_sample_kernel(const AT* __restrict__ hid, const AT* __rest
 
 int launch_heads_sample(int prec, const void* hid, const void* wf, const float* bias, int B, int fc, int A, uint64_t seed, uint64_t step,
                         uint32_t env_offset, float* head, float* logits, float* value, int32_t* actions, cudaStream_t st,
-                        const int* errflag, int* errhost) {
+                        const int* errflag, int* errhost, const int32_t* taken, int n_taken, float* logp_taken) {
   if (B <= 0) return CB_OK;
   if (A + 1 > MAX_A) { set_error("n_actions too large"); return CB_EINVAL; }
   ProfScope ps(K_SAMPLE, st);
   const int grid = (B * 32 + 127) / 128;
   if (prec == CB_PREC_FP32_REF)
     heads_sample_kernel<float><<<grid, 128, 0, st>>>((const float*)hid, (const float*)wf, bias, B, fc, A, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step,
-                                                      (uint32_t)(step >> 32), env_offset, head, logits, value, actions, errflag, errhost);
+                                                      (uint32_t)(step >> 32), env_offset, head, logits, value, actions, errflag, errhost, taken, n_taken, logp_taken);
   else
     heads_sample_kernel<bf16><<<grid, 128, 0, st>>>((const bf16*)hid, (const bf16*)wf, bias, B, fc, A, (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)step,
-                                                     (uint32_t)(step >> 32), env_offset, head, logits, value, actions, errflag, errhost);
+                                                     (uint32_t)(step >> 32), env_offset, head, logits, value, actions, errflag, errhost, taken, n_taken, logp_taken);
   CB_CUDA(cudaGetLastError());
   return CB_OK;
 }

@@ -1,4 +1,4 @@
-// Thin inline-PTX wrappers for tcgen05 / TMEM / mbarrier on sm_100a (used by conv0_tc.cu).
+// Thin inline-PTX wrappers for tcgen05 / TMEM / mbarrier on sm_100a, shared by every tensor-core kernel of the library.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>

@@ -6,6 +6,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 namespace cb {
 namespace tma {
@@ -13,8 +14,13 @@ namespace tma {
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
+// CB_DISABLE_TMA=1 in the environment makes every tensor-map request fail, which selects the kernels that stage their operands through
+// the load/store units (conv3x3_tc_kernel, wgrad3x3_tc_kernel; the fc layer falls back to the SIMT GEMM): the paths a driver without
+// cuTensorMapEncodeTiled would take.  tests/test_gpu_learner.py::test_no_tma_fallback_kernels runs them under the oracle.
 inline EncodeTiledFn encode_fn() {
   static EncodeTiledFn fn = nullptr;
+  static const bool disabled = [] { const char* e = getenv("CB_DISABLE_TMA"); return e && e[0] == '1'; }();
+  if (disabled) return nullptr;
   if (!fn) {
     void* p = nullptr; cudaDriverEntryPointQueryResult q;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) fn = (EncodeTiledFn)p;

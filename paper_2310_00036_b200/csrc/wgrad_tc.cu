@@ -2,306 +2,26 @@
 //
 //   dW[tap][c][o] = sum_q X[q + shift(tap)][c] * DY[q][o]        db[o] = sum_q DY[q][o]
 //
-// with q running over the pixel-linear positions of conv_tc.cu (DY is staged with zeros at halo
-// positions, X with its zero halo and ReLU applied on the way in).  The contraction index is the PIXEL, so
-// both operands are MN-major: in the plane layout plane[ch/8][q][ch%8] (16 B per (position, chunk)) a
-// core matrix is 8 positions x 8 channels with the K rows 16 B apart -- exactly the canonical MN-major
-// no-swizzle UMMA layout (LBO = 128 B between groups of 8 positions, SBO = plane stride between groups
-// of 8 channels).  A tap is again a constant shift of A's start address.
-//
-// UMMA needs M = 128 rows while a layer has Cin = 16/32 (+1 bias row) real ones: the descriptor simply
-// walks on into the following planes (a plane of ones for the bias row, then DY, then zeros); those
-// rows of D are never read.  The 9 accumulators [128 x Cout] stay in TMEM (9*Cout <= 288 columns) for
-// the whole life of the CTA, which runs over a fixed set of (frame-group, row-band) work items and
-// writes ONE fp32 partial [9][Cin+1][Cout] at the end; a second kernel adds the partials in CTA order,
-// so the result is bitwise reproducible (no atomics; the item -> CTA map depends on the shape only).
+// with q running over the pixel-linear positions of conv_tc.cu.  The contraction index is the PIXEL, so both operands are MN-major.
+// X and DY are landed once each by TMA as whole pixels (one swizzled shared-memory row per position); the descriptors WALK over that
+// single copy (see wgrad3x3_sw_kernel below): ONE tcgen05.mma per 16 positions yields all nine taps.  The accumulator stays in TMEM for
+// the whole life of the CTA, which runs over a fixed set of (frame-group, row-band) items and writes ONE fp32 partial [9][Cin+1][Cout]
+// at the end; a second kernel adds the partials in CTA order, so the result is bitwise reproducible (no atomics; the item -> CTA map
+// depends on the shape only).  Without TMA wgrad_tc_supported() is false and the layer runs on the SIMT split-K GEMM.
 #include "common.cuh"
 #include "tma.cuh"
 
 #include <cstring>
+#include "tc_ptx.cuh"
 
 namespace cb {
 namespace tcw {
 
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-  uint64_t d = (uint64_t)((saddr >> 4) & 0x3FFFu);
-  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16;
-  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32;
-  d |= (uint64_t)1 << 46;
-  return d;
-}
-__device__ __forceinline__ void mma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}\n"
-               :: "r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
-// one lane of a converged warp; the compiler then issues the tcgen05 instruction from the uniform datapath
-// instead of looping over the active lanes of a divergent branch (which costs ~50 clk per MMA)
-__device__ __forceinline__ bool elect_one() {
-  uint32_t pred = 0;
-  asm volatile("{\n\t.reg .b32 rx;\n\t.reg .pred px;\n\telect.sync rx|px, %1;\n\t@px mov.s32 %0, 1;\n\t}\n" : "+r"(pred) : "r"(0xFFFFFFFFu));
-  return pred != 0;
-}
-__device__ __forceinline__ void mma_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" :: "r"(bar) : "memory");
-}
-__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity) {
-  for (uint32_t it = 0; it < (1u << 24); ++it) {
-    uint32_t ok;
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
-                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-    if (ok) return true;
-  }
-  return false;
-}
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
-  uint32_t r[16];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
-                 "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-               : "r"(taddr) : "memory");
-  asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
-#pragma unroll
-  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
-}
+using namespace ptx;      // tcgen05 / TMEM / mbarrier wrappers: tc_ptx.cuh
 
-struct WgradTcArgs {
-  const bf16* x;      // [F, H, W, CIN]  layer input (pre-activation when relu_in)
-  const bf16* dy;     // [F, H, W, COUT]
-  float* partial;     // [gridDim.x][9][CIN+1][COUT]
-  int F, H, W, G, R, nbands, npix_alloc, kext, relu_in, stage_planes, use_tma, dy_rows;
-  int repl;           // ST3 with TMA: only the dj = 0 planes are landed (the TMA unit moves about one 16-byte piece per clock, so three
-                      // shifted boxes would bound the kernel); the loader warps derive the dj = 1, 2 copies in shared memory
-  int c_off, cin_total;      // the kernel handles input channels [c_off, c_off + CIN) of a layer with cin_total channels
-  int* error_flag;
-};
-
+constexpr int NLOAD = 256;       // warps 0-7: loaders / bias sums (warps 0-3 later read TMEM); warp 8 issues the MMAs; warp 9 produces
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
-}
-
-constexpr int NLOAD = 256;       // warps 0-7: stage operands (warps 0-3 later read TMEM); warp 8: one thread issues the MMAs
-
-// UM = UMMA M (64 or 128): rows 0..CIN(+bias) are real, the rest walks into the following planes and is ignored.
-// Two shared-memory stages: the loader warps fill stage s+1 while the tensor core works on stage s.
-// ST3 (Cin = 16 only): the loaders store every X element three times, shifted by dj = 0,1,2 positions, into planes
-// (dj, chunk); the M walk of ONE MMA then covers the three taps (di, 0..2) at rows dj*CIN + c -- 3 instead of 9
-// MMAs per 16 positions, and 49 instead of 17 useful rows of 64.
-template <int CIN, int COUT, int UM, bool ST3>
-__global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_tc_kernel(const WgradTcArgs a, const __grid_constant__ CUtensorMap xmap, const __grid_constant__ CUtensorMap ymap) {
-  extern __shared__ __align__(128) uint8_t smem[];
-  constexpr int XCH = CIN / 8, YCH = COUT / 8, XPL = ST3 ? 3 * XCH : XCH;      // X planes per stage
-  constexpr int NACC = ST3 ? 3 : 9;
-  constexpr uint32_t TCOLS = (NACC * COUT <= 128) ? 128u : ((NACC * COUT <= 256) ? 256u : 512u);
-  static_assert(!ST3 || 3 * CIN + 1 <= UM, "3-tap stacking needs 3*CIN+1 rows");
-  __shared__ __align__(8) uint64_t bars[7];          // full[2], empty[2], done, raw[2] (TMA landed)
-  __shared__ uint32_t tmem_base_smem;
-  const int tid = threadIdx.x, warp = tid >> 5;
-  const int Wp = a.W + 2, Rb = (a.R + 2) * Wp;          // positions per frame region of a band
-  const uint32_t P = (uint32_t)a.npix_alloc * 16u;      // plane stride
-  const uint32_t stage_bytes = (uint32_t)a.stage_planes * P;
-  // per stage: planes [0, XCH) X | XCH: ones (bias row) | [XCH+1, XCH+1+YCH) DY | padding planes (zeros)
-  const uint32_t bar0 = smem_u32(&bars[0]);
-  if (tid == 0) {
-    for (int i = 0; i < 7; ++i) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" :: "r"(bar0 + 8u * i) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
-  }
-  if (warp == NLOAD / 32) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" :: "r"(smem_u32(&tmem_base_smem)), "r"(TCOLS) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
-  }
-  // total allocation: the last stage's A descriptor may walk UM/8 planes from its start
-  const uint32_t total_bytes = stage_bytes + (uint32_t)max(a.stage_planes, UM / 8) * P;
-  for (uint32_t i = tid; i < total_bytes / 16; i += NLOAD + 64) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
-  __syncthreads();
-  {
-    const uint32_t one2 = 0x3F803F80u;    // two bf16 ones
-    for (int st = 0; st < 2; ++st)
-      for (uint32_t i = tid; i < P / 16; i += NLOAD + 64) reinterpret_cast<uint4*>(smem + (size_t)st * stage_bytes + (size_t)XPL * P)[i] = make_uint4(one2, one2, one2, one2);
-  }
-  asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-  __syncthreads();
-  asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-  const uint32_t tmem_base = tmem_base_smem;
-  const int ngroups = (a.F + a.G - 1) / a.G, nitems = ngroups * a.nbands;
-  const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
-
-  const bool direct = a.use_tma && !a.relu_in && !a.repl;      // nothing to do between the TMA landing and the MMAs: the issuer waits on raw[] itself
-  if (warp < NLOAD / 32) {
-    // ================= loaders =================
-    for (int it = 0; it < (direct ? 0 : my_items); ++it) {
-      const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
-      if (!a.use_tma && use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 2; }
-      uint8_t* xs = smem + (size_t)s * stage_bytes;
-      uint8_t* ys = xs + (size_t)(XPL + 1) * P;
-      const int grp = item / a.nbands, band = item - grp * a.nbands;
-      const int f0 = grp * a.G, nf = min(a.G, a.F - f0), yb = band * a.R;
-      if (a.use_tma) {
-        // operands were landed by the TMA producer thread; only the ReLU (in place) is left to these warps
-        if (!mbar_wait(bar0 + 8u * (5 + s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 7; }
-        if (a.repl) {
-          const int n16 = a.G * Rb;
-          const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
-          for (int i = tid; i < n16 * XCH; i += NLOAD) {
-            const int ch = i / n16, pos = i - ch * n16;
-            uint8_t* p = xs + (size_t)ch * P + (size_t)pos * 16;
-            uint4 v = *reinterpret_cast<uint4*>(p);
-            if (a.relu_in) {
-              __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
-#pragma unroll
-              for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
-              *reinterpret_cast<uint4*>(p) = v;
-            }
-            if (pos >= 1) *reinterpret_cast<uint4*>(p + (size_t)XCH * P - 16) = v;          // plane (1, ch), one position earlier
-            if (pos >= 2) *reinterpret_cast<uint4*>(p + (size_t)2 * XCH * P - 32) = v;      // plane (2, ch), two positions earlier
-          }
-        } else if (a.relu_in) {
-          const int n16 = a.G * Rb;
-          for (int i = tid; i < n16 * XPL; i += NLOAD) {
-            const int pl = i / n16, pos = i - pl * n16;
-            uint4* p = reinterpret_cast<uint4*>(xs + (size_t)pl * P + (size_t)pos * 16);
-            uint4 v = *p;
-            __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v);
-            const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
-            *p = v;
-          }
-        }
-      } else {
-      const int xn = a.G * Rb * XCH;
-      for (int i0 = tid; i0 < xn; i0 += NLOAD * 4) {
-        uint4 v[4]; uint32_t dst[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int i = i0 + u * NLOAD;
-          v[u] = make_uint4(0, 0, 0, 0); dst[u] = 0xFFFFFFFFu;
-          if (i < xn) {
-            int ch = i % XCH, pos = i / XCH;
-            int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, xp = rem - lr * Wp;
-            int y = yb - 1 + lr, x = xp - 1;
-            dst[u] = (uint32_t)ch * P + (uint32_t)pos * 16u;
-            if (j < nf && (unsigned)y < (unsigned)a.H && (unsigned)x < (unsigned)a.W)
-              v[u] = *reinterpret_cast<const uint4*>(a.x + (((size_t)(f0 + j) * a.H + y) * a.W + x) * a.cin_total + a.c_off + ch * 8);
-          }
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          if (dst[u] == 0xFFFFFFFFu) continue;
-          if (a.relu_in) {
-            __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&v[u]);
-            const __nv_bfloat162 z = __float2bfloat162_rn(0.f);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) h[k] = __hmax2(h[k], z);
-          }
-          *reinterpret_cast<uint4*>(xs + dst[u]) = v[u];
-          if (ST3) {      // dst = ch*P + pos*16: the copies for dj = 1, 2 live XCH / 2*XCH planes further, 1 / 2 positions earlier
-            const uint32_t pos16 = dst[u] % P;
-            if (pos16 >= 16u) *reinterpret_cast<uint4*>(xs + dst[u] + (uint32_t)XCH * P - 16u) = v[u];
-            if (pos16 >= 32u) *reinterpret_cast<uint4*>(xs + dst[u] + 2u * (uint32_t)XCH * P - 32u) = v[u];
-          }
-        }
-      }
-      const int yn = a.kext * YCH;
-      for (int i0 = tid; i0 < yn; i0 += NLOAD * 4) {
-        uint4 v[4]; uint32_t dst[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int i = i0 + u * NLOAD;
-          v[u] = make_uint4(0, 0, 0, 0); dst[u] = 0xFFFFFFFFu;
-          if (i < yn) {
-            int ch = i % YCH, pos = i / YCH;
-            int j = pos / Rb, rem = pos - j * Rb, lr = rem / Wp, x = rem - lr * Wp;
-            int y = yb + lr;
-            dst[u] = (uint32_t)ch * P + (uint32_t)pos * 16u;
-            if (j < nf && lr < a.R && y < a.H && x < a.W)
-              v[u] = *reinterpret_cast<const uint4*>(a.dy + (((size_t)(f0 + j) * a.H + y) * a.W + x) * COUT + ch * 8);
-          }
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) if (dst[u] != 0xFFFFFFFFu) *reinterpret_cast<uint4*>(ys + dst[u]) = v[u];
-      }
-      }
-      asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-      asm volatile("bar.sync 1, %0;\n" :: "n"(NLOAD) : "memory");
-      if (tid == 0) mbar_arrive(bar0 + 8u * s);
-    }
-    // ================= epilogue (warps 0-3 own the TMEM lanes) =================
-    if (warp < 4) {
-    if (my_items > 0 && !mbar_wait(bar0 + 8u * 4, 0u)) { if (a.error_flag) *a.error_flag = 2; }
-    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-    float* out = a.partial + (size_t)blockIdx.x * 9 * (CIN + 1) * COUT;
-    // UM = 128: accumulator row r sits in TMEM lane r; UM = 64: in lane 32*(r/16) + r%16
-    const int lane = tid & 31;
-    const int row = (UM == 128) ? tid : ((lane < 16) ? warp * 16 + lane : 1 << 20);
-    constexpr int LAST_ROW = ST3 ? 3 * CIN : CIN;         // the bias row
-    const bool warp_needed = (UM == 128) ? (warp * 32 <= LAST_ROW) : (warp * 16 <= LAST_ROW);
-    if (warp_needed) {
-      for (int acc = 0; acc < NACC; ++acc) {
-#pragma unroll
-        for (int c0 = 0; c0 < COUT; c0 += 16) {
-          float v[16];
-          tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + (uint32_t)(acc * COUT + c0), v);
-          if (row > LAST_ROW) continue;
-          int tap, r;
-          if (ST3) { if (row == LAST_ROW) { if (acc) continue; tap = 0; r = CIN; } else { tap = acc * 3 + row / CIN; r = row % CIN; } }
-          else { tap = acc; r = row; }
-#pragma unroll
-          for (int i = 0; i < 16; ++i) out[((size_t)tap * (CIN + 1) + r) * COUT + c0 + i] = v[i];
-        }
-      }
-    }
-    }
-  } else if (tid == NLOAD + 32) {
-    // ================= TMA producer: runs one stage ahead of the tensor core =================
-    if (a.use_tma) {
-      tma::prefetch_map(&xmap); tma::prefetch_map(&ymap);
-      const uint32_t xbytes = (uint32_t)(a.G * Rb) * 16u, ybytes = (uint32_t)(a.G * a.dy_rows * Wp) * 16u;
-      for (int it = 0; it < my_items; ++it) {
-        const int item = blockIdx.x + it * gridDim.x, s = it & 1, use = it >> 1;
-        if (use > 0 && !mbar_wait(bar0 + 8u * (2 + s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 7; }
-        const int grp = item / a.nbands, band = item - grp * a.nbands, f0 = grp * a.G, yb = band * a.R;
-        const uint32_t xs = smem_u32(smem + (size_t)s * stage_bytes), ys = xs + (uint32_t)(XPL + 1) * P, rb = bar0 + 8u * (5 + s);
-        const int npl = a.repl ? XCH : XPL;
-        tma::arrive_expect_tx(rb, xbytes * (uint32_t)npl + ybytes * YCH);
-        for (int pl = 0; pl < npl; ++pl) {       // plane (dj, ch): X shifted by dj positions = box started dj columns further right
-          const int dj = ST3 ? pl / XCH : 0, ch = ST3 ? pl % XCH : pl;
-          tma::load_4d(xs + (uint32_t)pl * P, &xmap, a.c_off + ch * 8, -1 + dj, yb - 1, f0, rb);
-        }
-        for (int ch = 0; ch < YCH; ++ch) tma::load_4d(ys + (uint32_t)ch * P, &ymap, ch * 8, 0, yb, f0, rb);
-      }
-    }
-  } else if (warp == NLOAD / 32) {
-    // ================= MMA issuer: the whole warp runs the loop, one elected lane issues =================
-    const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | (1u << 16) | ((uint32_t)(COUT >> 3) << 17) | ((uint32_t)(UM >> 4) << 24);
-    const uint32_t desc_hi = ((P >> 4) & 0x3FFFu) | (1u << 14);        // SBO = plane stride, descriptor version bit 46
-    uint32_t accumulate = 0;
-    for (int it = 0; it < my_items; ++it) {
-      const int s = it & 1, use = it >> 1;
-      if (!mbar_wait(bar0 + 8u * (direct ? 5 + s : s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 2; }
-      asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-      const uint32_t x_base = smem_u32(smem + (size_t)s * stage_bytes), y_base = x_base + (uint32_t)(XPL + 1) * P;
-      const uint32_t x_lo = ((x_base >> 4) & 0x3FFFu) | (8u << 16), y_lo = ((y_base >> 4) & 0x3FFFu) | (8u << 16);   // LBO = 128 B
-      for (int k0 = 0; k0 < a.kext; k0 += 16) {
-        const uint64_t bd = ((uint64_t)desc_hi << 32) | (uint64_t)(y_lo + (uint32_t)k0);
-#pragma unroll
-        for (int acc = 0; acc < NACC; ++acc) {
-          const uint32_t shift = ST3 ? (uint32_t)(acc * Wp) : (uint32_t)((acc / 3) * Wp + (acc % 3));
-          const uint64_t ad = ((uint64_t)desc_hi << 32) | (uint64_t)(x_lo + (uint32_t)k0 + shift);
-          if (elect_one()) mma_f16(tmem_base + (uint32_t)(acc * COUT), ad, bd, idesc, accumulate);
-        }
-        accumulate = 1;
-      }
-      if (elect_one()) mma_commit(bar0 + 8u * (2 + s));          // stage s may be refilled once these MMAs have read it
-      __syncwarp();
-    }
-    if (elect_one()) mma_commit(bar0 + 8u * 4);                  // everything issued so far has completed -> accumulators final
-    __syncwarp();
-  }
-  asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-  __syncthreads();
-  if (warp == NLOAD / 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" :: "r"(tmem_base), "r"(TCOLS) : "memory");
 }
 
 // sums the per-CTA partials in CTA order and scatters to the canonical gradient
@@ -371,7 +91,7 @@ __global__ void __launch_bounds__(RL * RB) wgrad_tc_reduce_batch_kernel(const __
 }
 
 // ------------------------------------------------------------------------------------------------
-// Swizzled variant (TMA, Cin in {16, 32}): whole pixels are landed once, one shared-memory row of 2*CIN (X) or 2*COUT (DY)
+// The kernel (TMA, Cin in {16, 32, 64}): whole pixels are landed once, one shared-memory row of 2*CIN (X) or 2*COUT (DY)
 // bytes per position, in the 32B/64B/128B swizzle pattern.  The A descriptor is MN-major with LBO = one row: the M walk
 // steps to the NEXT POSITION, so rows dj*CIN + c of one MMA are the taps (di, 0..2) without any shifted copy of X
 // (the pattern is a function of the absolute address, so descriptors may start at any row).  The B descriptor walks N the
@@ -551,45 +271,12 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
 bool wgrad_tc_supported(const Geom& g) {
   // Cin = 64 runs as two launches over 32 input channels each; Cin = 16 supports Cout <= 32
   const bool okc = (g.Cin == 16 && (g.Cout == 16 || g.Cout == 32)) || ((g.Cin == 32 || g.Cin == 64) && (g.Cout == 16 || g.Cout == 32 || g.Cout == 64));
-  return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && okc && g.H == g.Ho && g.W == g.Wo;
+  return g.kh == 3 && g.kw == 3 && g.s == 1 && g.p == 1 && okc && g.H == g.Ho && g.W == g.Wo && tma::encode_fn() != nullptr;      // TMA-fed only
 }
 
 constexpr int WGRAD_TC_MAX_CTAS = 148;
 size_t wgrad_tc_partial_elems(const Geom& g) { return (size_t)WGRAD_TC_MAX_CTAS * 9 * (g.Cin + 1) * g.Cout; }
 
-// 3-tap stacking needs 3*Cin+1 accumulator rows: UMMA M = 64 for Cin = 16, M = 128 for Cin = 32
-constexpr int wgrad_um(int cin) { return cin == 16 ? 64 : 128; }
-
-struct WPlan { int G, R, nbands, npix_alloc, kext, stage_planes; size_t smem; };
-static WPlan wgrad_plan(int H, int W, int cin, int cout) {
-  const int xpl = 3 * (cin / 8), WGRAD_UM = wgrad_um(cin);
-  const int Wp = W + 2, slack = 2 * Wp + 2;
-  WPlan p;
-  p.stage_planes = std::max(WGRAD_UM / 8, xpl + 1 + cout / 8);
-  const int total_planes = p.stage_planes + std::max(p.stage_planes, WGRAD_UM / 8);
-  const int maxpix = (216 * 1024) / (16 * total_planes);
-  if ((H + 2) * Wp + slack + 16 <= maxpix) {
-    p.R = H; p.nbands = 1; p.G = std::min(8, (maxpix - slack - 16) / ((H + 2) * Wp));
-  } else {
-    int rmax = (maxpix - slack - 16) / Wp - 2; if (rmax < 1) rmax = 1;
-    p.G = 1; p.nbands = (H + rmax - 1) / rmax; p.R = (H + p.nbands - 1) / p.nbands;
-  }
-  p.kext = (p.G * (p.R + 2) * Wp + 15) / 16 * 16;
-  p.npix_alloc = (p.kext + slack + 7) / 8 * 8;
-  p.smem = (size_t)total_planes * p.npix_alloc * 16;
-  return p;
-}
-
-template <int CIN, int COUT>
-static int launch_w(const tcw::WgradTcArgs& a, const CUtensorMap& xmap, const CUtensorMap& ymap, size_t smem, int grid, cudaStream_t st) {
-  { int rc = ensure_dyn_smem((const void*)tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true>, smem); if (rc) return rc; }
-  tcw::wgrad3x3_tc_kernel<CIN, COUT, wgrad_um(CIN), true><<<grid, tcw::NLOAD + 64, smem, st>>>(a, xmap, ymap);
-  CB_CUDA(cudaGetLastError());
-  return CB_OK;
-}
-
-// plan of the swizzled kernel: 2 stages of G whole frames (or one row band) in <= 208 KB (measured: two large stages beat three or
-// four smaller ones, the per-item hand-off costs more than the extra depth buys); a function of the shape only
 struct SwPlan { int G, R, nbands, npix_alloc, kext, nstages; size_t stage_bytes, y_off, smem; bool ok; int dy_off, x_off; };
 static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
   const int Wp = W + 2;
@@ -669,31 +356,8 @@ int launch_wgrad_tc(const Geom& g, const ParamMap& pm, int F, const bf16* x, con
       return CB_OK;
     }
   }
-  const int cin_k = g.Cin == 64 ? 32 : g.Cin;      // channels per kernel launch
-  WPlan p = wgrad_plan(g.H, g.W, cin_k, g.Cout);
-  if (p.smem > 224 * 1024) { set_error("wgrad_tc: plan does not fit shared memory"); return CB_EINVAL; }
-  const int nitems = ((F + p.G - 1) / p.G) * p.nbands;
-  const int grid = std::min(nitems, WGRAD_TC_MAX_CTAS);
-  // TMA boxes: X [8][W+2][R+2][G] started at (-1+dj, yb-1); DY [8][W+2][rows][G] started at (0, yb) with rows = R for banded
-  // plans (G = 1: the rows below the band must stay zero) and R+2 = H+2 for whole frames (out-of-bounds rows are zero-filled)
-  const int dy_rows = p.nbands > 1 ? p.R : p.R + 2;
-  CUtensorMap xmap, ymap; memset(&xmap, 0, sizeof xmap); memset(&ymap, 0, sizeof ymap);
-  const bool use_tma = g.W + 2 <= 256 && p.R + 2 <= 256 && tma::make_nhwc_map(&xmap, x, F, g.H, g.W, g.Cin, g.W + 2, p.R + 2, p.G) &&
-                       tma::make_nhwc_map(&ymap, dy, F, g.H, g.W, g.Cout, g.W + 2, dy_rows, p.G);
-  for (int c_off = 0; c_off < g.Cin; c_off += cin_k) {
-    tcw::WgradTcArgs a{x, dy, partial, F, g.H, g.W, p.G, p.R, p.nbands, p.npix_alloc, p.kext, relu_in ? 1 : 0, p.stage_planes, use_tma ? 1 : 0, dy_rows,
-                       use_tma ? 1 : 0, c_off, g.Cin, error_flag};
-    int rc;
-    if (cin_k == 16 && g.Cout == 16) rc = launch_w<16, 16>(a, xmap, ymap, p.smem, grid, st);
-    else if (cin_k == 16) rc = launch_w<16, 32>(a, xmap, ymap, p.smem, grid, st);
-    else if (g.Cout == 16) rc = launch_w<32, 16>(a, xmap, ymap, p.smem, grid, st);
-    else if (g.Cout == 32) rc = launch_w<32, 32>(a, xmap, ymap, p.smem, grid, st);
-    else rc = launch_w<32, 64>(a, xmap, ymap, p.smem, grid, st);
-    if (rc) return rc;
-    tcw::wgrad_tc_reduce_kernel<<<(tcw::RL * 9 * (cin_k + 1) * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, cin_k, c_off, grad);
-    CB_CUDA(cudaGetLastError());
-  }
-  return CB_OK;
+  set_error("wgrad_tc: no plan for this shape, or the driver refused a tensor map");
+  return CB_ECUDA;
 }
 
 }  // namespace cb

@@ -675,3 +675,20 @@ def test_stale_packed_weights_and_alignment_are_errors():
     with pytest.raises(binding.CleanbaError):
         net.policy_forward(dp, flat[1:1 + B * 4 * 84 * 84].view(B, 4, 84, 84), precision="bf16")      # obs not 4-byte aligned
     net.check_errors()
+
+
+def test_no_tma_fallback_kernels():
+    """What runs when the driver cannot encode tensor maps (cuTensorMapEncodeTiled missing, or CB_DISABLE_TMA=1): the TMA-fed tcgen05 kernels
+    report "unsupported" and every 3x3 / fc layer takes the SIMT implicit GEMM in bf16 storage (the first layer keeps its own tcgen05 kernel, which
+    stages through the LSU), under the same oracle checks.  The switch is read once per process, so the cases run in a child interpreter."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, CB_DISABLE_TMA="1")
+    sel = ["tests/test_gpu_learner.py::test_learner_impala_resnet_small", "tests/test_gpu_learner.py::test_learner_impala_wide_small",
+           "tests/test_gpu_learner.py::test_learner_ppo_resnet_bf16_tensor_core", "tests/test_gpu_learner.py::test_policy_forward_config1_shape"]
+    out = subprocess.run([sys.executable, "-m", "pytest", "-q", "-x", "-m", "gpu", "-k", "bf16 or wide or config1"] + sel, cwd=root, env=env,
+                         capture_output=True, text=True, timeout=1200)
+    assert out.returncode == 0, out.stdout[-3000:] + out.stderr[-2000:]
+    assert " passed" in out.stdout
