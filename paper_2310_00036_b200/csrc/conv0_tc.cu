@@ -262,6 +262,275 @@ __global__ void __launch_bounds__(256) conv0_fwd_kernel(const Args a) {
   if (warp == 0) tmem_dealloc(tmem_base, TMEM_COLS);
 }
 
+// stage_band with every global load of the thread issued BEFORE the first conversion (NQ quads of 4 pixels x CIN channels in registers):
+// the loader warps of the warp-specialised kernel are few, so their load latency must overlap within a thread
+// The same with 8-byte positions [c0 c1 c2 c3] (no constant-one channel, zero halo): the operand of the pixel-pair formulation below
+template <int NQ>
+__device__ __forceinline__ void stage_band8(const Args& a, uint8_t* xs, size_t fr, int yb, int tid, int nthr) {
+  const int Wp = a.W + 2, W4 = a.W / 4, rows = a.R + 2, nq = rows * W4;
+  const uint32_t magic_W4 = (uint32_t)((0x100000000ull + (uint64_t)W4 - 1) / (uint64_t)W4);
+  for (int base = 0; base < nq; base += NQ * nthr) {
+    uint32_t px[NQ][4]; int lrs[NQ], x0s[NQ];
+#pragma unroll
+    for (int j = 0; j < NQ; ++j) {
+      const int i = base + j * nthr + tid;
+      px[j][0] = px[j][1] = px[j][2] = px[j][3] = 0; lrs[j] = -1; x0s[j] = 0;
+      if (i < nq) {
+        const int lr = (int)__umulhi((uint32_t)i, magic_W4), x0 = (i - lr * W4) * 4, y = yb - 1 + lr;
+        lrs[j] = lr; x0s[j] = x0;
+        if ((unsigned)y < (unsigned)a.H) {
+#pragma unroll
+          for (int c = 0; c < 4; ++c) if (c < a.CIN) px[j][c] = pool::ldg_early_u32(a.obs + ((fr * a.CIN + c) * a.H + y) * a.W + x0);
+        }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < NQ; ++j) {
+      if (lrs[j] < 0) continue;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const float v0 = (float)((px[j][0] >> (8 * k)) & 255u), v1 = (float)((px[j][1] >> (8 * k)) & 255u);
+        const float v2 = (float)((px[j][2] >> (8 * k)) & 255u), v3 = (float)((px[j][3] >> (8 * k)) & 255u);
+        __nv_bfloat162 p01 = __floats2bfloat162_rn(v0, v1), p23 = __floats2bfloat162_rn(v2, v3);
+        uint2 o; o.x = *reinterpret_cast<uint32_t*>(&p01); o.y = *reinterpret_cast<uint32_t*>(&p23);
+        *reinterpret_cast<uint2*>(xs + (size_t)(lrs[j] * Wp + x0s[j] + 1 + k) * 8) = o;
+      }
+    }
+  }
+  for (int i = tid; i < rows * 2; i += nthr) {       // halo columns
+    int lr = i >> 1, xp = (i & 1) ? Wp - 1 : 0;
+    *reinterpret_cast<uint2*>(xs + (size_t)(lr * Wp + xp) * 8) = make_uint2(0, 0);
+  }
+}
+
+template <int NQ>
+__device__ __forceinline__ void stage_band_batched(const Args& a, uint8_t* xs, size_t fr, int yb, int tid, int nthr) {
+  const int Wp = a.W + 2, W4 = a.W / 4, rows = a.R + 2, nq = rows * W4;
+  const uint32_t ONE = 0x3F80u;
+  const uint32_t magic_W4 = (uint32_t)((0x100000000ull + (uint64_t)W4 - 1) / (uint64_t)W4);
+  for (int base = 0; base < nq; base += NQ * nthr) {
+    uint32_t px[NQ][4]; int lrs[NQ], x0s[NQ];
+#pragma unroll
+    for (int j = 0; j < NQ; ++j) {
+      const int i = base + j * nthr + tid;
+      px[j][0] = px[j][1] = px[j][2] = px[j][3] = 0; lrs[j] = -1; x0s[j] = 0;
+      if (i < nq) {
+        const int lr = (int)__umulhi((uint32_t)i, magic_W4), x0 = (i - lr * W4) * 4, y = yb - 1 + lr;
+        lrs[j] = lr; x0s[j] = x0;
+        if ((unsigned)y < (unsigned)a.H) {
+#pragma unroll
+          for (int c = 0; c < 4; ++c) if (c < a.CIN) px[j][c] = pool::ldg_early_u32(a.obs + ((fr * a.CIN + c) * a.H + y) * a.W + x0);
+        }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < NQ; ++j) {
+      if (lrs[j] < 0) continue;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const float v0 = (float)((px[j][0] >> (8 * k)) & 255u), v1 = (float)((px[j][1] >> (8 * k)) & 255u);
+        const float v2 = (float)((px[j][2] >> (8 * k)) & 255u), v3 = (float)((px[j][3] >> (8 * k)) & 255u);
+        __nv_bfloat162 p01 = __floats2bfloat162_rn(v0, v1), p23 = __floats2bfloat162_rn(v2, v3);
+        uint4 o; o.x = *reinterpret_cast<uint32_t*>(&p01); o.y = *reinterpret_cast<uint32_t*>(&p23); o.z = ONE; o.w = 0;
+        *reinterpret_cast<uint4*>(xs + (size_t)(lrs[j] * Wp + x0s[j] + 1 + k) * 16) = o;
+      }
+    }
+  }
+  for (int i = tid; i < rows * 2; i += nthr) {       // halo columns
+    int lr = i >> 1, xp = (i & 1) ? Wp - 1 : 0;
+    *reinterpret_cast<uint4*>(xs + (size_t)(lr * Wp + xp) * 16) = make_uint4(0, 0, ONE, 0);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Warp-specialised form of the fused first layer (conv 3x3 + max-pool 3x3 s2), one persistent CTA per SM.  An item is a band of Rp pooled
+// rows of one frame (R = 2 Rp + 1 conv rows).
+// PIXEL PAIRS: a position is 8 bytes [c0 c1 c2 c3] and an A row is the PAIR of output positions (2r, 2r+1) (Wp is even, so a pair never
+// straddles an image row): for tap row di the pair needs the four input positions 2r + di Wp .. + 3 = 32 contiguous bytes = the two
+// 16-byte K chunks of one K = 16 MMA (rows 16 bytes apart: LBO = 16 B, SBO = 128 B), against block-Toeplitz weights [16 x 2 Cout] (pixel e of
+// the pair uses positions e .. e+2).  THREE MMAs per 256 positions instead of twelve, and a quarter of the operand bytes read from shared
+// memory -- the kernel was bound by the shared-memory port (operand reads of the tensor core + epilogue stores + pool loads), not by issue.  Four roles hand items to each other through mbarriers, each two items deep, so that staging,
+// tensor-core work, accumulator drain and pooling of DIFFERENT items overlap (the CTA-wide barriers of conv0_fwd_kernel serialised them):
+//   warps 0-3    loaders:  uint8 frame rows -> bf16 positions of plane[s]                     PFULL[s] (4 arrivals)   <- PEMPTY[s] (MMA commit)
+//   warp  4      MMA:      all tiles of the item into TMEM buffer s (256 columns each)        TFULL[s] (commit)       <- TEMPTY[s] (8 arrivals)
+//   warps 5-12   epilogue: TMEM -> x 1/255 + bias -> bf16 conv band ctile[s]                  CFULL[s] (8 arrivals)   <- CEMPTY[s] (NPOOL arrivals)
+//   warps 13-24  pool (the heaviest role: ~200 instructions per 8-channel window):     3x3 s2 SAME max + first arg-max (A10, A11) -> pooled map, arg-max bytes
+constexpr int WS_LOAD_WARPS = 4, WS_EPI_WARPS = 8, WS_POOL_WARPS = 12, WS_THREADS = (WS_LOAD_WARPS + 1 + WS_EPI_WARPS + WS_POOL_WARPS) * 32;
+struct WsArgs { Args a; uint32_t plane_bytes, ctile_bytes; };
+// Bank-conflict-free layout of the conv band: inside every 64-byte block (a pixel pair at 16 channels, one pixel at 32) the 16-byte chunk
+// c sits at c ^ bitrev2((block >> 1) & 3).  The epilogue's lanes (64 / 128 bytes apart) and the pool's lanes (one or two pixels apart) then
+// spread over all eight 16-byte bank groups instead of hitting two of them (measured before: 61 % of the shared-memory wavefronts were replays).
+__device__ __forceinline__ uint32_t ct_swz(uint32_t byte_off) {
+  const uint32_t v = (byte_off >> 7) & 3u;
+  return byte_off ^ ((((v & 1u) << 1) | (v >> 1)) << 4);
+}
+
+__device__ __forceinline__ void mbar_arrive_cta(uint32_t bar) {
+  asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
+}
+
+template <int COUT>
+__global__ void __launch_bounds__(WS_THREADS, 1) conv0_fwd_ws_kernel(const WsArgs wa) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  const Args& a = wa.a;
+  constexpr uint32_t W_BYTES = 3u * 2u * (2u * COUT) * 16u;      // [di][chunk][2 Cout][8]
+  __shared__ __align__(8) uint64_t bars[12];      // PFULL[2] PEMPTY[2] TFULL[2] TEMPTY[2] CFULL[2] CEMPTY[2]
+  __shared__ uint32_t tmem_base_smem;
+  __shared__ __align__(16) float bias_s[32];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, Wp = a.W + 2;
+  const uint32_t bar0 = smem_u32(&bars[0]);
+  auto PFULL = [&](int s) { return bar0 + 8u * (uint32_t)s; };        auto PEMPTY = [&](int s) { return bar0 + 8u * (uint32_t)(2 + s); };
+  auto TFULL = [&](int s) { return bar0 + 8u * (uint32_t)(4 + s); };  auto TEMPTY = [&](int s) { return bar0 + 8u * (uint32_t)(6 + s); };
+  auto CFULL = [&](int s) { return bar0 + 8u * (uint32_t)(8 + s); };  auto CEMPTY = [&](int s) { return bar0 + 8u * (uint32_t)(10 + s); };
+  uint8_t* w_smem = smem; uint8_t* planes = smem + W_BYTES; uint8_t* ctiles = planes + 2 * (size_t)wa.plane_bytes;
+  if (tid == 0) {
+    for (int s = 0; s < 2; ++s) {
+      mbar_init(PFULL(s), WS_LOAD_WARPS); mbar_init(PEMPTY(s), 1); mbar_init(TFULL(s), 1); mbar_init(TEMPTY(s), WS_EPI_WARPS);
+      mbar_init(CFULL(s), WS_EPI_WARPS); mbar_init(CEMPTY(s), WS_POOL_WARPS);
+    }
+  }
+  if (tid < COUT) bias_s[tid] = a.bias[tid];
+  if (warp == WS_LOAD_WARPS) tmem_alloc(smem_u32(&tmem_base_smem), 512);
+  for (uint32_t i = tid; i < W_BYTES / 16; i += WS_THREADS) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w + 6 * 2 * COUT * 8)[i];      // the pair image follows the per-pixel one
+  for (uint32_t i = tid; i < 2 * wa.plane_bytes / 16; i += WS_THREADS) reinterpret_cast<uint4*>(planes)[i] = make_uint4(0, 0, 0, 0);
+  fence_async_smem();
+  tc_fence_before(); __syncthreads(); tc_fence_after();
+  const uint32_t tmem_base = tmem_base_smem;
+  const int nitems = a.F * a.nbands;
+  const int my_items = ((int)blockIdx.x < nitems) ? (nitems - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+  const int Ho = (a.H + 1) / 2, Wo = (a.W + 1) / 2;
+  int th_ = (Ho - 1) * 2 + 3 - a.H; if (th_ < 0) th_ = 0; const int ph = th_ / 2;
+  int tw_ = (Wo - 1) * 2 + 3 - a.W; if (tw_ < 0) tw_ = 0; const int pw = tw_ / 2;
+  const int ntiles = (a.R * Wp + 255) / 256;      // 128 position pairs per tile
+  auto item_geom = [&](int it, int& f, int& py0, int& yb) {
+    const int item = blockIdx.x + it * gridDim.x; f = item / a.nbands; const int band = item - f * a.nbands;
+    py0 = band * a.Rp; yb = max(0, 2 * py0 - ph);
+  };
+
+  if (warp < WS_LOAD_WARPS) {
+    // ================= loaders =================
+    for (int it = 0; it < my_items; ++it) {
+      const int s = it & 1, use = it >> 1; int f, py0, yb; item_geom(it, f, py0, yb);
+      if (use > 0 && !mbar_wait(PEMPTY(s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 3; }
+      const size_t fr = a.frame_idx ? (size_t)a.frame_idx[f] : (size_t)f;
+      stage_band8<5>(a, planes + (size_t)s * wa.plane_bytes, fr, yb, tid, WS_LOAD_WARPS * 32);
+      fence_async_smem();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cta(PFULL(s));
+    }
+  } else if (warp == WS_LOAD_WARPS) {
+    // ================= MMA issuer =================
+    const uint32_t idesc = make_idesc(128, 2 * COUT, 0, 0);
+    const uint32_t b_lo = ((smem_u32(w_smem) >> 4) & 0x3FFFu) | ((uint32_t)(2 * COUT) << 16), hi = 8u | (1u << 14);   // B: LBO 2 Cout * 16 B, SBO 128 B;  A: LBO 16 B, SBO 128 B
+    for (int it = 0; it < my_items; ++it) {
+      const int s = it & 1, use = it >> 1;
+      if (!mbar_wait(PFULL(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 3; }
+      if (use > 0 && !mbar_wait(TEMPTY(s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 3; }
+      tc_fence_after();
+      const uint32_t a_lo = (((smem_u32(planes) + (uint32_t)s * wa.plane_bytes) >> 4) & 0x3FFFu) | (1u << 16);
+      for (int t = 0; t < ntiles; ++t) {
+        const uint32_t td = tmem_base + (uint32_t)(s * 256 + t * 2 * COUT);
+#pragma unroll
+        for (int di = 0; di < 3; ++di) {
+          const uint32_t pos = (uint32_t)(t * 256 + di * Wp);                  // first input position of the tile's first pair: even, so pos * 8 bytes is a multiple of 16
+          const uint64_t ad = ((uint64_t)hi << 32) | (uint64_t)(a_lo + (pos >> 1));
+          const uint64_t bd = ((uint64_t)hi << 32) | (uint64_t)(b_lo + (uint32_t)di * 2u * (2u * COUT));
+          if (elect_one()) mma_f16(td, ad, bd, idesc, di ? 1u : 0u);
+        }
+      }
+      if (elect_one()) { mma_commit(TFULL(s)); mma_commit(PEMPTY(s)); }
+      __syncwarp();
+    }
+  } else if (warp < WS_LOAD_WARPS + 1 + WS_EPI_WARPS) {
+    // ================= epilogue: warp e drains lanes 32 (e % 4) .. +31 of every second tile =================
+    const int e = warp - (WS_LOAD_WARPS + 1), q4 = warp & 3, half = e >> 2;      // TMEM lane quarter = warp index % 4 (hardware rule)
+    const uint32_t magic_Wp = (uint32_t)((0x100000000ull + (uint64_t)Wp - 1) / (uint64_t)Wp);
+    for (int it = 0; it < my_items; ++it) {
+      const int s = it & 1, use = it >> 1; int f, py0, yb; item_geom(it, f, py0, yb);
+      if (!mbar_wait(TFULL(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 3; }
+      if (use > 0 && !mbar_wait(CEMPTY(s), (uint32_t)((use - 1) & 1))) { if (a.error_flag) *a.error_flag = 3; }
+      tc_fence_after();
+      bf16* ct = reinterpret_cast<bf16*>(ctiles + (size_t)s * wa.ctile_bytes);
+      for (int t = half; t < ntiles; t += 2) {
+        const int q = t * 256 + 2 * (q4 * 32 + lane), yl = (int)__umulhi((uint32_t)q, magic_Wp), x = q - yl * Wp, y = yb + yl;      // the pair (q, q+1): same image row
+        const bool rowok = yl < a.R && y < a.H;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const bool valid = rowok && x + e < a.W;
+#pragma unroll
+          for (int c0 = 0; c0 < COUT; c0 += 16) {
+            float v[16];
+            tmem_ld16(tmem_base + ((uint32_t)(q4 * 32) << 16) + (uint32_t)(s * 256 + t * 2 * COUT + e * COUT + c0), v);
+            if (!valid) continue;
+            uint4 o0, o1;
+            __nv_bfloat162* p0 = reinterpret_cast<__nv_bfloat162*>(&o0); __nv_bfloat162* p1 = reinterpret_cast<__nv_bfloat162*>(&o1);
+#pragma unroll
+            for (int i = 0; i < 16; i += 4) {
+              const float4 b4 = *reinterpret_cast<const float4*>(bias_s + c0 + i);
+              v[i] = fmaf(v[i], 1.0f / 255.0f, b4.x); v[i + 1] = fmaf(v[i + 1], 1.0f / 255.0f, b4.y); v[i + 2] = fmaf(v[i + 2], 1.0f / 255.0f, b4.z); v[i + 3] = fmaf(v[i + 3], 1.0f / 255.0f, b4.w);
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
+            const uint32_t off = (uint32_t)(((yl * a.W + x + e) * COUT + c0) * 2);
+            *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(ct) + ct_swz(off)) = o0;
+            *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(ct) + ct_swz(off + 16)) = o1;
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) { mbar_arrive_cta(TEMPTY(s)); mbar_arrive_cta(CFULL(s)); }
+    }
+  } else {
+    // ================= pool =================
+    const int pt = tid - (WS_LOAD_WARPS + 1 + WS_EPI_WARPS) * 32;
+    constexpr int C8 = COUT / 8, NP = WS_POOL_WARPS * 32;
+    const uint32_t magic_Wo = (uint32_t)((0x100000000ull + (uint64_t)Wo - 1) / (uint64_t)Wo);
+    for (int it = 0; it < my_items; ++it) {
+      const int s = it & 1, use = it >> 1; int f, py0, yb; item_geom(it, f, py0, yb);
+      if (!mbar_wait(CFULL(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 3; }
+      const bf16* ct = reinterpret_cast<const bf16*>(ctiles + (size_t)s * wa.ctile_bytes);
+      const int pr = min(a.Rp, Ho - py0);
+      for (int i = pt; i < pr * Wo * C8; i += NP) {
+        const int c8 = i % C8, q = i / C8, qy = (int)__umulhi((uint32_t)q, magic_Wo), ox = q - qy * Wo, oy = py0 + qy;
+        uint4 v[9]; uint32_t valid = 0;
+        const int iy0 = oy * 2 - ph, ix0 = ox * 2 - pw;
+        const uint8_t* ctb = reinterpret_cast<const uint8_t*>(ct);
+        if (iy0 >= 0 && iy0 + 2 < a.H && ix0 >= 0 && ix0 + 2 < a.W) {      // interior window (all but the border ones): no per-tap predicates
+          const uint32_t base = (uint32_t)((((iy0 - yb) * a.W + ix0) * COUT + c8 * 8) * 2), rowp = (uint32_t)(a.W * COUT * 2);
+#pragma unroll
+          for (int di = 0; di < 3; ++di)
+#pragma unroll
+            for (int dj = 0; dj < 3; ++dj) v[di * 3 + dj] = *reinterpret_cast<const uint4*>(ctb + ct_swz(base + di * rowp + dj * COUT * 2));
+          valid = 0x1FFu;
+        } else {
+#pragma unroll
+          for (int di = 0; di < 3; ++di) {
+            const int iy = iy0 + di;
+#pragma unroll
+            for (int dj = 0; dj < 3; ++dj) {
+              const int ix = ix0 + dj;
+              if ((unsigned)iy < (unsigned)a.H && (unsigned)ix < (unsigned)a.W) {
+                v[di * 3 + dj] = *reinterpret_cast<const uint4*>(ctb + ct_swz((uint32_t)((((iy - yb) * a.W + ix) * COUT + c8 * 8) * 2)));
+                valid |= 1u << (di * 3 + dj);
+              }
+            }
+          }
+        }
+        const size_t o = (((size_t)f * Ho + oy) * Wo + ox) * COUT + c8 * 8;
+        uint4 r; uint2 pk;
+        pool::window_max(v, valid, r, pk);
+        *reinterpret_cast<uint4*>(a.pool_out + o) = r;
+        *reinterpret_cast<uint2*>(a.pool_arg_out + o) = pk;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cta(CEMPTY(s));
+    }
+  }
+  tc_fence_before(); __syncthreads();
+  if (warp == WS_LOAD_WARPS) tmem_dealloc(tmem_base, 512);
+}
+
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
 }
@@ -439,7 +708,7 @@ bool conv0_tc_supported(const Geom& g) {
 }
 constexpr int CONV0_MAX_CTAS = 148;
 size_t conv0_partial_elems(const Geom& g) { return (size_t)CONV0_MAX_CTAS * 3 * 24 * g.Cout; }
-size_t conv0_wimg_elems(const Geom& g) { return (size_t)6 * 2 * g.Cout * 8; }
+size_t conv0_wimg_elems(const Geom& g) { return (size_t)2 * 6 * 2 * g.Cout * 8; }      // two images of 96 Cout elements: [6][2][Cout][8] (one pixel per row) and [3][2][2 Cout][8] (pixel pairs)
 
 int launch_conv0_pack(const Geom& g, const ParamMap& pm, const float* params, bf16* wimg, cudaStream_t st) {
   tc0::conv0_pack_kernel<<<(6 * 2 * g.Cout * 8 + 255) / 256, 256, 0, st>>>(params, g, pm, wimg);
@@ -465,6 +734,25 @@ int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* fr
   } else {
     R = std::min(g.H, (90 * 1024 / 16 - 2 * Wp - 130) / Wp - 2); if (R < 1) R = 1;
     nb = (g.H + R - 1) / R; R = (g.H + nb - 1) / nb;
+  }
+  if (pool_out) {
+    // warp-specialised kernel: bands of Rp pooled rows whose tiles fit one 256-column TMEM buffer, two planes + two conv bands in shared memory
+    const int Ho = (g.H + 1) / 2;
+    auto tiles_of = [&](int rp) { return ((2 * rp + 1) * Wp + 255) / 256; };      // 128 position pairs per tile
+    auto npix_of = [&](int rp) { return (tiles_of(rp) * 256 + 2 * Wp + 16 + 15) / 16 * 16; };        // 8-byte positions (a multiple of 128 bytes); the last tile's MMAs read up to 2 Wp + 3 positions further
+    auto smem_of = [&](int rp) { return (size_t)3 * 2 * 2 * g.Cout * 16 + 2 * (size_t)npix_of(rp) * 8 + 2 * (size_t)(2 * rp + 1) * g.W * g.Cout * 2; };
+    int rp = 1; while (rp < Ho && tiles_of(rp + 1) * 2 * g.Cout <= 256 && smem_of(rp + 1) <= (size_t)200 * 1024) ++rp;
+    if (Wp % 2 == 0 && tiles_of(rp) * 2 * g.Cout <= 256 && smem_of(rp) <= (size_t)200 * 1024) {
+      const int nbw = (Ho + rp - 1) / rp; rp = (Ho + nbw - 1) / nbw;      // equal bands
+      const int Rw = 2 * rp + 1, npw = npix_of(rp);
+      tc0::WsArgs wa{{obs, frame_idx, wimg, bias, out, nullptr, nullptr, nullptr, nullptr, F, g.H, g.W, g.Cin, Rw, nbw, npw, 0, 0, 0, 0, pool_out, pool_arg, rp, error_flag},
+                     (uint32_t)npw * 8u, (uint32_t)((size_t)Rw * g.W * g.Cout * 2)};
+      const int gridw = std::min(F * nbw, 148); int rcw;
+      if (g.Cout == 16) { if ((rcw = ensure_dyn_smem((const void*)tc0::conv0_fwd_ws_kernel<16>, smem_of(rp)))) return rcw; tc0::conv0_fwd_ws_kernel<16><<<gridw, tc0::WS_THREADS, smem_of(rp), st>>>(wa); }
+      else { if ((rcw = ensure_dyn_smem((const void*)tc0::conv0_fwd_ws_kernel<32>, smem_of(rp)))) return rcw; tc0::conv0_fwd_ws_kernel<32><<<gridw, tc0::WS_THREADS, smem_of(rp), st>>>(wa); }
+      CB_CUDA(cudaGetLastError());
+      return CB_OK;
+    }
   }
   const int npix = ((R * Wp + 127) / 128) * 128 + 2 * Wp + 8;
   const size_t smem = (size_t)6 * 2 * g.Cout * 16 + (size_t)npix * 16 + ctile;

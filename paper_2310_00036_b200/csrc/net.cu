@@ -101,6 +101,15 @@ __global__ void pack_all_kernel(const float* __restrict__ params, const PackDesc
       float v = (c < g.Cin && dj < 3) ? params[d.pm.w(o, c, di, dj, g)] : 0.f;
       w0img[i] = __float2bfloat16_rn(v);
     }
+    // pixel-pair image (conv0_fwd_ws_kernel): [di][chunk][n = e Cout + o][8]; K index kk = 8 chunk + col = 4 j + c (input position j of the four a
+    // pair reads, channel c); pixel e of the pair sees position j as tap dj = j - e
+    bf16* img2 = w0img + tot0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < tot0; i += gridDim.x * blockDim.x) {
+      const int col = i & 7, n = (i >> 3) % (2 * g.Cout), chunk = ((i >> 3) / (2 * g.Cout)) & 1, di = (i >> 3) / (2 * g.Cout) / 2;
+      const int kk = 8 * chunk + col, j = kk >> 2, c = kk & 3, e = n / g.Cout, o = n - e * g.Cout, dj = j - e;
+      const float v = (c < g.Cin && dj >= 0 && dj < 3) ? params[d.pm.w(o, c, di, dj, g)] : 0.f;
+      img2[i] = __float2bfloat16_rn(v);
+    }
   }
 }
 
