@@ -9,6 +9,8 @@
 #include <stdint.h>
 #include <stddef.h>
 #include <algorithm>
+#include <cstring>
+#include <utility>
 #include <cmath>
 #include <string>
 #include <vector>
@@ -159,6 +161,10 @@ bool conv_tc_fits(int H, int W, int cin, int cout);
 int launch_conv_tc(int mode, int F, int H, int W, int cin, int cout, const bf16* in, const bf16* w, const float* bias, const bf16* aux0,
                    const bf16* aux1, bf16* out, bool relu_in, bool relu_out, int* error_flag, cudaStream_t st);
 
+// conv_pool_tc.cu: stage conv + the max-pool that follows it in one kernel (forward)
+bool conv_pool_tc_supported(const Geom& g);
+int launch_conv_pool_tc(const Geom& g, int F, const bf16* in, const bf16* w, const float* bias, bf16* pool_out, uint8_t* pool_arg, int* error_flag, cudaStream_t st);
+
 // wgrad_tc.cu
 bool wgrad_tc_supported(const Geom& g);
 size_t wgrad_tc_partial_elems(const Geom& g);
@@ -211,6 +217,17 @@ int launch_sum_ranks(const float* in, int G, size_t n, float scale, float* out, 
 int launch_env_reset(uint64_t seed, int B, int C, int H, int W, int32_t* state, uint8_t* obs, cudaStream_t st);
 int launch_env_step(uint64_t seed, int B, int C, int H, int W, uint32_t g, const int32_t* actions, int32_t* state, const uint8_t* obs_in, uint8_t* out0,
                     uint8_t* out1, float* rewards, uint8_t* dones, cudaStream_t st);
+// Launch with the programmatic-stream-serialization attribute: the kernel MUST call ptx::pdl_wait() before it touches memory written by
+// earlier work (tc_ptx.cuh).  Hides the launch gap and the prologue of the persistent tensor-core kernels behind the tail of their predecessor.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg; memset(&cfg, 0, sizeof cfg);
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization; attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
 // one opt-in per (device, kernel): cudaFuncAttributeMaxDynamicSharedMemorySize raised to at least `bytes`
 int ensure_dyn_smem(const void* func, size_t bytes);
 // loss kernels write dhead [N, A+1] in the mode's storage type and per-sample terms; reduce writes stats

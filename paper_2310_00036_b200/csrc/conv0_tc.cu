@@ -357,14 +357,6 @@ __device__ __forceinline__ void stage_band_batched(const Args& a, uint8_t* xs, s
 //   warps 13-24  pool (the heaviest role: ~200 instructions per 8-channel window):     3x3 s2 SAME max + first arg-max (A10, A11) -> pooled map, arg-max bytes
 constexpr int WS_LOAD_WARPS = 4, WS_EPI_WARPS = 8, WS_POOL_WARPS = 12, WS_THREADS = (WS_LOAD_WARPS + 1 + WS_EPI_WARPS + WS_POOL_WARPS) * 32;
 struct WsArgs { Args a; uint32_t plane_bytes, ctile_bytes; };
-// Bank-conflict-free layout of the conv band: inside every 64-byte block (a pixel pair at 16 channels, one pixel at 32) the 16-byte chunk
-// c sits at c ^ bitrev2((block >> 1) & 3).  The epilogue's lanes (64 / 128 bytes apart) and the pool's lanes (one or two pixels apart) then
-// spread over all eight 16-byte bank groups instead of hitting two of them (measured before: 61 % of the shared-memory wavefronts were replays).
-__device__ __forceinline__ uint32_t ct_swz(uint32_t byte_off) {
-  const uint32_t v = (byte_off >> 7) & 3u;
-  return byte_off ^ ((((v & 1u) << 1) | (v >> 1)) << 4);
-}
-
 __device__ __forceinline__ void mbar_arrive_cta(uint32_t bar) {
   asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}\n" :: "r"(bar) : "memory");
 }
@@ -389,10 +381,11 @@ __global__ void __launch_bounds__(WS_THREADS, 1) conv0_fwd_ws_kernel(const WsArg
       mbar_init(CFULL(s), WS_EPI_WARPS); mbar_init(CEMPTY(s), WS_POOL_WARPS);
     }
   }
-  if (tid < COUT) bias_s[tid] = a.bias[tid];
   if (warp == WS_LOAD_WARPS) tmem_alloc(smem_u32(&tmem_base_smem), 512);
-  for (uint32_t i = tid; i < W_BYTES / 16; i += WS_THREADS) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w + 6 * 2 * COUT * 8)[i];      // the pair image follows the per-pixel one
   for (uint32_t i = tid; i < 2 * wa.plane_bytes / 16; i += WS_THREADS) reinterpret_cast<uint4*>(planes)[i] = make_uint4(0, 0, 0, 0);
+  pdl_wait(); pdl_trigger();
+  if (tid < COUT) bias_s[tid] = a.bias[tid];
+  for (uint32_t i = tid; i < W_BYTES / 16; i += WS_THREADS) reinterpret_cast<uint4*>(w_smem)[i] = reinterpret_cast<const uint4*>(a.w + 6 * 2 * COUT * 8)[i];      // the pair image follows the per-pixel one
   fence_async_smem();
   tc_fence_before(); __syncthreads(); tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
@@ -472,8 +465,8 @@ __global__ void __launch_bounds__(WS_THREADS, 1) conv0_fwd_ws_kernel(const WsArg
 #pragma unroll
             for (int i = 0; i < 4; ++i) { p0[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]); p1[i] = __floats2bfloat162_rn(v[8 + 2 * i], v[8 + 2 * i + 1]); }
             const uint32_t off = (uint32_t)(((yl * a.W + x + e) * COUT + c0) * 2);
-            *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(ct) + ct_swz(off)) = o0;
-            *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(ct) + ct_swz(off + 16)) = o1;
+            *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(ct) + pool::ct_swz<COUT>(off)) = o0;
+            *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(ct) + pool::ct_swz<COUT>(off + 16)) = o1;
           }
         }
       }
@@ -484,45 +477,11 @@ __global__ void __launch_bounds__(WS_THREADS, 1) conv0_fwd_ws_kernel(const WsArg
   } else {
     // ================= pool =================
     const int pt = tid - (WS_LOAD_WARPS + 1 + WS_EPI_WARPS) * 32;
-    constexpr int C8 = COUT / 8, NP = WS_POOL_WARPS * 32;
-    const uint32_t magic_Wo = (uint32_t)((0x100000000ull + (uint64_t)Wo - 1) / (uint64_t)Wo);
+    constexpr int NP = WS_POOL_WARPS * 32;
     for (int it = 0; it < my_items; ++it) {
       const int s = it & 1, use = it >> 1; int f, py0, yb; item_geom(it, f, py0, yb);
       if (!mbar_wait(CFULL(s), (uint32_t)(use & 1))) { if (a.error_flag) *a.error_flag = 3; }
-      const bf16* ct = reinterpret_cast<const bf16*>(ctiles + (size_t)s * wa.ctile_bytes);
-      const int pr = min(a.Rp, Ho - py0);
-      for (int i = pt; i < pr * Wo * C8; i += NP) {
-        const int c8 = i % C8, q = i / C8, qy = (int)__umulhi((uint32_t)q, magic_Wo), ox = q - qy * Wo, oy = py0 + qy;
-        uint4 v[9]; uint32_t valid = 0;
-        const int iy0 = oy * 2 - ph, ix0 = ox * 2 - pw;
-        const uint8_t* ctb = reinterpret_cast<const uint8_t*>(ct);
-        if (iy0 >= 0 && iy0 + 2 < a.H && ix0 >= 0 && ix0 + 2 < a.W) {      // interior window (all but the border ones): no per-tap predicates
-          const uint32_t base = (uint32_t)((((iy0 - yb) * a.W + ix0) * COUT + c8 * 8) * 2), rowp = (uint32_t)(a.W * COUT * 2);
-#pragma unroll
-          for (int di = 0; di < 3; ++di)
-#pragma unroll
-            for (int dj = 0; dj < 3; ++dj) v[di * 3 + dj] = *reinterpret_cast<const uint4*>(ctb + ct_swz(base + di * rowp + dj * COUT * 2));
-          valid = 0x1FFu;
-        } else {
-#pragma unroll
-          for (int di = 0; di < 3; ++di) {
-            const int iy = iy0 + di;
-#pragma unroll
-            for (int dj = 0; dj < 3; ++dj) {
-              const int ix = ix0 + dj;
-              if ((unsigned)iy < (unsigned)a.H && (unsigned)ix < (unsigned)a.W) {
-                v[di * 3 + dj] = *reinterpret_cast<const uint4*>(ctb + ct_swz((uint32_t)((((iy - yb) * a.W + ix) * COUT + c8 * 8) * 2)));
-                valid |= 1u << (di * 3 + dj);
-              }
-            }
-          }
-        }
-        const size_t o = (((size_t)f * Ho + oy) * Wo + ox) * COUT + c8 * 8;
-        uint4 r; uint2 pk;
-        pool::window_max(v, valid, r, pk);
-        *reinterpret_cast<uint4*>(a.pool_out + o) = r;
-        *reinterpret_cast<uint2*>(a.pool_arg_out + o) = pk;
-      }
+      pool::pool_band<COUT>(ctiles + (size_t)s * wa.ctile_bytes, yb, py0, min(a.Rp, Ho - py0), f, a.H, a.W, Ho, Wo, ph, pw, a.pool_out, a.pool_arg_out, pt, NP);
       __syncwarp();
       if (lane == 0) mbar_arrive_cta(CEMPTY(s));
     }
@@ -562,6 +521,7 @@ __global__ void __launch_bounds__(WNLOAD + 32) conv0_wgrad_kernel(const Args a) 
     for (uint32_t i = tid; i < XB / 16; i += WNLOAD + 32) reinterpret_cast<uint4*>(xs)[i] = make_uint4(0, 0, 0x3F80u, 0);
     for (uint32_t i = tid; i < (uint32_t)a.w_ybytes / 16; i += WNLOAD + 32) reinterpret_cast<uint4*>(xs + XB)[i] = make_uint4(0, 0, 0, 0);
   }
+  pdl_wait(); pdl_trigger();      // the prologue above is private to the CTA (tc_ptx.cuh)
   fence_async_smem();
   tc_fence_before(); __syncthreads(); tc_fence_after();
   const uint32_t tmem_base = tmem_base_smem;
@@ -748,8 +708,8 @@ int launch_conv0_fwd(const Geom& g, int F, const uint8_t* obs, const int32_t* fr
       tc0::WsArgs wa{{obs, frame_idx, wimg, bias, out, nullptr, nullptr, nullptr, nullptr, F, g.H, g.W, g.Cin, Rw, nbw, npw, 0, 0, 0, 0, pool_out, pool_arg, rp, error_flag},
                      (uint32_t)npw * 8u, (uint32_t)((size_t)Rw * g.W * g.Cout * 2)};
       const int gridw = std::min(F * nbw, 148); int rcw;
-      if (g.Cout == 16) { if ((rcw = ensure_dyn_smem((const void*)tc0::conv0_fwd_ws_kernel<16>, smem_of(rp)))) return rcw; tc0::conv0_fwd_ws_kernel<16><<<gridw, tc0::WS_THREADS, smem_of(rp), st>>>(wa); }
-      else { if ((rcw = ensure_dyn_smem((const void*)tc0::conv0_fwd_ws_kernel<32>, smem_of(rp)))) return rcw; tc0::conv0_fwd_ws_kernel<32><<<gridw, tc0::WS_THREADS, smem_of(rp), st>>>(wa); }
+      if (g.Cout == 16) { if ((rcw = ensure_dyn_smem((const void*)tc0::conv0_fwd_ws_kernel<16>, smem_of(rp)))) return rcw; CB_CUDA(launch_pdl(tc0::conv0_fwd_ws_kernel<16>, dim3(gridw), dim3(tc0::WS_THREADS), smem_of(rp), st, wa)); }
+      else { if ((rcw = ensure_dyn_smem((const void*)tc0::conv0_fwd_ws_kernel<32>, smem_of(rp)))) return rcw; CB_CUDA(launch_pdl(tc0::conv0_fwd_ws_kernel<32>, dim3(gridw), dim3(tc0::WS_THREADS), smem_of(rp), st, wa)); }
       CB_CUDA(cudaGetLastError());
       return CB_OK;
     }
@@ -784,8 +744,8 @@ int launch_conv0_wgrad(const Geom& g, const ParamMap& pm, int F, const uint8_t* 
   tc0::Args a{obs, frame_idx, nullptr, nullptr, nullptr, dy, partial, pool_arg, dpool, F, g.H, g.W, g.Cin, R, nb, npix, kext, xoff, yoff, (int)ybytes,
               nullptr, nullptr, 0, error_flag};
   static size_t c16 = 0, c32 = 0; int rc;
-  if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_wgrad_kernel<16>, smem, &c16))) return rc; tc0::conv0_wgrad_kernel<16><<<grid, tc0::WNLOAD + 32, smem, st>>>(a); }
-  else { if ((rc = set_smem(tc0::conv0_wgrad_kernel<32>, smem, &c32))) return rc; tc0::conv0_wgrad_kernel<32><<<grid, tc0::WNLOAD + 32, smem, st>>>(a); }
+  if (g.Cout == 16) { if ((rc = set_smem(tc0::conv0_wgrad_kernel<16>, smem, &c16))) return rc; CB_CUDA(launch_pdl(tc0::conv0_wgrad_kernel<16>, dim3(grid), dim3(tc0::WNLOAD + 32), smem, st, a)); }
+  else { if ((rc = set_smem(tc0::conv0_wgrad_kernel<32>, smem, &c32))) return rc; CB_CUDA(launch_pdl(tc0::conv0_wgrad_kernel<32>, dim3(grid), dim3(tc0::WNLOAD + 32), smem, st, a)); }
   CB_CUDA(cudaGetLastError());
   tc0::conv0_wgrad_reduce_kernel<<<(3 * 24 * g.Cout + 255) / 256, 256, 0, st>>>(partial, grid, g, pm, grad);
   CB_CUDA(cudaGetLastError());

@@ -226,6 +226,8 @@ __global__ void pool_fwd_v8_kernel(const bf16* __restrict__ x, bf16* __restrict_
 // windows is rounded to bf16 after each addition.  The finished band leaves as one linear copy.
 __global__ void __launch_bounds__(256) pool_bwd_scatter_kernel(const uint8_t* __restrict__ arg, const bf16* __restrict__ dy, bf16* __restrict__ dx,
                                                                int F, int C, int H, int W, int RB, int nbands) {
+  asm volatile("griddepcontrol.wait;\n" ::: "memory");      // launched through launch_pdl: resident before its predecessor has drained
+  asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory");
   extern __shared__ __align__(16) uint8_t tile[];
   const int Ho = pool_out(H), Wo = pool_out(W), ph = pool_pad_lo(H), pw = pool_pad_lo(W), C8 = C / 8, tid = threadIdx.x;
   for (int item = blockIdx.x; item < F * nbands; item += gridDim.x) {
@@ -387,7 +389,13 @@ static int forward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int32
     double in_bytes = (double)F * g.H * g.W * g.Cin * (L.u8_in ? 1 : sizeof(AT));
     ProfScope ps(K_CONV_FWD, st, (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && !L.relu_in && dense_tc_supported(g)) ? 2 : 1, 2.0 * M * N * K, in_bytes + (double)M * N * (L.f32_out ? 4 : sizeof(AT)) * (skip ? 2 : 1) + (double)K * N * sizeof(AT));
     int rc;
-    if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out && conv_tc_fits(g.H, g.W, g.Cin, g.Cout)) {
+    const Op* nxt = oi + 1 < net->fwd.size() ? &net->fwd[oi + 1] : nullptr;
+    if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && !L.relu_in && !L.relu_out && !skip && nxt && nxt->kind == OP_POOL && nxt->in_t == L.out_t &&
+        conv_pool_tc_supported(g)) {
+      // a stage conv whose only consumer is the max-pool: one kernel, the conv output never reaches HBM (the adjoint needs only the arg-max)
+      pool_fused = true;
+      rc = launch_conv_pool_tc(g, F, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (bf16*)ws.act[nxt->out_t], (uint8_t*)ws.act[nxt->mask_t], ws.errflag, st);
+    } else if (std::is_same<AT, bf16>::value && conv_tc_supported(g) && !L.f32_out && conv_tc_fits(g.H, g.W, g.Cin, g.Cout)) {
       rc = launch_conv_tc(0, F, g.H, g.W, g.Cin, g.Cout, (const bf16*)ws.act[L.in_t], ws.wtc_f + L.wf_off, bias, (const bf16*)skip, nullptr,
                           (bf16*)ws.act[L.out_t], L.relu_in, L.relu_out, ws.errflag, st);
     } else if (std::is_same<AT, bf16>::value && !L.u8_in && !L.f32_out && !L.relu_in && dense_tc_supported(g)) {
@@ -439,8 +447,8 @@ static int backward_t(cb_net* net, Workspace& ws, const uint8_t* obs, const int3
         const int nb = (op.H + RB - 1) / RB; RB = (op.H + nb - 1) / nb;
         const size_t smem = (size_t)RB * row_bytes;
         if (smem > 48 * 1024) { int rc = ensure_dyn_smem((const void*)pool_bwd_scatter_kernel, smem); if (rc) return rc; }
-        pool_bwd_scatter_kernel<<<std::min(F * nb, 148 * 8), 256, smem, st>>>((const uint8_t*)ws.act[op.mask_t], (const bf16*)ws.grad[op.dy], (bf16*)ws.grad[op.dx],
-                                                                             F, op.C, op.H, op.W, RB, nb);
+        CB_CUDA(launch_pdl(pool_bwd_scatter_kernel, dim3(std::min(F * nb, 148 * 8)), dim3(256), smem, st, (const uint8_t*)ws.act[op.mask_t], (const bf16*)ws.grad[op.dy],
+                           (bf16*)ws.grad[op.dx], F, op.C, op.H, op.W, RB, nb));
       } else
         pool_bwd_kernel<AT><<<grid_for(total), 256, 0, st>>>((const AT*)ws.act[op.in_t], (const AT*)ws.grad[op.dy], (AT*)ws.grad[op.dx], F, op.C, op.H, op.W);
       CB_CUDA(cudaGetLastError());

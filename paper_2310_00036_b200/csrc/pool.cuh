@@ -63,6 +63,60 @@ __device__ __forceinline__ void window_max(const uint4 (&v)[9], uint32_t valid, 
   arg.x = __byte_perm(a[0], a[1], 0x6420); arg.y = __byte_perm(a[2], a[3], 0x6420);
 }
 
+// Bank-conflict-free layout of a conv band kept in shared memory as [row][x][channel] bf16: inside every 64-byte block (a pixel pair at 16
+// channels, one pixel at 32, half a pixel at 64) the 16-byte chunk c sits at c ^ f((block >> 1) & 3).  The lanes of a TMEM-draining warp (64 /
+// 128 bytes apart) and the lanes of a pooling warp (one or two pixels apart) then spread over all eight 16-byte bank groups.  At 16 channels
+// f must swap the two bits (neighbouring pool lanes are ONE block apart); from 32 channels on the identity does (two shift/logic instructions).
+template <int COUT>
+__device__ __forceinline__ uint32_t ct_swz(uint32_t byte_off) {
+  if (COUT == 16) return byte_off ^ (((byte_off >> 2) & 0x20u) | ((byte_off >> 4) & 0x10u));
+  return byte_off ^ ((byte_off >> 3) & 0x30u);
+}
+
+// 3x3 stride-2 SAME max-pool (A10) with first arg-max (A11) over `pr` pooled rows starting at row py0 of frame f, read from the swizzled conv
+// band `ctb` whose first row is conv row yb.  Thread pt of NP; writes the pooled map and the arg-max bytes.
+template <int COUT>
+__device__ __forceinline__ void pool_band(const uint8_t* ctb, int yb, int py0, int pr, int f, int H, int W, int Ho, int Wo, int ph, int pw,
+                                          __nv_bfloat16* __restrict__ pool_out, uint8_t* __restrict__ pool_arg, int pt, int NP) {
+  constexpr int C8 = COUT / 8, LC8 = COUT == 16 ? 1 : (COUT == 32 ? 2 : 3);
+  constexpr uint32_t PIX = COUT * 2;
+  const uint32_t magic_Wo = (uint32_t)((0x100000000ull + (uint64_t)Wo - 1) / (uint64_t)Wo);
+  const uint32_t rowp = (uint32_t)W * PIX;
+  const size_t obase = (size_t)f * Ho * Wo * COUT;
+  const int ntask = pr * Wo * C8;
+  for (int i = pt; i < ntask; i += NP) {
+    const int c8 = i & (C8 - 1), q = i >> LC8, qy = (int)__umulhi((uint32_t)q, magic_Wo), ox = q - qy * Wo, oy = py0 + qy;
+    uint4 v[9]; uint32_t valid = 0;
+    const int iy0 = oy * 2 - ph, ix0 = ox * 2 - pw;
+    if (iy0 >= 0 && iy0 + 2 < H && ix0 >= 0 && ix0 + 2 < W) {      // interior window (all but the border ones): no per-tap predicates
+      const uint32_t base = (uint32_t)((iy0 - yb) * W + ix0) * PIX + (uint32_t)c8 * 16u;
+#pragma unroll
+      for (int di = 0; di < 3; ++di)
+#pragma unroll
+        for (int dj = 0; dj < 3; ++dj) v[di * 3 + dj] = *reinterpret_cast<const uint4*>(ctb + ct_swz<COUT>(base + di * rowp + dj * PIX));
+      valid = 0x1FFu;
+    } else {
+#pragma unroll
+      for (int di = 0; di < 3; ++di) {
+        const int iy = iy0 + di;
+#pragma unroll
+        for (int dj = 0; dj < 3; ++dj) {
+          const int ix = ix0 + dj;
+          if ((unsigned)iy < (unsigned)H && (unsigned)ix < (unsigned)W) {
+            v[di * 3 + dj] = *reinterpret_cast<const uint4*>(ctb + ct_swz<COUT>((uint32_t)((iy - yb) * W + ix) * PIX + (uint32_t)c8 * 16u));
+            valid |= 1u << (di * 3 + dj);
+          }
+        }
+      }
+    }
+    const size_t o = obase + (size_t)((uint32_t)(oy * Wo + ox) * (uint32_t)COUT + (uint32_t)c8 * 8u);
+    uint4 r; uint2 pk;
+    window_max(v, valid, r, pk);
+    *reinterpret_cast<uint4*>(pool_out + o) = r;
+    *reinterpret_cast<uint2*>(pool_arg + o) = pk;
+  }
+}
+
 // loads the compiler may not sink to their first use: issued where written (ahead of a barrier wait), consumed after it
 __device__ __forceinline__ uint32_t ldg_early_u32(const void* p) {
   uint32_t v; asm volatile("ld.global.nc.u32 %0, [%1];\n" : "=r"(v) : "l"(p)); return v;

@@ -50,6 +50,12 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity) {
   }
   return false;
 }
+// Programmatic dependent launch (kernels launched through cb::launch_pdl, common.cuh): a CTA of the NEXT kernel in the stream may start while
+// the previous kernel is still draining and run its private prologue (barrier init, TMEM allocation, shared-memory zero fill); pdl_wait()
+// blocks until every earlier kernel has completed and its writes are visible -- nothing written by an earlier kernel may be read, and no
+// global memory may be written, before it.  pdl_trigger() lets the kernel after this one start its own prologue.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;\n" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;\n" ::: "memory"); }
 __device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }

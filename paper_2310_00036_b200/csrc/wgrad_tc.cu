@@ -140,6 +140,7 @@ __global__ void __launch_bounds__(NLOAD + 64) wgrad3x3_sw_kernel(const WgradSwAr
   }
   // everything outside the landed boxes (slack positions, DY rows below a band) stays zero for the whole kernel
   for (uint32_t i = tid; i < a.stage_bytes * (uint32_t)NS / 16; i += NLOAD + 64) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
+  pdl_wait(); pdl_trigger();      // the prologue above is private to the CTA (tc_ptx.cuh)
   asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
   asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
   __syncthreads();
@@ -312,8 +313,7 @@ static SwPlan sw_plan(int F, int H, int W, int cin, int cout) {
 template <int CIN, int COUT>
 static int launch_sw(const tcw::WgradSwArgs& a, const CUtensorMap& xmap, const CUtensorMap& ymap, size_t smem, int grid, cudaStream_t st) {
   { int rc = ensure_dyn_smem((const void*)tcw::wgrad3x3_sw_kernel<CIN, COUT>, smem); if (rc) return rc; }
-  tcw::wgrad3x3_sw_kernel<CIN, COUT><<<grid, tcw::NLOAD + 64, smem, st>>>(a, xmap, ymap);
-  CB_CUDA(cudaGetLastError());
+  CB_CUDA(launch_pdl(tcw::wgrad3x3_sw_kernel<CIN, COUT>, dim3(grid), dim3(tcw::NLOAD + 64), smem, st, a, xmap, ymap));
   return CB_OK;
 }
 
