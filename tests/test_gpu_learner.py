@@ -692,3 +692,24 @@ def test_no_tma_fallback_kernels():
                          capture_output=True, text=True, timeout=1200)
     assert out.returncode == 0, out.stdout[-3000:] + out.stderr[-2000:]
     assert " passed" in out.stdout
+
+
+def test_learner_ppo_with_rmsprop_and_bad_actions():
+    """cb_hparams.optimizer = 1 under the PPO schedule (reachable through the ABI; oracle: test_ppo_with_rmsprop_follows_the_same_schedule), and
+    out-of-range actions: clamped by the kernels that index with them (cleanba.h), never read out of bounds."""
+    arch, T, B = TINY_IMPALA, 4, 4
+    hp, ho = _hp_pair("ppo", "fp32", T, B, epochs=1, minibatches=2, optimizer=1)
+    ho.rms_decay, ho.rms_eps = float(hp.rms_decay), float(hp.rms_eps)
+    bt = _batch(arch, T, B, 1070, False)
+    params = synth.gen_params(arch, 1071, bias_scale=0.05, head_scale=0.1); P = params.size
+    nu = (synth.rng(1072).random(P) * 1e-5 + 1e-6).astype(np.float32); z = np.zeros(P, np.float32)
+    net = binding.Net(arch); dp, dm, dv = dev(params), dev(z), dev(nu)
+    args = [dev(bt[k]) for k in ("obs", "actions", "rewards", "dones", "behaviour_logits")]
+    k1, stats = net.learner_step(dp, dm, dv, 10, *args, hp); net.check_errors()
+    ref = oracle.learner_step(orc_arch(arch), ho, params, z, nu, 10, bt["obs"], bt["actions"], bt["rewards"], bt["dones"], bt["behaviour_logits"])
+    assert k1 == ref["opt_step"] == 12 and not host(dm).any()
+    assert rel_l2(host(dp), ref["params"]) < 1e-4 and rel_l2(host(dv), ref["v"]) < 1e-3
+    bad = bt["actions"].copy(); bad[0, 0] = 1000; bad[1, 1] = -7
+    net2 = binding.Net(arch); dp2 = dev(params)
+    _, st2 = net2.learner_step(dp2, dev(z), dev(nu), 10, args[0], dev(bad), *args[2:], hp); net2.check_errors()
+    assert np.isfinite(host(st2)).all() and np.isfinite(host(dp2)).all()
