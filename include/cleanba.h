@@ -200,6 +200,13 @@ int cb_ppo_loss(int m, int A, const float* head, const int32_t* idx, const int32
 int cb_permutation(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* stream);
 /* The same with caller-provided scratch (dev uint32 [N]), so that no allocation happens inside the call. */
 int cb_permutation_ws(uint64_t seed, uint32_t epoch, int N, int32_t* perm, uint32_t* scratch, void* stream);
+/* The same for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the scratch
+ * is a static device array of CB_PERM_STATIC_MAX draws (256 KiB held by every GPU that loads the library, until exit); the call
+ * performs no cudaMalloc / cudaFree.  perm: dev int32 [N], written; N > CB_PERM_STATIC_MAX -> CB_EINVAL (use cb_permutation_ws).
+ * All calls on a device share the array: calls that overlap on the GPU (other streams, concurrent graph replays) race; calls
+ * ordered on one stream are safe, and no state carries from one call to the next (every draw is written before it is read). */
+#define CB_PERM_STATIC_MAX 65536
+int cb_permutation_static(uint64_t seed, uint32_t epoch, int N, int32_t* perm, void* stream);
 /* O9 (A12, A13): global-norm clip + Adam over flat fp32 buffers of P elements (16-byte aligned);
  * k = update count (from 1).  grad_norm: dev fp32 [1], written (pre-clip norm; nullable).
  * scratch: dev, at least cb_clip_adam_scratch_bytes(P) bytes. */

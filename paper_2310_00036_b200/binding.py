@@ -21,7 +21,7 @@ EXPORTS = ["cb_net_create", "cb_net_destroy", "cb_param_count", "cb_param_layout
            "cb_permutation", "cb_clip_adam_scratch_bytes", "cb_clip_adam", "cb_last_error",
            "cb_launch_count", "cb_profile_begin", "cb_profile_end", "cb_clip_rmsprop", "cb_linear_lr",
            "cb_learner_begin", "cb_learner_grad", "cb_learner_apply", "cb_sum_ranks", "cb_check_errors",
-           "cb_debug_inject_timeout", "cb_permutation_ws",
+           "cb_debug_inject_timeout", "cb_permutation_ws", "cb_permutation_static",
            "cb_pipeline_create", "cb_pipeline_destroy", "cb_pipeline_run", "cb_pipeline_wait", "cb_pipeline_state", "cb_pipeline_records",
            "cb_pipeline_rollout", "cb_pipeline_policy_version", "cb_env_state_ints", "cb_env_reset", "cb_env_step",
            "cb_loss_scratch_bytes", "cb_impala_loss", "cb_ppo_loss"]
@@ -422,6 +422,19 @@ def permutation(seed, epoch, N):
     torch = _torch()
     perm = torch.empty((N,), dtype=torch.int32, device="cuda")
     _check(lib().cb_permutation(C.c_uint64(seed), C.c_uint32(epoch), C.c_int(N), _ptr(perm), _stream()))
+    return perm
+
+
+PERM_STATIC_MAX = 65536      # CB_PERM_STATIC_MAX
+
+
+def permutation_static(seed, epoch, N, out=None):
+    """cb_permutation_static: no allocation inside the call (static device scratch, N <= PERM_STATIC_MAX).  `out`: a caller-owned
+    int32 [N] device tensor; without it one is allocated HERE, by torch, before the call."""
+    torch = _torch()
+    perm = out if out is not None else torch.empty((N,), dtype=torch.int32, device="cuda")
+    assert perm.dtype == torch.int32 and perm.numel() >= N and perm.is_contiguous()
+    _check(lib().cb_permutation_static(C.c_uint64(seed), C.c_uint32(epoch), C.c_int(N), _ptr(perm), _stream()))
     return perm
 
 
