@@ -10,6 +10,7 @@ SO = os.path.join(HERE, "libcleanba.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Wno-deprecated-gpu-targets"]
+FLAGS += os.environ.get("CB_NVCC_FLAGS", "").split()      # extra nvcc flags for instrumented / debug builds (-D..., -G, ...)
 
 
 def sources():
